@@ -1,0 +1,221 @@
+// ORACLE -- TEST INFRASTRUCTURE ONLY (see hg_oracle_core.hpp for the rules).
+//
+// C-ABI batch drivers around the scalar oracle functions, loaded by
+// oracle/__init__.py through ctypes.  Inputs are the fp32 problem instance
+// (promoted exactly to fp64); results are fp64.  AoS layouts throughout:
+//   src, dst : float  [n][4][2]   (x,y of points M,N,P,Q)
+//   H        : double [n][3][3]   row-major
+// Batch loops are OpenMP-parallel over independent sets; that is the only
+// parallelism, and nothing is tuned.
+#include "hg_oracle_core.hpp"
+
+#include <cstring>
+#include <omp.h>
+
+namespace {
+
+inline void load_set(const float* p, double o[8])
+{
+    for (int i = 0; i < 8; ++i) o[i] = static_cast<double>(p[i]);
+}
+
+}  // namespace
+
+extern "C" {
+
+int hgo_num_threads(void) { return omp_get_max_threads(); }
+void hgo_set_num_threads(int n) { omp_set_num_threads(n); }
+
+// method: 0 = DLT-GE (h33 = 1), 1 = ACA (raw scale), 2 = SKS, 3 = closed form Eq. 33'
+// ok (nullable): per-set flag, 0 where DLT-GE met a zero pivot (H then holds NaN).
+void hgo_solve(int method, const float* src, const float* dst, double* H, int64_t n, uint8_t* ok)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double s[8], d[8];
+        load_set(src + 8 * i, s);
+        load_set(dst + 8 * i, d);
+        double* Hi = H + 9 * i;
+        bool good = true;
+        switch (method) {
+            case 0: good = hgo::dlt_ge(s, d, Hi); break;
+            case 1: hgo::aca<double>(s, d, Hi); break;
+            case 2: hgo::sks<double>(s, d, Hi); break;
+            default: hgo::closed_form<double>(s, d, Hi); break;
+        }
+        if (!good) for (int k = 0; k < 9; ++k) Hi[k] = NAN;
+        if (ok) ok[i] = good ? 1 : 0;
+    }
+}
+
+// Same with fp64 inputs (used by the exact-integer and homogeneity pins).
+void hgo_solve_f64(int method, const double* src, const double* dst, double* H, int64_t n)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        const double* s = src + 8 * i;
+        const double* d = dst + 8 * i;
+        double* Hi = H + 9 * i;
+        switch (method) {
+            case 0: if (!hgo::dlt_ge(s, d, Hi)) for (int k = 0; k < 9; ++k) Hi[k] = NAN; break;
+            case 1: hgo::aca<double>(s, d, Hi); break;
+            case 2: hgo::sks<double>(s, d, Hi); break;
+            default: hgo::closed_form<double>(s, d, Hi); break;
+        }
+    }
+}
+
+// ACA core parameters c11,c22,c33 (Eq. 32) and SKS kernel parameters aK,bK,uK,vK (Eq. 15).
+void hgo_aca_core(const float* src, const float* dst, double* core3, int64_t n)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        double s[8], d[8], H[9];
+        load_set(src + 8 * i, s);
+        load_set(dst + 8 * i, d);
+        hgo::aca<double>(s, d, H, core3 + 3 * i);
+    }
+}
+void hgo_sks_kernel(const float* src, const float* dst, double* kern4, int64_t n)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        double s[8], d[8], H[9];
+        load_set(src + 8 * i, s);
+        load_set(dst + 8 * i, d);
+        hgo::sks<double>(s, d, H, kern4 + 4 * i);
+    }
+}
+
+// Normal form (unit Frobenius, sign-fixed) in place.
+void hgo_normal_form(double* H, int64_t n)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) hgo::normal_form(H + 9 * i);
+}
+
+// Paper-style operation counts of one evaluation.  method: 1 = ACA, 2 = SKS.
+// out = { add/sub, mul, div, FLOPs = add + mul + 4*div }.
+void hgo_op_counts(int method, int64_t out[4])
+{
+    using hgo::Counted;
+    // any non-degenerate quadrilateral pair
+    const double sv[8] = { 10, 20, 310, 35, 290, 260, 25, 240 };
+    const double dv[8] = { 40, 30, 350, 60, 300, 300, 15, 270 };
+    Counted s[8], d[8], H[9];
+    for (int i = 0; i < 8; ++i) { s[i] = Counted(sv[i]); d[i] = Counted(dv[i]); }
+    Counted::reset();
+    if (method == 1) hgo::aca<Counted>(s, d, H);
+    else             hgo::sks<Counted>(s, d, H);
+    out[0] = Counted::n_add;
+    out[1] = Counted::n_mul;
+    out[2] = Counted::n_div;
+    out[3] = Counted::flops();
+}
+
+// Algorithm 1 (TensorACA-rect).  offsets float [n][4][2] in corner order TL,TR,BR,BL of the
+// source rectangle TL=(x0,y0), extents (w,h); target corner = source corner + offset.
+// Roles per R6: M=TL, N=TR, Q=BR, P=BL.
+void hgo_aca_rect(const float* offsets, float x0, float y0, float w, float h, double* H, int64_t n)
+{
+    const double X0 = x0, Y0 = y0, Wd = w, Hd = h;
+    const double cx[4] = { X0, X0 + Wd, X0 + Wd, X0 };
+    const double cy[4] = { Y0, Y0, Y0 + Hd, Y0 + Hd };
+    for (int64_t i = 0; i < n; ++i) {
+        double t[4][2];
+        for (int k = 0; k < 4; ++k) {
+            t[k][0] = cx[k] + static_cast<double>(offsets[8 * i + 2 * k]);
+            t[k][1] = cy[k] + static_cast<double>(offsets[8 * i + 2 * k + 1]);
+        }
+        hgo::aca_rect<double>(X0, Y0, Wd, Wd / Hd, t[0], t[1], t[3], t[2], H + 9 * i);
+    }
+}
+
+// Offsets -> H -> dense grid (reading R10).  General ACA on corners in API order
+// (M,N,P,Q = TL,TR,BR,BL), then grid[b][j][i] = pi(H_b * (x_i, y_j, 1)) with
+// x_i = x0 + i*w/(grid_w-1), y_j = y0 + j*h/(grid_h-1) (x_i = x0 when grid_w == 1).
+// H_out (nullable) double [n][9] raw scale; grid (nullable) double [n][grid_h][grid_w][2].
+void hgo_offsets_to_grid(const float* offsets, float x0, float y0, float w, float h,
+                         int32_t grid_w, int32_t grid_h, double* H_out, double* grid, int64_t n)
+{
+    const double X0 = x0, Y0 = y0, Wd = w, Hd = h;
+    const double s[8] = { X0, Y0, X0 + Wd, Y0, X0 + Wd, Y0 + Hd, X0, Y0 + Hd };
+#pragma omp parallel for schedule(static)
+    for (int64_t b = 0; b < n; ++b) {
+        double d[8], H[9];
+        for (int k = 0; k < 8; ++k) d[k] = s[k] + static_cast<double>(offsets[8 * b + k]);
+        hgo::aca<double>(s, d, H);
+        if (H_out) std::memcpy(H_out + 9 * b, H, sizeof(H));
+        if (!grid) continue;
+        double* g = grid + static_cast<int64_t>(2) * grid_w * grid_h * b;
+        for (int32_t j = 0; j < grid_h; ++j) {
+            const double y = (grid_h > 1) ? Y0 + j * Hd / (grid_h - 1) : Y0;
+            for (int32_t i = 0; i < grid_w; ++i) {
+                const double x = (grid_w > 1) ? X0 + i * Wd / (grid_w - 1) : X0;
+                const double X = H[0] * x + H[1] * y + H[2];
+                const double Y = H[3] * x + H[4] * y + H[5];
+                const double W = H[6] * x + H[7] * y + H[8];
+                g[2 * (static_cast<int64_t>(j) * grid_w + i) + 0] = X / W;
+                g[2 * (static_cast<int64_t>(j) * grid_w + i) + 1] = Y / W;
+            }
+        }
+    }
+}
+
+// RANSAC hypothesise-and-score (reading R9).
+//   src_xy, dst_xy : float [n_pts][2];  hyp_idx : int32 [n_hyp][4]
+//   solver: 1 = ACA-fp64 (the parity reference), 0 = DLT-GE (cross-check)
+//   counts[h]      = #{ k : r_k <= t },  r_k = forward transfer residual in fp64, W == 0 -> outlier
+//   band_counts[h] = #{ k : |r_k - t| <= band_rel * t }   (the allowance of north_star)
+//   best: max count, ties -> lowest hypothesis index; best_H = that H in normal form.
+void hgo_ransac(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                const int32_t* hyp_idx, int64_t n_hyp, double t, double band_rel, int solver,
+                int32_t* counts, int32_t* band_counts,
+                double* best_H, int64_t* best_index, int32_t* best_count)
+{
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t hI = 0; hI < n_hyp; ++hI) {
+        double s[8], d[8], H[9];
+        for (int k = 0; k < 4; ++k) {
+            const int32_t j = hyp_idx[4 * hI + k];
+            s[2 * k] = src_xy[2 * j];     s[2 * k + 1] = src_xy[2 * j + 1];
+            d[2 * k] = dst_xy[2 * j];     d[2 * k + 1] = dst_xy[2 * j + 1];
+        }
+        bool good = true;
+        if (solver == 0) good = hgo::dlt_ge(s, d, H);
+        else             hgo::aca<double>(s, d, H);
+        int32_t c = 0, bc = 0;
+        if (good) {
+            for (int32_t k = 0; k < n_pts; ++k) {
+                const double r = hgo::transfer_residual(H, src_xy[2 * k], src_xy[2 * k + 1],
+                                                        dst_xy[2 * k], dst_xy[2 * k + 1]);
+                if (r <= t) ++c;
+                if (std::fabs(r - t) <= band_rel * t) ++bc;
+            }
+        }
+        counts[hI] = c;
+        if (band_counts) band_counts[hI] = bc;
+    }
+    int64_t bi = -1;
+    int32_t bcnt = -1;
+    for (int64_t hI = 0; hI < n_hyp; ++hI)
+        if (counts[hI] > bcnt) { bcnt = counts[hI]; bi = hI; }
+    if (best_index) *best_index = bi;
+    if (best_count) *best_count = bcnt;
+    if (best_H && bi >= 0) {
+        double s[8], d[8];
+        for (int k = 0; k < 4; ++k) {
+            const int32_t j = hyp_idx[4 * bi + k];
+            s[2 * k] = src_xy[2 * j];     s[2 * k + 1] = src_xy[2 * j + 1];
+            d[2 * k] = dst_xy[2 * j];     d[2 * k + 1] = dst_xy[2 * j + 1];
+        }
+        hgo::aca<double>(s, d, best_H);
+        hgo::normal_form(best_H);
+    }
+}
+
+// Residuals of one H against all correspondences (used by tests to look at single pairs).
+void hgo_residuals(const double* H, const float* src_xy, const float* dst_xy, int32_t n_pts, double* r)
+{
+    for (int32_t k = 0; k < n_pts; ++k)
+        r[k] = hgo::transfer_residual(H, src_xy[2 * k], src_xy[2 * k + 1], dst_xy[2 * k], dst_xy[2 * k + 1]);
+}
+
+}  // extern "C"

@@ -1,0 +1,178 @@
+/*
+ * hg.h -- C ABI of libhg: batched minimal 4-point homography on one B200 (sm_100a).
+ *
+ * Implements the data-parallel hot path of arXiv 2402.18008 ("Fast and Interpretable 2D
+ * Homography Decomposition: SKS and ACA transformations"); "P:<line>" cites
+ * /root/reference/PAPER.md.  One 3x3 homography H (up to scale) is computed from each set of
+ * four point correspondences {M,N,P,Q}_1 -> {M,N,P,Q}_2 (Eq. 1), for millions of
+ * sets per call (Sec. 6.4: "each 4-point homography is assigned to one thread").
+ *
+ * Conventions shared by every entry point
+ * ---------------------------------------
+ *  - Every pointer is a DEVICE pointer owned by the caller unless the name ends in `_host`
+ *    (those entry points take HOST pointers, pinned or pageable, and do the copies themselves).
+ *  - The library keeps no state and allocates no device memory (the `_host` entry points
+ *    allocate and free their own staging buffers and streams inside the call).
+ *  - Device entry points only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as void*;
+ *    NULL = the legacy default stream) and never synchronise; `_host` entry points return
+ *    after their result is complete in host memory.
+ *  - Return value: HG_OK (0) or a negative hg_status_t.  No exceptions, no errno.
+ *    n == 0 (or n_hyp == 0) is HG_OK and a no-op.  Numerical conditions are never errors:
+ *    a degenerate set (three collinear points on either plane) yields ACA's finite singular H
+ *    and SKS's non-finite H (reading R8).
+ *  - Point roles (reading R11): points 0,1,2,3 of a set are M,N,P,Q; ACA uses
+ *    M,N,P as anchors, SKS uses M,N.
+ *  - H is row-major h11,h12,h13,h21,...,h33 and defined up to scale; its sign is never fixed.
+ */
+#ifndef HG_H_
+#define HG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define HG_API __attribute__((visibility("default")))
+#else
+#define HG_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    HG_OK = 0,
+    HG_ERR_INVALID_ARG = -1, /* NULL pointer with n > 0, negative size, unknown enum value        */
+    HG_ERR_ALIGNMENT   = -2, /* a base pointer is not 16-byte aligned                             */
+    HG_ERR_CUDA        = -3, /* a CUDA runtime call or kernel launch failed                       */
+    HG_ERR_WORKSPACE   = -4  /* workspace_bytes < hg_ransac_workspace_bytes(...)                  */
+} hg_status_t;
+
+/* Memory layout of the point sets and of H.
+ *   HG_SOA: src/dst = float[8][n]  planes x0,y0,x1,y1,x2,y2,x3,y3 (plane stride n);
+ *           H       = float[9][n]  planes h11,h12,h13,h21,...,h33.
+ *           The streaming layout: every warp access is a full 128-byte line.
+ *   HG_AOS: src/dst = float[n][4][2];  H = float[n][3][3] row-major.                              */
+typedef enum { HG_SOA = 0, HG_AOS = 1 } hg_layout_t;
+
+/* Scale of the returned H.
+ *   HG_NORM_NONE:      the method's raw scale (ACA: Eq. 31-32; SKS: Eq. 11/16).  The
+ *                      raw ACA H is a degree-7..9 polynomial of the inputs (Eq. 35),
+ *                      about 1e23 for 640x480 coordinates: it overflows fp32 for |coords| >~ 1e4.
+ *   HG_NORM_H33:       H / h33 (the 12-FLOP normalisation of P:301; h33 == 0 gives inf/NaN).
+ *   HG_NORM_FROBENIUS: H / ||H||_F (overflow-safe).                                               */
+typedef enum { HG_NORM_NONE = 0, HG_NORM_H33 = 1, HG_NORM_FROBENIUS = 2 } hg_norm_t;
+
+/* Arithmetic used between the fp32 loads and the fp32 stores.
+ *   HG_PREC_F64: inputs promoted exactly to fp64, the whole solve and the normalisation in fp64,
+ *                H rounded to fp32 once.  Meets the parity tolerances; the default everywhere.
+ *   HG_PREC_F32: plain fp32 (FMA-contracted).  Cancellation in c11-c33, c22-c33 makes h31,h32
+ *                inaccurate for near-affine H; provided for measurement and for callers that
+ *                accept ~1e-3 relative error.                                                     */
+typedef enum { HG_PREC_F64 = 0, HG_PREC_F32 = 1 } hg_precision_t;
+
+/* --------------------------------------------------------------------------------------------
+ * hg_aca_batched -- Affine-Core-Affine solve, H = H_A2^-1 * H_C * H_A1 (Sec. 4.2-4.4,
+ * Eq. 23-32, Table 4): 85 FLOPs and no division per homography before
+ * normalisation.
+ *   src, dst : n source / target 4-point sets in `layout`            (read,  64 B per set)
+ *   H        : n homographies in `layout`, scaled per `norm`         (write, 36 B per set)
+ *   n        : number of sets, >= 0.  HG_SOA planes have stride n; n need not be a multiple of 4
+ *              (the 128-bit fast path needs n % 4 == 0, otherwise a scalar-load path is used).
+ * Errors: HG_ERR_INVALID_ARG (NULL with n > 0, n < 0, bad enum), HG_ERR_ALIGNMENT (src, dst or H
+ * not 16-byte aligned), HG_ERR_CUDA (launch failure).
+ * -------------------------------------------------------------------------------------------- */
+HG_API int hg_aca_batched(const float* src, const float* dst, float* H, int64_t n,
+                   hg_layout_t layout, hg_norm_t norm, hg_precision_t prec, void* cuda_stream);
+
+/* hg_sks_batched -- Similarity-Kernel-Similarity solve, H = H_S2^-1 * H_K * H_S1 with
+ * H_K = H_E^-1 * H_S' * H_E (Sec. 3.1-3.4, Eq. 6-16, Table 3): five reciprocals per
+ * homography.  Arguments, layouts and errors exactly as hg_aca_batched.                          */
+HG_API int hg_sks_batched(const float* src, const float* dst, float* H, int64_t n,
+                   hg_layout_t layout, hg_norm_t norm, hg_precision_t prec, void* cuda_stream);
+
+/* Host-buffer forms of the two solves (the end-to-end path of bench.py): src/dst/H are HOST
+ * pointers in `layout`.  The call splits the batch into chunks and pipelines host->device
+ * copies, the solve kernel and device->host copies on internal streams, then waits.  Copies are
+ * asynchronous only if the host buffers are page-locked.  `chunk_sets` = sets per chunk
+ * (0 = library default).  Extra error: HG_ERR_CUDA if staging memory cannot be allocated.        */
+HG_API int hg_aca_batched_host(const float* src_host, const float* dst_host, float* H_host, int64_t n,
+                        hg_layout_t layout, hg_norm_t norm, hg_precision_t prec,
+                        int64_t chunk_sets);
+HG_API int hg_sks_batched_host(const float* src_host, const float* dst_host, float* H_host, int64_t n,
+                        hg_layout_t layout, hg_norm_t norm, hg_precision_t prec,
+                        int64_t chunk_sets);
+
+/* --------------------------------------------------------------------------------------------
+ * hg_offsets_to_grid -- the deep-homography use (4-point parameterisation, P:25, P:131,
+ * P:540-544): for each item, target corners = source-rectangle corners + predicted offsets,
+ * H by ACA, then (fused, same kernel) the dense sampling grid of H over the patch
+ * (reading R10: grid[b][j][i] = pi(H_b * (x_i, y_j, 1)), forward map, pixel units).
+ *   offsets : float[n][4][2], corner order TL,TR,BR,BL                (read, 32 B per item)
+ *   x0,y0,w,h : source rectangle: TL corner (x0,y0), extents w,h (C1/C5: 0,0,127,127).
+ *               Requires w != 0 and h != 0.
+ *   grid_w, grid_h : pixels per row / rows; x_i = x0 + i*w/(grid_w-1) (x0 if grid_w == 1),
+ *               y_j likewise (C5: 128,128 -> integer pixels 0..127).  Ignored if grid == NULL.
+ *   H       : nullable, float[n][3][3], scaled per `norm`              (write, 36 B per item)
+ *   grid    : nullable, float[n][grid_h][grid_w][2], (x,y) order       (write, 8 B per pixel)
+ * The solve is always fp64-internal.  Errors: HG_ERR_INVALID_ARG (offsets NULL with n > 0,
+ * both outputs NULL is allowed and a no-op, grid != NULL with grid_w < 1 or grid_h < 1, w == 0
+ * or h == 0, n < 0), HG_ERR_ALIGNMENT (offsets/grid not 16-byte aligned, H not 4-byte aligned),
+ * HG_ERR_CUDA.
+ * -------------------------------------------------------------------------------------------- */
+HG_API int hg_offsets_to_grid(const float* offsets, float x0, float y0, float w, float h,
+                       int32_t grid_w, int32_t grid_h, float* H, float* grid, int64_t n,
+                       hg_norm_t norm, void* cuda_stream);
+
+/* --------------------------------------------------------------------------------------------
+ * hg_ransac_hypothesize_score -- RANSAC hypothesis generation fused with inlier scoring
+ * (hypothesise-and-verify loop, Sec. 2.2; parallel hypotheses P:703).
+ * For every hypothesis: gather its 4 correspondences, ACA solve (fp64 internal), then count
+ * the correspondences whose forward transfer error ||pi(H*s) - d||_2 <= threshold_px
+ * (reading R9: inclusive, W == 0 -> outlier, no degeneracy test, no local optimisation).
+ * Scoring runs in fp32 with a per-hypothesis rigorous error band; every pair that falls inside
+ * the band is re-decided in fp64, so counts equal an fp64 evaluation.
+ *   src_xy, dst_xy : float[n_pts][2] correspondences                  (read)
+ *   hyp_idx        : int32[n_hyp][4], the 4 indices of a row distinct and in [0,n_pts)
+ *                    (out-of-range indices are undefined behaviour)   (read, 16 B per hyp.)
+ *   threshold_px   : t > 0
+ *   counts         : nullable, int32[n_hyp] inlier count per hypothesis (write, 4 B per hyp.)
+ *   best_H         : nullable, float[9] row-major unit-Frobenius H of the best hypothesis
+ *   best_index     : nullable, int64: argmax of counts, ties -> lowest hypothesis index
+ *   best_count     : nullable, int32: its count
+ *   workspace      : device scratch of >= hg_ransac_workspace_bytes(n_pts, n_hyp) bytes,
+ *                    16-byte aligned; contents undefined before and after the call.
+ * Errors: HG_ERR_INVALID_ARG (NULL inputs, n_pts < 4, n_hyp < 0, threshold not > 0),
+ * HG_ERR_ALIGNMENT, HG_ERR_WORKSPACE, HG_ERR_CUDA.
+ * -------------------------------------------------------------------------------------------- */
+HG_API size_t hg_ransac_workspace_bytes(int32_t n_pts, int64_t n_hyp);
+HG_API int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                                const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
+                                int32_t* counts, float* best_H, int64_t* best_index,
+                                int32_t* best_count, void* workspace, size_t workspace_bytes,
+                                void* cuda_stream);
+
+/* After hg_ransac_hypothesize_score has completed on its stream, the first 4 int64 words of
+ * the workspace hold statistics of that call (device memory; copy them out to read):
+ *   [0] packed best key, [1] number of hypotheses re-scored by the fp64 fix-up pass,
+ *   [2] number of (hypothesis, point) pairs decided in fp64, [3] reserved.                      */
+#define HG_RANSAC_STAT_WORDS 4
+
+/* Host-buffer form: all pointers are HOST pointers; the call allocates device memory and the
+ * workspace, copies in, runs, copies counts/best out and waits.                                  */
+HG_API int hg_ransac_hypothesize_score_host(const float* src_xy_host, const float* dst_xy_host,
+                                     int32_t n_pts, const int32_t* hyp_idx_host, int64_t n_hyp,
+                                     float threshold_px, int32_t* counts_host, float* best_H_host,
+                                     int64_t* best_index_host, int32_t* best_count_host);
+
+/* Human-readable name of a status code (static storage, never NULL). */
+HG_API const char* hg_status_string(int status);
+
+/* Library version (major*10000 + minor*100 + patch) and the SM architecture it was built for. */
+HG_API int hg_version(void);
+HG_API int hg_built_for_sm(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HG_H_ */

@@ -1,0 +1,274 @@
+"""paper_2402_18008_b200 -- thin Python binding of libhg (include/hg.h).
+
+Batched minimal 4-point homography by the ACA and SKS decompositions of arXiv 2402.18008 on one
+B200.  Every function below only marshals arguments (torch tensors -> device pointers, the
+current CUDA stream -> ``cuda_stream``) and calls the C entry point of the same name; all
+arithmetic runs in the hand-written sm_100a kernels of ``csrc/``.  There is no CPU or PyTorch
+fallback: if ``libhg.so`` cannot be built/loaded, or a tensor is not where the entry point expects
+it, the call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import torch
+
+from . import _build
+
+__all__ = [
+    "HgError", "lib", "lib_path", "SOA", "AOS", "NORM_NONE", "NORM_H33", "NORM_FROBENIUS",
+    "PREC_F64", "PREC_F32", "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host",
+    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_ransac_workspace_bytes",
+    "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_status_string",
+    "hg_version", "hg_built_for_sm", "EXPORTS",
+]
+
+# include/hg.h enums
+HG_OK = 0
+SOA, AOS = 0, 1
+NORM_NONE, NORM_H33, NORM_FROBENIUS = 0, 1, 2
+PREC_F64, PREC_F32 = 0, 1
+RANSAC_STAT_WORDS = 4
+
+# every symbol include/hg.h declares
+EXPORTS = [
+    "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
+    "hg_offsets_to_grid", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
+    "hg_ransac_hypothesize_score_host", "hg_status_string", "hg_version", "hg_built_for_sm",
+]
+
+
+class HgError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = int(status)
+        super().__init__("%s failed: %s (%d)" % (where, hg_status_string(status), status))
+
+
+_lib = None
+_c_int, _c_i32, _c_i64, _c_f32 = ctypes.c_int, ctypes.c_int32, ctypes.c_int64, ctypes.c_float
+_vp = ctypes.c_void_p
+
+
+def lib_path() -> Path:
+    return _build.LIB
+
+
+def lib() -> ctypes.CDLL:
+    """Load libhg.so (building it with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(str(path))
+        solve_args = [_vp, _vp, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
+        L.hg_aca_batched.argtypes = solve_args
+        L.hg_sks_batched.argtypes = solve_args
+        host_args = [_vp, _vp, _vp, _c_i64, _c_int, _c_int, _c_int, _c_i64]
+        L.hg_aca_batched_host.argtypes = host_args
+        L.hg_sks_batched_host.argtypes = host_args
+        L.hg_offsets_to_grid.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _c_i32, _c_i32, _vp, _vp,
+                                         _c_i64, _c_int, _vp]
+        L.hg_ransac_workspace_bytes.argtypes = [_c_i32, _c_i64]
+        L.hg_ransac_workspace_bytes.restype = ctypes.c_size_t
+        L.hg_ransac_hypothesize_score.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp,
+                                                  _vp, ctypes.c_size_t, _vp]
+        L.hg_ransac_hypothesize_score_host.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp]
+        L.hg_status_string.argtypes = [_c_int]
+        L.hg_status_string.restype = ctypes.c_char_p
+        for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
+                     "hg_offsets_to_grid", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host",
+                     "hg_version", "hg_built_for_sm"):
+            getattr(L, name).restype = _c_int
+        _lib = L
+    return _lib
+
+
+def hg_status_string(status: int) -> str:
+    return lib().hg_status_string(int(status)).decode()
+
+
+def hg_version() -> int:
+    return int(lib().hg_version())
+
+
+def hg_built_for_sm() -> int:
+    return int(lib().hg_built_for_sm())
+
+
+# ---- argument marshalling -----------------------------------------------------------------------
+def _ptr(t, dtype, device_type: str, name: str):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor):
+        raise TypeError("%s must be a torch.Tensor" % name)
+    if t.dtype != dtype:
+        raise TypeError("%s must be %s, got %s" % (name, dtype, t.dtype))
+    if t.device.type != device_type:
+        raise ValueError("%s must live on %s, got %s (no fallback path exists)" % (name, device_type, t.device))
+    if not t.is_contiguous():
+        raise ValueError("%s must be contiguous" % name)
+    return _vp(t.data_ptr())
+
+
+def _stream(stream=None):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return _vp(int(stream.cuda_stream))
+
+
+def _check(status: int, where: str):
+    if status != HG_OK:
+        raise HgError(status, where)
+
+
+def _n_sets(src: torch.Tensor, layout: int) -> int:
+    if layout == SOA:
+        if src.dim() != 2 or src.shape[0] != 8:
+            raise ValueError("SoA point sets are float32 [8, n]")
+        return int(src.shape[1])
+    if src.dim() != 3 or tuple(src.shape[1:]) != (4, 2):
+        raise ValueError("AoS point sets are float32 [n, 4, 2]")
+    return int(src.shape[0])
+
+
+def _h_shape(n: int, layout: int):
+    return (9, n) if layout == SOA else (n, 3, 3)
+
+
+def _solve(fn_name: str, src, dst, H, layout, norm, prec, stream):
+    n = _n_sets(src, layout)
+    if tuple(dst.shape) != tuple(src.shape):
+        raise ValueError("src and dst shapes differ")
+    if H is None:
+        H = torch.empty(_h_shape(n, layout), dtype=torch.float32, device=src.device)
+    elif tuple(H.shape) != _h_shape(n, layout):
+        raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
+    fn = getattr(lib(), fn_name)
+    ps, pd, ph = (_ptr(src, torch.float32, "cuda", "src"), _ptr(dst, torch.float32, "cuda", "dst"),
+                  _ptr(H, torch.float32, "cuda", "H"))
+    with torch.cuda.device(src.device):
+        st = fn(ps, pd, ph, n, int(layout), int(norm), int(prec), _stream(stream))
+    _check(st, fn_name)
+    return H
+
+
+def hg_aca_batched(src, dst, H=None, layout: int = SOA, norm: int = NORM_NONE, prec: int = PREC_F64,
+                   stream=None) -> torch.Tensor:
+    """ACA solve of n sets on the current device/stream.  SoA: src, dst [8,n] -> H [9,n];
+    AoS: [n,4,2] -> [n,3,3].  Returns H (allocated if not given).  Asynchronous."""
+    return _solve("hg_aca_batched", src, dst, H, layout, norm, prec, stream)
+
+
+def hg_sks_batched(src, dst, H=None, layout: int = SOA, norm: int = NORM_NONE, prec: int = PREC_F64,
+                   stream=None) -> torch.Tensor:
+    """SKS solve; same contract as hg_aca_batched."""
+    return _solve("hg_sks_batched", src, dst, H, layout, norm, prec, stream)
+
+
+def _solve_host(fn_name: str, src, dst, H, layout, norm, prec, chunk_sets):
+    n = _n_sets(src, layout)
+    if tuple(dst.shape) != tuple(src.shape):
+        raise ValueError("src and dst shapes differ")
+    if H is None:
+        H = torch.empty(_h_shape(n, layout), dtype=torch.float32, pin_memory=True)
+    elif tuple(H.shape) != _h_shape(n, layout):
+        raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
+    st = getattr(lib(), fn_name)(_ptr(src, torch.float32, "cpu", "src"), _ptr(dst, torch.float32, "cpu", "dst"),
+                                 _ptr(H, torch.float32, "cpu", "H"), n, int(layout), int(norm), int(prec),
+                                 int(chunk_sets))
+    _check(st, fn_name)
+    return H
+
+
+def hg_aca_batched_host(src, dst, H=None, layout: int = SOA, norm: int = NORM_NONE, prec: int = PREC_F64,
+                        chunk_sets: int = 0) -> torch.Tensor:
+    """Host-buffer ACA solve (CPU tensors, ideally pinned): chunked H2D -> kernel -> D2H pipeline
+    inside the library on the current CUDA device.  Synchronous."""
+    return _solve_host("hg_aca_batched_host", src, dst, H, layout, norm, prec, chunk_sets)
+
+
+def hg_sks_batched_host(src, dst, H=None, layout: int = SOA, norm: int = NORM_NONE, prec: int = PREC_F64,
+                        chunk_sets: int = 0) -> torch.Tensor:
+    return _solve_host("hg_sks_batched_host", src, dst, H, layout, norm, prec, chunk_sets)
+
+
+def hg_offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w: int, grid_h: int,
+                       want_H: bool = True, want_grid: bool = True, H=None, grid=None,
+                       norm: int = NORM_H33, stream=None):
+    """offsets float32 [n,4,2] (corners TL,TR,BR,BL) -> (H [n,3,3] or None, grid [n,grid_h,grid_w,2] or None)."""
+    if offsets.dim() != 3 or tuple(offsets.shape[1:]) != (4, 2):
+        raise ValueError("offsets are float32 [n, 4, 2]")
+    n = int(offsets.shape[0])
+    po = _ptr(offsets, torch.float32, "cuda", "offsets")
+    if want_H and H is None:
+        H = torch.empty((n, 3, 3), dtype=torch.float32, device=offsets.device)
+    if want_grid and grid is None:
+        grid = torch.empty((n, grid_h, grid_w, 2), dtype=torch.float32, device=offsets.device)
+    if H is not None and tuple(H.shape) != (n, 3, 3):
+        raise ValueError("H must be [n,3,3]")
+    if grid is not None and tuple(grid.shape) != (n, grid_h, grid_w, 2):
+        raise ValueError("grid must be [n,grid_h,grid_w,2]")
+    with torch.cuda.device(offsets.device):
+        st = lib().hg_offsets_to_grid(po, x0, y0, w, h,
+                                      int(grid_w), int(grid_h), _ptr(H, torch.float32, "cuda", "H"),
+                                      _ptr(grid, torch.float32, "cuda", "grid"), n, int(norm), _stream(stream))
+    _check(st, "hg_offsets_to_grid")
+    return H, grid
+
+
+def hg_ransac_workspace_bytes(n_pts: int, n_hyp: int) -> int:
+    return int(lib().hg_ransac_workspace_bytes(int(n_pts), int(n_hyp)))
+
+
+def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, counts=None, workspace=None,
+                                want_counts: bool = True, stream=None):
+    """src_xy, dst_xy float32 [n_pts,2]; hyp_idx int32 [n_hyp,4] (all on the GPU).
+    Returns dict(counts int32 [n_hyp] or None, best_H float32 [3,3], best_index int64 [1],
+    best_count int32 [1], workspace uint8) -- device tensors, produced asynchronously."""
+    n_pts, n_hyp = int(src_xy.shape[0]), int(hyp_idx.shape[0])
+    if tuple(src_xy.shape) != (n_pts, 2) or tuple(dst_xy.shape) != (n_pts, 2):
+        raise ValueError("src_xy, dst_xy are float32 [n_pts, 2]")
+    if tuple(hyp_idx.shape) != (n_hyp, 4):
+        raise ValueError("hyp_idx is int32 [n_hyp, 4]")
+    dev = src_xy.device
+    _ptr(src_xy, torch.float32, "cuda", "src_xy")
+    if want_counts and counts is None:
+        counts = torch.empty((n_hyp,), dtype=torch.int32, device=dev)
+    need = hg_ransac_workspace_bytes(n_pts, n_hyp)
+    if workspace is None:
+        workspace = torch.empty((max(need, 16),), dtype=torch.uint8, device=dev)
+    best_H = torch.empty((3, 3), dtype=torch.float32, device=dev)
+    best_index = torch.empty((1,), dtype=torch.int64, device=dev)
+    best_count = torch.empty((1,), dtype=torch.int32, device=dev)
+    with torch.cuda.device(dev):
+        st = lib().hg_ransac_hypothesize_score(
+            _ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
+            _ptr(hyp_idx, torch.int32, "cuda", "hyp_idx"), n_hyp, float(threshold_px),
+            _ptr(counts, torch.int32, "cuda", "counts"), _ptr(best_H, torch.float32, "cuda", "best_H"),
+            _ptr(best_index, torch.int64, "cuda", "best_index"), _ptr(best_count, torch.int32, "cuda", "best_count"),
+            _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()), _stream(stream))
+    _check(st, "hg_ransac_hypothesize_score")
+    return {"counts": counts, "best_H": best_H, "best_index": best_index, "best_count": best_count,
+            "workspace": workspace}
+
+
+def ransac_stats(workspace: torch.Tensor) -> dict:
+    """Decode the statistics words a finished hg_ransac_hypothesize_score call left in its workspace."""
+    w = workspace[: 8 * RANSAC_STAT_WORDS].cpu().view(torch.int64)
+    return {"best_key": int(w[0]), "n_fixup": int(w[1]), "n_pairs_f64": int(w[2])}
+
+
+def hg_ransac_hypothesize_score_host(src_xy, dst_xy, hyp_idx, threshold_px: float, want_counts: bool = True):
+    """Host-buffer form (CPU tensors in, CPU tensors out); synchronous."""
+    n_pts, n_hyp = int(src_xy.shape[0]), int(hyp_idx.shape[0])
+    counts = torch.empty((n_hyp,), dtype=torch.int32) if want_counts else None
+    best_H = torch.empty((3, 3), dtype=torch.float32)
+    best_index = torch.empty((1,), dtype=torch.int64)
+    best_count = torch.empty((1,), dtype=torch.int32)
+    st = lib().hg_ransac_hypothesize_score_host(
+        _ptr(src_xy, torch.float32, "cpu", "src_xy"), _ptr(dst_xy, torch.float32, "cpu", "dst_xy"), n_pts,
+        _ptr(hyp_idx, torch.int32, "cpu", "hyp_idx"), n_hyp, float(threshold_px),
+        _ptr(counts, torch.int32, "cpu", "counts"), _ptr(best_H, torch.float32, "cpu", "best_H"),
+        _ptr(best_index, torch.int64, "cpu", "best_index"), _ptr(best_count, torch.int32, "cpu", "best_count"))
+    _check(st, "hg_ransac_hypothesize_score_host")
+    return {"counts": counts, "best_H": best_H, "best_index": best_index, "best_count": best_count}

@@ -1,0 +1,493 @@
+// hg_ransac.cu -- hg_ransac_hypothesize_score: RANSAC hypothesis generation fused with inlier
+// scoring (rows a-R0..a-R5 of SURVEY.md section 8(a)).
+//
+// Four launches on the caller's stream, no host synchronisation:
+//   1. prep     : correspondence table -> packed, threshold-folded fp32 table in the workspace
+//                 (+ coordinate bounds for the error band)
+//   2. score    : one thread per hypothesis: gather 4 correspondences, fp64 ACA solve, fold the
+//                 threshold into H, then sweep the whole table from shared memory (staged by
+//                 bulk-async copies / mbarrier) with packed FFMA2 arithmetic, two points per
+//                 instruction.  Counts "surely inlier" and "surely outlier" pairs against a
+//                 rigorous per-hypothesis fp32 error band.
+//   3. fix-up   : hypotheses that had at least one pair inside the band are re-swept by one warp
+//                 each; the in-band pairs are decided in fp64 by the definition (reading R9).
+//   4. finalize : decode the packed (count, index) maximum, re-solve that hypothesis, emit best_H.
+// Compute-bound on the FP32 pipe: 14 packed instructions per two (hypothesis, point) pairs.
+#include "hg_device.cuh"
+#include "hg_host.h"
+
+namespace hg {
+
+constexpr int kRBlock     = 512;    // threads (= hypotheses) per scoring CTA
+constexpr int kChunkPairs = 1024;   // point pairs per shared-memory stage: 1024 * 32 B = 32 KB
+constexpr int kStages     = 2;
+constexpr int kFixBlock   = 256;
+constexpr size_t kHeaderBytes = 64;
+
+struct RansacHeader {               // first 64 bytes of the workspace
+    unsigned long long best_key;    // (count << 32) | (0xFFFFFFFF - hypothesis index)
+    unsigned long long n_fixup;     // length of the fix-up worklist
+    unsigned long long n_pairs_f64; // (hypothesis, point) pairs decided in fp64
+    unsigned long long reserved;
+    unsigned int bound_bits[4];     // float bits of max|sx|, max|sy|, max|dx/t|, max|dy/t|
+    unsigned int pad[4];
+};
+static_assert(sizeof(RansacHeader) == kHeaderBytes, "header layout");
+
+// Per-hypothesis constants of the fp32 sweep.
+struct HypConst {
+    float h[9];     // rows 1,2 of H scaled by 1/(t*max|h|), row 3 by 1/max|h|
+    float K;        // band slope:  |computed - exact| of (ex^2 + ey^2 - W^2) <= K*|W| + K0 whenever it matters
+    float K0;       // band offset
+    float K0x2;
+};
+
+// ---- packed fp32 helpers -------------------------------------------------------------------
+__device__ __forceinline__ float2 f2(float v) { return make_float2(v, v); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 abs2(float2 a) { return make_float2(fabsf(a.x), fabsf(a.y)); }
+
+// Two points against one hypothesis.  Outputs a < 0 <=> surely inlier, nb < 0 <=> surely outlier.
+// ndx, ndy hold -d/t.  14 packed FP32 instructions.
+__device__ __forceinline__ void score2(const HypConst& c, float2 sx, float2 sy, float2 ndx, float2 ndy,
+                                       float2& a, float2& nb)
+{
+    const float2 X = __ffma2_rn(f2(c.h[0]), sx, __ffma2_rn(f2(c.h[1]), sy, f2(c.h[2])));
+    const float2 Y = __ffma2_rn(f2(c.h[3]), sx, __ffma2_rn(f2(c.h[4]), sy, f2(c.h[5])));
+    const float2 W = __ffma2_rn(f2(c.h[6]), sx, __ffma2_rn(f2(c.h[7]), sy, f2(c.h[8])));
+    const float2 ex = __ffma2_rn(ndx, W, X);                     // X/t - (dx/t) W
+    const float2 ey = __ffma2_rn(ndy, W, Y);
+    const float2 w2 = __ffma2_rn(W, W, f2(-c.K0));               // W^2 - K0
+    const float2 p  = __ffma2_rn(ex, ex, neg2(w2));
+    const float2 dp = __ffma2_rn(ey, ey, p);                     // ex^2 + ey^2 - W^2 + K0
+    const float2 aw = abs2(W);
+    a = __ffma2_rn(f2(c.K), aw, dp);                             // diff + (K|W| + K0)
+    const float2 g2 = __ffma2_rn(f2(c.K), aw, f2(c.K0x2));       // K|W| + 2 K0
+    nb = __fadd2_rn(g2, neg2(dp));                               // (K|W| + K0) - diff
+}
+
+__device__ __forceinline__ unsigned sign_bit(float v) { return __float_as_uint(v) >> 31; }
+
+// ---- hypothesis set-up (shared by score, fix-up and finalize) --------------------------------
+__device__ __forceinline__ void gather_sets(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy,
+                                            const int4 id, double s[8], double d[8])
+{
+    const int ids[4] = { id.x, id.y, id.z, id.w };
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float2 sp = __ldg(src_xy + ids[k]);
+        const float2 dq = __ldg(dst_xy + ids[k]);
+        s[2 * k] = sp.x; s[2 * k + 1] = sp.y;
+        d[2 * k] = dq.x; d[2 * k + 1] = dq.y;
+    }
+}
+
+// fp64 ACA solve, max-abs normalisation, threshold folding and the error band.
+// Returns false for an unusable H (all zero or non-finite): such a hypothesis scores 0 (R9: W == 0).
+__device__ __forceinline__ bool make_hypothesis(const double s[8], const double d[8], double inv_t,
+                                                const float bounds[4], double Hn[9], HypConst& c)
+{
+    double H[9];
+    aca_solve<double>(s, d, H);
+    double m = 0.0;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) m = fmax(m, fabs(H[k]));
+    const bool ok = (m > 0.0) && (m < 1.0e300);                  // false for 0, inf, NaN
+    const double r = ok ? K<double>::rcp(m) : 0.0;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) Hn[k] = H[k] * r;
+    const double rt = inv_t;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) c.h[k] = static_cast<float>(Hn[k] * rt);
+#pragma unroll
+    for (int k = 6; k < 9; ++k) c.h[k] = static_cast<float>(Hn[k]);
+    // Error band, u = 2^-24:
+    //   A_r = |h_r1| Sx + |h_r2| Sy + |h_r3|;  c1 = u (3 A1 + 4 Dx A3), c2 = u (3 A2 + 4 Dy A3), eW = 3 u A3
+    //   C = c1 + c2 + eW;  K = 4 C + 16 u A3;  K0 = 32 C^2      (evaluated in fp64, rounded up)
+    const double u = 5.9604644775390625e-08;
+    const double Sx = bounds[0], Sy = bounds[1], Dx = bounds[2], Dy = bounds[3];
+    const double A1 = fabs(double(c.h[0])) * Sx + fabs(double(c.h[1])) * Sy + fabs(double(c.h[2]));
+    const double A2 = fabs(double(c.h[3])) * Sx + fabs(double(c.h[4])) * Sy + fabs(double(c.h[5]));
+    const double A3 = fabs(double(c.h[6])) * Sx + fabs(double(c.h[7])) * Sy + fabs(double(c.h[8]));
+    const double C = u * (3.0 * A1 + 4.0 * Dx * A3) + u * (3.0 * A2 + 4.0 * Dy * A3) + 3.0 * u * A3;
+    const double Kd = (4.0 * C + 16.0 * u * A3) * 1.000001;
+    const double K0d = 32.0 * C * C * 1.000001;
+    c.K = __double2float_ru(Kd);
+    c.K0 = __double2float_ru(K0d);
+    c.K0x2 = 2.0f * c.K0;
+    return ok;
+}
+
+// The definition, in fp64 (reading R9): ||pi(H s) - d||_2 <= t, W == 0 -> outlier.
+__device__ __forceinline__ bool inlier_f64(const double H[9], double sx, double sy, double dx, double dy, double t)
+{
+    const double X = fma(H[0], sx, fma(H[1], sy, H[2]));
+    const double Y = fma(H[3], sx, fma(H[4], sy, H[5]));
+    const double W = fma(H[6], sx, fma(H[7], sy, H[8]));
+    if (W == 0.0) return false;
+    const double ex = X / W - dx, ey = Y / W - dy;
+    return sqrt(fma(ex, ex, ey * ey)) <= t;
+}
+
+// ---- mbarrier / bulk-async copy (TMA 1-D) -----------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{ asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count) : "memory"); }
+__device__ __forceinline__ void fence_barrier_init()
+{ asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{ asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_u32(bar)), "r"(bytes) : "memory"); }
+__device__ __forceinline__ void bulk_copy_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" :: "r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// ---- 1. prep ---------------------------------------------------------------------------------
+// Table entry of point pair k (points 2k, 2k+1; an odd tail point is duplicated):
+//   float4 (sx0, sx1, sy0, sy1), float4 (-dx0/t, -dx1/t, -dy0/t, -dy1/t)
+__global__ void __launch_bounds__(256)
+ransac_prep_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts,
+                   int n_pairs, double inv_t, float4* __restrict__ table, RansacHeader* __restrict__ hdr)
+{
+    float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_pairs; k += gridDim.x * blockDim.x) {
+        const int i0 = 2 * k, i1 = (2 * k + 1 < n_pts) ? 2 * k + 1 : 2 * k;
+        const float2 s0 = __ldg(src_xy + i0), s1 = __ldg(src_xy + i1);
+        const float2 d0 = __ldg(dst_xy + i0), d1 = __ldg(dst_xy + i1);
+        const float4 A = make_float4(s0.x, s1.x, s0.y, s1.y);
+        const float4 B = make_float4(static_cast<float>(-double(d0.x) * inv_t), static_cast<float>(-double(d1.x) * inv_t),
+                                     static_cast<float>(-double(d0.y) * inv_t), static_cast<float>(-double(d1.y) * inv_t));
+        table[2 * k] = A;
+        table[2 * k + 1] = B;
+        m0 = fmaxf(m0, fmaxf(fabsf(A.x), fabsf(A.y)));
+        m1 = fmaxf(m1, fmaxf(fabsf(A.z), fabsf(A.w)));
+        m2 = fmaxf(m2, fmaxf(fabsf(B.x), fabsf(B.y)));
+        m3 = fmaxf(m3, fmaxf(fabsf(B.z), fabsf(B.w)));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, o));
+        m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, o));
+        m2 = fmaxf(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+        m3 = fmaxf(m3, __shfl_xor_sync(0xffffffffu, m3, o));
+    }
+    if ((threadIdx.x & 31) == 0) {       // non-negative floats order like their bit patterns
+        atomicMax(&hdr->bound_bits[0], __float_as_uint(m0));
+        atomicMax(&hdr->bound_bits[1], __float_as_uint(m1));
+        atomicMax(&hdr->bound_bits[2], __float_as_uint(m2));
+        atomicMax(&hdr->bound_bits[3], __float_as_uint(m3));
+    }
+}
+
+// ---- 2. score --------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long pack_key(unsigned count, unsigned index)
+{ return (static_cast<unsigned long long>(count) << 32) | static_cast<unsigned long long>(0xFFFFFFFFu - index); }
+
+__device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
+        v = (w > v) ? w : v;
+    }
+    return v;
+}
+
+__global__ void __launch_bounds__(kRBlock, 2)
+ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts,
+                    const float4* __restrict__ table, int n_pairs, const int4* __restrict__ hyp_idx,
+                    int n_hyp, double inv_t, int* __restrict__ counts, RansacHeader* __restrict__ hdr,
+                    unsigned* __restrict__ worklist)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float4* stage_buf = reinterpret_cast<float4*>(smem_raw);                       // kStages * kChunkPairs * 2 float4
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(kStages) * kChunkPairs * 32);
+
+    const int n_chunks = (n_pairs + kChunkPairs - 1) / kChunkPairs;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+        fence_barrier_init();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int c = 0; c < kStages && c < n_chunks; ++c) {
+            const int pairs = min(kChunkPairs, n_pairs - c * kChunkPairs);
+            mbar_arrive_expect_tx(&full[c], pairs * 32u);
+            bulk_copy_g2s(stage_buf + size_t(c) * kChunkPairs * 2, table + size_t(c) * kChunkPairs * 2, pairs * 32u, &full[c]);
+        }
+    }
+
+    // hypothesis set-up overlaps the first table copies
+    const int hidx = blockIdx.x * kRBlock + threadIdx.x;
+    const bool active = hidx < n_hyp;
+    HypConst hc;
+    bool ok = false;
+    {
+        const float bounds[4] = { __uint_as_float(hdr->bound_bits[0]), __uint_as_float(hdr->bound_bits[1]),
+                                  __uint_as_float(hdr->bound_bits[2]), __uint_as_float(hdr->bound_bits[3]) };
+        double s[8], d[8], Hn[9];
+        const int4 id = active ? __ldg(hyp_idx + hidx) : make_int4(0, 1, 2, 3);
+        gather_sets(src_xy, dst_xy, id, s, d);
+        ok = make_hypothesis(s, d, inv_t, bounds, Hn, hc) && active;
+    }
+
+    unsigned n_in = 0, n_out = 0;
+    const int full_pairs = n_pts >> 1;                     // pairs holding two distinct points
+    for (int c = 0; c < n_chunks; ++c) {
+        const int st = c % kStages;
+        mbar_wait(&full[st], (c / kStages) & 1);
+        const float4* tb = stage_buf + size_t(st) * kChunkPairs * 2;
+        const int first = c * kChunkPairs;
+        const int pairs = min(kChunkPairs, full_pairs - first);          // may be <= 0 in a tail-only chunk
+#pragma unroll 4
+        for (int k = 0; k < pairs; ++k) {
+            const float4 A = tb[2 * k], B = tb[2 * k + 1];
+            float2 a, nb;
+            score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w), a, nb);
+            n_in += sign_bit(a.x) + sign_bit(a.y);
+            n_out += sign_bit(nb.x) + sign_bit(nb.y);
+        }
+        // odd tail point: the duplicated pair counts once
+        if ((n_pts & 1) && full_pairs >= first && full_pairs < first + kChunkPairs) {
+            const int k = full_pairs - first;
+            const float4 A = tb[2 * k], B = tb[2 * k + 1];
+            float2 a, nb;
+            score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w), a, nb);
+            n_in += sign_bit(a.x);
+            n_out += sign_bit(nb.x);
+        }
+        if (c + kStages < n_chunks) {                      // refill this stage (uniform branch)
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                const int cn = c + kStages;
+                const int pn = min(kChunkPairs, n_pairs - cn * kChunkPairs);
+                mbar_arrive_expect_tx(&full[st], pn * 32u);
+                bulk_copy_g2s(stage_buf + size_t(st) * kChunkPairs * 2, table + size_t(cn) * kChunkPairs * 2, pn * 32u, &full[st]);
+            }
+        }
+    }
+
+    // results: exact when no pair fell in the band; otherwise queue for the fix-up pass
+    const bool ambiguous = ok && (n_in + n_out != static_cast<unsigned>(n_pts));
+    const unsigned count = ok ? n_in : 0u;
+    unsigned long long key = 0ull;
+    if (active && !ambiguous) {
+        if (counts) counts[hidx] = static_cast<int>(count);
+        key = pack_key(count, static_cast<unsigned>(hidx));
+    }
+    key = warp_max_u64(key);
+    if ((threadIdx.x & 31) == 0 && key != 0ull) atomicMax(&hdr->best_key, key);
+    const unsigned amb_mask = __ballot_sync(0xffffffffu, ambiguous);
+    if (amb_mask) {
+        const int lane = threadIdx.x & 31;
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(&hdr->n_fixup, static_cast<unsigned long long>(__popc(amb_mask)));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (ambiguous) worklist[base + __popc(amb_mask & ((1u << lane) - 1u))] = static_cast<unsigned>(hidx);
+    }
+}
+
+// ---- 3. fix-up -------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kFixBlock)
+ransac_fixup_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts,
+                    const float4* __restrict__ table, const int4* __restrict__ hyp_idx, double inv_t, double t,
+                    int* __restrict__ counts, RansacHeader* __restrict__ hdr, const unsigned* __restrict__ worklist)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * kFixBlock + threadIdx.x) >> 5;
+    const int n_warps = (gridDim.x * kFixBlock) >> 5;
+    const unsigned long long n_work = hdr->n_fixup;
+    const float bounds[4] = { __uint_as_float(hdr->bound_bits[0]), __uint_as_float(hdr->bound_bits[1]),
+                              __uint_as_float(hdr->bound_bits[2]), __uint_as_float(hdr->bound_bits[3]) };
+    const int full_pairs = n_pts >> 1;
+    for (unsigned long long w = warp; w < n_work; w += n_warps) {
+        const unsigned hidx = worklist[w];
+        HypConst hc;
+        double s[8], d[8], Hn[9];
+        gather_sets(src_xy, dst_xy, __ldg(hyp_idx + hidx), s, d);
+        make_hypothesis(s, d, inv_t, bounds, Hn, hc);
+        unsigned cnt = 0, n64 = 0;
+        const int n_pairs = (n_pts + 1) >> 1;
+        for (int k = lane; k < n_pairs; k += 32) {
+            const float4 A = __ldg(table + 2 * k), B = __ldg(table + 2 * k + 1);
+            float2 a, nb;
+            score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w), a, nb);
+            const bool two = k < full_pairs;
+            // lane .x
+            if (sign_bit(a.x)) ++cnt;
+            else if (!sign_bit(nb.x)) {
+                const float2 sp = __ldg(src_xy + 2 * k), dq = __ldg(dst_xy + 2 * k);
+                cnt += inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, t) ? 1u : 0u;
+                ++n64;
+            }
+            if (two) {
+                if (sign_bit(a.y)) ++cnt;
+                else if (!sign_bit(nb.y)) {
+                    const float2 sp = __ldg(src_xy + 2 * k + 1), dq = __ldg(dst_xy + 2 * k + 1);
+                    cnt += inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, t) ? 1u : 0u;
+                    ++n64;
+                }
+            }
+        }
+        cnt = __reduce_add_sync(0xffffffffu, cnt);
+        n64 = __reduce_add_sync(0xffffffffu, n64);
+        if (lane == 0) {
+            if (counts) counts[hidx] = static_cast<int>(cnt);
+            atomicMax(&hdr->best_key, pack_key(cnt, hidx));
+            atomicAdd(&hdr->n_pairs_f64, static_cast<unsigned long long>(n64));
+        }
+    }
+}
+
+// ---- 4. finalize -----------------------------------------------------------------------------
+__global__ void ransac_finalize_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy,
+                                       const int4* __restrict__ hyp_idx, const RansacHeader* __restrict__ hdr,
+                                       float* __restrict__ best_H, long long* __restrict__ best_index,
+                                       int* __restrict__ best_count)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const unsigned long long key = hdr->best_key;
+    const unsigned idx = 0xFFFFFFFFu - static_cast<unsigned>(key & 0xFFFFFFFFull);
+    if (best_index) *best_index = static_cast<long long>(idx);
+    if (best_count) *best_count = static_cast<int>(key >> 32);
+    if (best_H) {
+        double s[8], d[8], H[9];
+        gather_sets(src_xy, dst_xy, __ldg(hyp_idx + idx), s, d);
+        aca_solve<double>(s, d, H);
+        normalise<double>(H, 2);
+#pragma unroll
+        for (int k = 0; k < 9; ++k) best_H[k] = static_cast<float>(H[k]);
+    }
+}
+
+static size_t align16(size_t v) { return (v + 15) & ~size_t(15); }
+static size_t table_bytes(int32_t n_pts) { return size_t((n_pts + 1) / 2) * 32; }
+
+}  // namespace hg
+
+extern "C" size_t hg_ransac_workspace_bytes(int32_t n_pts, int64_t n_hyp)
+{
+    if (n_pts < 0 || n_hyp < 0) return 0;
+    return hg::kHeaderBytes + hg::align16(hg::table_bytes(n_pts)) + hg::align16(size_t(n_hyp) * sizeof(unsigned));
+}
+
+extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                                           const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
+                                           int32_t* counts, float* best_H, int64_t* best_index,
+                                           int32_t* best_count, void* workspace, size_t workspace_bytes,
+                                           void* cuda_stream)
+{
+    using namespace hg;
+    if (n_hyp < 0 || n_hyp > 0x7fffffffLL) return HG_ERR_INVALID_ARG;
+    if (n_pts < 4) return HG_ERR_INVALID_ARG;
+    if (!(threshold_px > 0.0f) || !(threshold_px < 3.0e38f)) return HG_ERR_INVALID_ARG;
+    if (n_hyp == 0) return HG_OK;
+    if (!src_xy || !dst_xy || !hyp_idx || !workspace) return HG_ERR_INVALID_ARG;
+    if (!aligned16(src_xy) || !aligned16(dst_xy) || !aligned16(hyp_idx) || !aligned16(workspace)) return HG_ERR_ALIGNMENT;
+    if ((counts && !aligned4(counts)) || (best_H && !aligned4(best_H)) ||
+        (best_index && (reinterpret_cast<uintptr_t>(best_index) & 7u)) || (best_count && !aligned4(best_count)))
+        return HG_ERR_ALIGNMENT;
+    if (workspace_bytes < hg_ransac_workspace_bytes(n_pts, n_hyp)) return HG_ERR_WORKSPACE;
+
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    RansacHeader* hdr = reinterpret_cast<RansacHeader*>(ws);
+    float4* table = reinterpret_cast<float4*>(ws + kHeaderBytes);
+    unsigned* worklist = reinterpret_cast<unsigned*>(ws + kHeaderBytes + align16(table_bytes(n_pts)));
+    const float2* s2 = reinterpret_cast<const float2*>(src_xy);
+    const float2* d2 = reinterpret_cast<const float2*>(dst_xy);
+    const int4* idx4 = reinterpret_cast<const int4*>(hyp_idx);
+    const int n_pairs = (n_pts + 1) / 2;
+    const double t = static_cast<double>(threshold_px);
+    const double inv_t = 1.0 / t;
+
+    if (cudaMemsetAsync(hdr, 0, kHeaderBytes, st) != cudaSuccess) return HG_ERR_CUDA;
+    {
+        int blocks = (n_pairs + 255) / 256;
+        if (blocks > 1184) blocks = 1184;
+        ransac_prep_kernel<<<blocks, 256, 0, st>>>(s2, d2, n_pts, n_pairs, inv_t, table, hdr);
+        if (launch_status() != HG_OK) return HG_ERR_CUDA;
+    }
+    {
+        const size_t smem = size_t(kStages) * kChunkPairs * 32 + kStages * sizeof(uint64_t);
+        static bool attr_set = false;          // idempotent; a race only repeats the same call
+        if (!attr_set) {
+            if (cudaFuncSetAttribute(ransac_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
+                return HG_ERR_CUDA;
+            attr_set = true;
+        }
+        const unsigned blocks = static_cast<unsigned>((n_hyp + kRBlock - 1) / kRBlock);
+        ransac_score_kernel<<<blocks, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, idx4, int(n_hyp), inv_t,
+                                                           counts, hdr, worklist);
+        if (launch_status() != HG_OK) return HG_ERR_CUDA;
+    }
+    {
+        int64_t warps = n_hyp;                                   // at most one warp per hypothesis
+        int64_t blocks = (warps * 32 + kFixBlock - 1) / kFixBlock;
+        if (blocks > 148 * 8) blocks = 148 * 8;
+        ransac_fixup_kernel<<<static_cast<unsigned>(blocks), kFixBlock, 0, st>>>(s2, d2, n_pts, table, idx4, inv_t, t,
+                                                                                 counts, hdr, worklist);
+        if (launch_status() != HG_OK) return HG_ERR_CUDA;
+    }
+    if (best_H || best_index || best_count) {
+        ransac_finalize_kernel<<<1, 32, 0, st>>>(s2, d2, idx4, hdr, best_H, reinterpret_cast<long long*>(best_index), best_count);
+        if (launch_status() != HG_OK) return HG_ERR_CUDA;
+    }
+    return HG_OK;
+}
+
+extern "C" int hg_ransac_hypothesize_score_host(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                                                const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
+                                                int32_t* counts, float* best_H, int64_t* best_index,
+                                                int32_t* best_count)
+{
+    using namespace hg;
+    if (n_hyp < 0 || n_hyp > 0x7fffffffLL || n_pts < 4) return HG_ERR_INVALID_ARG;
+    if (n_hyp == 0) return HG_OK;
+    if (!src_xy || !dst_xy || !hyp_idx) return HG_ERR_INVALID_ARG;
+    const size_t pts_b = size_t(n_pts) * 2 * sizeof(float);
+    const size_t idx_b = size_t(n_hyp) * 4 * sizeof(int32_t);
+    const size_t cnt_b = size_t(n_hyp) * sizeof(int32_t);
+    const size_t ws_b = hg_ransac_workspace_bytes(n_pts, n_hyp);
+    // one allocation: src | dst | idx | counts | best (64 B) | workspace, every part 256-byte aligned
+    auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
+    const size_t o_src = 0, o_dst = o_src + up(pts_b), o_idx = o_dst + up(pts_b), o_cnt = o_idx + up(idx_b),
+                 o_best = o_cnt + up(cnt_b), o_ws = o_best + 256, total = o_ws + up(ws_b);
+    unsigned char* dev = nullptr;
+    cudaStream_t st = nullptr;
+    int rc = cuda_status(cudaMalloc(reinterpret_cast<void**>(&dev), total));
+    if (rc == HG_OK) rc = cuda_status(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    if (rc == HG_OK) rc = cuda_status(cudaMemcpyAsync(dev + o_src, src_xy, pts_b, cudaMemcpyHostToDevice, st));
+    if (rc == HG_OK) rc = cuda_status(cudaMemcpyAsync(dev + o_dst, dst_xy, pts_b, cudaMemcpyHostToDevice, st));
+    if (rc == HG_OK) rc = cuda_status(cudaMemcpyAsync(dev + o_idx, hyp_idx, idx_b, cudaMemcpyHostToDevice, st));
+    if (rc == HG_OK)
+        rc = hg_ransac_hypothesize_score(reinterpret_cast<float*>(dev + o_src), reinterpret_cast<float*>(dev + o_dst), n_pts,
+                                         reinterpret_cast<int32_t*>(dev + o_idx), n_hyp, threshold_px,
+                                         reinterpret_cast<int32_t*>(dev + o_cnt), reinterpret_cast<float*>(dev + o_best),
+                                         reinterpret_cast<int64_t*>(dev + o_best + 64),
+                                         reinterpret_cast<int32_t*>(dev + o_best + 128), dev + o_ws, up(ws_b), st);
+    if (rc == HG_OK && counts) rc = cuda_status(cudaMemcpyAsync(counts, dev + o_cnt, cnt_b, cudaMemcpyDeviceToHost, st));
+    if (rc == HG_OK && best_H) rc = cuda_status(cudaMemcpyAsync(best_H, dev + o_best, 9 * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (rc == HG_OK && best_index) rc = cuda_status(cudaMemcpyAsync(best_index, dev + o_best + 64, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    if (rc == HG_OK && best_count) rc = cuda_status(cudaMemcpyAsync(best_count, dev + o_best + 128, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    if (st) {
+        const int r2 = cuda_status(cudaStreamSynchronize(st));
+        if (rc == HG_OK) rc = r2;
+        cudaStreamDestroy(st);
+    }
+    if (dev) cudaFree(dev);
+    return rc;
+}

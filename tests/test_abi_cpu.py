@@ -1,0 +1,117 @@
+"""CPU-side checks of the C-ABI boundary: libhg.so builds, loads and exports every symbol that
+include/hg.h declares; argument validation (pure host logic) returns the documented status codes
+before anything touches a GPU.  No compute call is made here."""
+import ctypes
+import re
+from pathlib import Path
+
+import pytest
+import torch
+
+import paper_2402_18008_b200 as hg
+
+ROOT = Path(__file__).resolve().parents[1]
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "hg.h").read_text()
+    return sorted(set(re.findall(r"HG_API\s+[\w\s\*]+?\b(hg_\w+)\s*\(", text)))
+
+
+def test_header_and_binding_agree():
+    syms = declared_symbols()
+    assert len(syms) >= 11
+    assert sorted(hg.EXPORTS) == syms
+
+
+def test_library_exports_every_declared_symbol():
+    L = hg.lib()
+    for name in declared_symbols():
+        assert hasattr(L, name), name
+    assert hg.hg_built_for_sm() == 100
+    assert hg.hg_version() >= 100
+
+
+def test_status_strings():
+    assert hg.hg_status_string(0) == "HG_OK"
+    for code in (-1, -2, -3, -4):
+        assert hg.hg_status_string(code).startswith("HG_ERR_")
+    assert "unknown" in hg.hg_status_string(-99)
+
+
+def test_cubin_is_sm100a_only():
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-lelf", str(hg.lib_path())], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_(\d+a?)", out))
+    assert archs == {"100a"}, out
+
+
+FAKE = 0x10000          # 16-byte aligned, never dereferenced: validation fails or n == 0 first
+
+
+@pytest.mark.parametrize("fn", ["hg_aca_batched", "hg_sks_batched"])
+def test_solve_argument_validation(fn):
+    f = getattr(hg.lib(), fn)
+    assert f(None, None, None, 0, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == 0          # n == 0: no-op
+    assert f(FAKE, FAKE, FAKE, -1, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -1
+    assert f(None, FAKE, FAKE, 8, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -1
+    assert f(FAKE, FAKE, FAKE, 8, 7, hg.NORM_NONE, hg.PREC_F64, None) == -1              # bad layout
+    assert f(FAKE, FAKE, FAKE, 8, hg.SOA, 9, hg.PREC_F64, None) == -1                    # bad norm
+    assert f(FAKE, FAKE, FAKE, 8, hg.SOA, hg.NORM_NONE, 5, None) == -1                   # bad precision
+    assert f(FAKE + 4, FAKE, FAKE, 8, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -2
+    assert f(FAKE, FAKE, FAKE + 8, 8, hg.AOS, hg.NORM_NONE, hg.PREC_F64, None) == -2
+
+
+def test_host_solve_argument_validation():
+    f = hg.lib().hg_aca_batched_host
+    assert f(None, None, None, 0, hg.SOA, hg.NORM_NONE, hg.PREC_F64, 0) == 0
+    assert f(FAKE, FAKE, FAKE, -3, hg.SOA, hg.NORM_NONE, hg.PREC_F64, 0) == -1
+    assert f(FAKE, FAKE, None, 4, hg.SOA, hg.NORM_NONE, hg.PREC_F64, 0) == -1
+    assert f(FAKE, FAKE, FAKE, 4, hg.SOA, hg.NORM_NONE, hg.PREC_F64, -1) == -1
+
+
+def test_grid_argument_validation():
+    f = hg.lib().hg_offsets_to_grid
+    assert f(None, 0.0, 0.0, 127.0, 127.0, 128, 128, None, None, 0, hg.NORM_H33, None) == 0
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, None, None, 5, hg.NORM_H33, None) == 0   # nothing requested
+    assert f(FAKE, 0.0, 0.0, 0.0, 127.0, 128, 128, FAKE, FAKE, 5, hg.NORM_H33, None) == -1    # w == 0
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 0, 128, FAKE, FAKE, 5, hg.NORM_H33, None) == -1    # grid_w < 1
+    assert f(None, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE, 5, hg.NORM_H33, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE + 8, 5, hg.NORM_H33, None) == -2
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE, -5, hg.NORM_H33, None) == -1
+
+
+def test_ransac_argument_validation_and_workspace():
+    L = hg.lib()
+    ws = L.hg_ransac_workspace_bytes
+    assert ws(4096, 1 << 20) >= 64 + 4096 * 16 + 4 * (1 << 20)
+    assert ws(4097, 10) >= 64 + 2049 * 32 + 40
+    assert ws(4096, 1 << 20) % 16 == 0
+    f = L.hg_ransac_hypothesize_score
+    args_ok = [FAKE, FAKE, 100, FAKE, 10, 3.0, FAKE, FAKE, FAKE, FAKE, FAKE, 1 << 30, None]
+
+    def call(**kw):
+        a = list(args_ok)
+        names = ["src", "dst", "n_pts", "idx", "n_hyp", "t", "counts", "bH", "bi", "bc", "ws", "wsb", "st"]
+        for k, v in kw.items():
+            a[names.index(k)] = v
+        return f(*a)
+
+    assert call(n_hyp=0) == 0
+    assert call(n_pts=3) == -1
+    assert call(n_hyp=-1) == -1
+    assert call(t=0.0) == -1
+    assert call(t=float("nan")) == -1
+    assert call(src=None) == -1
+    assert call(ws=None) == -1
+    assert call(idx=FAKE + 4) == -2
+    assert call(bi=FAKE + 4) == -2
+    assert call(wsb=128) == -4
+
+
+def test_binding_refuses_cpu_tensors_on_the_device_entry_points():
+    s = torch.zeros((8, 16), dtype=torch.float32)
+    with pytest.raises(ValueError, match="no fallback"):
+        hg.hg_aca_batched(s, s)
+    with pytest.raises(TypeError):
+        hg.hg_aca_batched(s.double(), s.double())

@@ -1,0 +1,162 @@
+"""GPU parity of hg_offsets_to_grid and hg_ransac_hypothesize_score against the fp64 oracle.
+
+Grid tolerance: 1e-3 px absolute, the reprojection tolerance of
+north_star applied to every pixel.  RANSAC (north_star): counts exact except for correspondences
+whose fp64 residual lies within 1e-4 relative of the threshold, i.e.
+|count_gpu - count_oracle| <= band_count(hypothesis); best index equal unless the top counts tie
+within their bands.
+"""
+import numpy as np
+import pytest
+import torch
+
+import hg_workloads as W
+import oracle
+import paper_2402_18008_b200 as hg
+from util import align_to
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+GRID_TOL = 1e-3
+
+
+# ---- offsets -> H -> grid --------------------------------------------------------------------
+@pytest.mark.parametrize("rect,gw,gh,n", [((0.0, 0.0, 127.0, 127.0), 128, 128, 300),      # C5 shape
+                                          ((10.0, -4.0, 300.0, 90.0), 37, 11, 65),          # odd width: 64-bit stores
+                                          ((0.0, 0.0, 63.0, 31.0), 64, 32, 17),
+                                          ((5.0, 5.0, 20.0, 20.0), 1, 1, 4),
+                                          ((0.0, 0.0, 511.0, 3.0), 512, 4, 9),              # row wider than a block
+                                          ((0.0, 0.0, 1.0, 1.0), 2, 2, 1000)])
+def test_grid_matches_oracle(rect, gw, gh, n):
+    x0, y0, w, h = rect
+    scale = min(32.0, 0.2 * min(w, h))
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 5, max_offset=scale)
+    H, g = hg.hg_offsets_to_grid(off.to(DEV), x0, y0, w, h, gw, gh, norm=hg.NORM_H33)
+    H_ref, g_ref = oracle.offsets_to_grid(off.numpy(), x0, y0, w, h, gw, gh)
+    g = g.cpu().numpy().astype(np.float64)
+    assert g.shape == g_ref.shape
+    assert np.abs(g - g_ref).max() <= GRID_TOL, np.abs(g - g_ref).max()
+    Hg, Hr = align_to(H.cpu().numpy().astype(np.float64), H_ref)
+    assert (np.abs(Hg - Hr) <= 1e-4 * np.abs(Hr) + 1e-7).all()
+    assert np.all(H.cpu().numpy()[:, 2, 2] == 1.0)
+
+
+def test_grid_config5_corners_and_h_only_and_grid_only():
+    n = 2048
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 5).to(DEV)
+    H, g = hg.hg_offsets_to_grid(off, 0.0, 0.0, 127.0, 127.0, 128, 128)
+    corners = W.patch_corners().to(DEV)
+    got = torch.stack([g[:, 0, 0], g[:, 0, 127], g[:, 127, 127], g[:, 127, 0]], dim=1)
+    assert (got - (corners[None] + off)).abs().max().item() <= GRID_TOL
+    H_only, none = hg.hg_offsets_to_grid(off, 0.0, 0.0, 127.0, 127.0, 128, 128, want_grid=False)
+    assert none is None and torch.equal(H_only, H)
+    none, g_only = hg.hg_offsets_to_grid(off, 0.0, 0.0, 127.0, 127.0, 128, 128, want_H=False)
+    assert none is None and torch.equal(g_only, g)
+    # zero offsets: the grid is the pixel lattice itself
+    _, g0 = hg.hg_offsets_to_grid(torch.zeros((3, 4, 2), device=DEV), 0.0, 0.0, 127.0, 127.0, 128, 128)
+    xs = torch.arange(128.0, device=DEV)
+    assert (g0[..., 0] - xs[None, None, :]).abs().max().item() <= 1e-4
+    assert (g0[..., 1] - xs[None, :, None]).abs().max().item() <= 1e-4
+
+
+def test_grid_config1_h_only_matches_general_solver():
+    """C1 through the offsets entry point (H only, thread per item) = general ACA on the same corners."""
+    off = W.offsets_workload(1024, seed=W.SEED_BASE + 1)
+    H, _ = hg.hg_offsets_to_grid(off.to(DEV), 0.0, 0.0, 127.0, 127.0, 128, 128, want_grid=False, norm=hg.NORM_FROBENIUS)
+    s, d = W.offsets_to_sets(off)
+    Hg = hg.hg_aca_batched(s.to(DEV), d.to(DEV), layout=hg.AOS, norm=hg.NORM_FROBENIUS)
+    assert torch.equal(H, Hg)
+    Hr = oracle.aca(s.numpy(), d.numpy())
+    a, b = align_to(H.cpu().numpy().astype(np.float64), Hr)
+    assert (np.abs(a - b) <= 1e-4 * np.abs(b) + 1e-7).all()
+
+
+def test_grid_full_config5_sampled():
+    """C5 at BASELINE size: 8192 x 128 x 128 x 2; a sample of items compared with the oracle and
+    the corner property checked on every item."""
+    n = 8192
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 5)
+    H, g = hg.hg_offsets_to_grid(off.to(DEV), 0.0, 0.0, 127.0, 127.0, 128, 128)
+    sel = np.arange(0, n, 127)
+    _, g_ref = oracle.offsets_to_grid(off.numpy()[sel], 0.0, 0.0, 127.0, 127.0, 128, 128)
+    assert np.abs(g[torch.from_numpy(sel).to(DEV)].cpu().numpy() - g_ref).max() <= GRID_TOL
+    corners = W.patch_corners().to(DEV)
+    got = torch.stack([g[:, 0, 0], g[:, 0, 127], g[:, 127, 127], g[:, 127, 0]], dim=1)
+    assert (got - (corners[None] + off.to(DEV))).abs().max().item() <= GRID_TOL
+    assert torch.isfinite(g).all()
+
+
+# ---- RANSAC ------------------------------------------------------------------------------------
+def check_ransac(wl, t, out, ref):
+    counts = out["counts"].cpu().numpy()
+    diff = np.abs(counts.astype(np.int64) - ref["counts"].astype(np.int64))
+    assert (diff <= ref["band_counts"]).all(), (int((diff > ref["band_counts"]).sum()), int(diff.max()))
+    bi, bc = int(out["best_index"].item()), int(out["best_count"].item())
+    assert bc == counts.max() and bi == int(np.argmax(counts))            # argmax, ties -> lowest index
+    if ref["band_counts"][[bi, ref["best_index"]]].sum() == 0 and (diff == 0).all():
+        assert bi == ref["best_index"] and bc == ref["best_count"]
+    else:
+        assert abs(bc - ref["best_count"]) <= ref["band_counts"].max()
+    idx = wl["hyp_idx"].numpy()[bi]
+    H_ref = oracle.normal_form(oracle.aca(wl["src_xy"].numpy()[idx][None], wl["dst_xy"].numpy()[idx][None]))[0]
+    Hb = out["best_H"].cpu().numpy().astype(np.float64)
+    a, b = align_to(Hb[None], H_ref[None])
+    assert np.abs(a - b).max() <= 2e-7
+    assert abs(np.sqrt((Hb ** 2).sum()) - 1.0) <= 3e-7
+    return diff
+
+
+@pytest.mark.parametrize("n_pts,n_hyp,t", [(4096, 6000, 3.0), (1001, 5000, 3.0), (100, 777, 1.5),
+                                           (4, 1, 3.0), (2500, 3000, 0.75), (9000, 1500, 3.0)])
+def test_ransac_counts_match_oracle(n_pts, n_hyp, t):
+    wl = W.ransac_workload(n_pts=n_pts, n_hyp=n_hyp, seed=W.SEED_BASE + 4 + n_pts)
+    out = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV), t)
+    ref = oracle.ransac(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy(), t, band_rel=1e-4)
+    diff = check_ransac(wl, t, out, ref)
+    stats = hg.ransac_stats(out["workspace"])
+    print(n_pts, n_hyp, "mismatching (all inside the band):", int((diff > 0).sum()), stats)
+
+
+def test_ransac_duplicate_best_and_degenerate_hypotheses():
+    wl = W.ransac_workload(n_pts=512, n_hyp=400, seed=11)
+    src, dst, idx = wl["src_xy"].clone(), wl["dst_xy"].clone(), wl["hyp_idx"].clone()
+    # degenerate data: correspondences 0..3 coincide pairwise -> a hypothesis on them gives H = 0 -> count 0
+    src[1] = src[0]; dst[1] = dst[0]; src[3] = src[2]; dst[3] = dst[2]
+    idx[7] = torch.tensor([0, 1, 2, 3], dtype=torch.int32)
+    ref = oracle.ransac(src.numpy(), dst.numpy(), idx.numpy(), 3.0, band_rel=1e-4)
+    b = ref["best_index"]
+    idx2 = torch.cat([idx, idx[b:b + 1]], dim=0)                # a tie: the lower index must win
+    out = hg.hg_ransac_hypothesize_score(src.to(DEV), dst.to(DEV), idx2.to(DEV), 3.0)
+    ref2 = oracle.ransac(src.numpy(), dst.numpy(), idx2.numpy(), 3.0, band_rel=1e-4)
+    check_ransac({"src_xy": src, "dst_xy": dst, "hyp_idx": idx2}, 3.0, out, ref2)
+    assert out["counts"][7].item() == 0 == ref2["counts"][7]
+    assert int(out["best_index"].item()) == b
+
+
+def test_ransac_host_entry_point_and_no_counts():
+    wl = W.ransac_workload(n_pts=777, n_hyp=2000, seed=5)
+    dev = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV), 3.0)
+    host = hg.hg_ransac_hypothesize_score_host(wl["src_xy"], wl["dst_xy"], wl["hyp_idx"], 3.0)
+    assert torch.equal(host["counts"], dev["counts"].cpu())
+    assert torch.equal(host["best_H"], dev["best_H"].cpu())
+    assert host["best_index"].item() == dev["best_index"].item()
+    nc = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV), 3.0,
+                                        want_counts=False)
+    assert nc["counts"] is None and nc["best_index"].item() == dev["best_index"].item()
+
+
+def test_ransac_full_config4_sampled():
+    """C4 at BASELINE size (4096 correspondences, 2^20 hypotheses, t = 3 px), in the launch
+    configuration bench.py times; the oracle scores a strided sample of 8192 hypotheses plus the
+    GPU's best hypothesis."""
+    wl = W.ransac_workload(n_pts=4096, n_hyp=1 << 20, seed=W.SEED_BASE + 4)
+    out = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV), 3.0)
+    counts = out["counts"].cpu().numpy()
+    bi, bc = int(out["best_index"].item()), int(out["best_count"].item())
+    assert bc == counts.max() and bi == int(np.argmax(counts))
+    sel = np.unique(np.concatenate([np.arange(0, 1 << 20, 128), [bi, (1 << 20) - 1]]))
+    ref = oracle.ransac(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy()[sel], 3.0, band_rel=1e-4)
+    diff = np.abs(counts[sel].astype(np.int64) - ref["counts"])
+    assert (diff <= ref["band_counts"]).all(), int((diff > ref["band_counts"]).sum())
+    assert bc >= 0.6 * 0.7 * 4096
+    print("C4 sampled: mismatches inside band", int((diff > 0).sum()), "of", len(sel), hg.ransac_stats(out["workspace"]))

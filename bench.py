@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of libhg (BASELINE.json: "homographies/sec (ACA fp32, batch 2^26)
+and % of B200 peak HBM GB/s").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A step is one pass of the hot path over one batch: one `hg_aca_batched` call (SoA fp32 in/out,
+fp64-internal arithmetic) on config C3 = 2^26 general-position 4-point sets generated on the GPU by
+the seeded recipe of DESIGN.md (64 B read + 36 B written per homography; 6.7 GB per step, so every
+step streams from HBM: no L2 flush is needed).  Rank 0 prints ONE JSON line.
+
+  value      whole-job homographies/s, inputs resident in HBM, CUDA events on the launch stream,
+             max over ranks
+  e2e        the same through `hg_aca_batched_host` (pinned HOST buffers in, HOST buffer out;
+             chunked H2D -> kernel -> D2H pipeline inside the timed region)
+  roofline   algorithmic bytes (100 B x 2^26) / average launch duration, against MEASURED_PEAKS.json
+  cpu_baseline  the fp64 oracle (oracle/) on the host cores, on a bounded sample of the same workload
+  extras     the other hot-path rows at their BASELINE sizes (SKS C3, grid C5, RANSAC C4, C1 latency)
+
+`--impl reference` times the oracle alone (rank 0 only), same metric/unit/config.
+With N > 1 (torchrun, one rank per GPU) every rank solves its own 2^26 sets: weak scaling, no
+data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import torch  # noqa: E402
+
+METRIC = "homographies/sec (ACA fp32, batch 2^26)"
+UNIT = "homographies/s"
+LOG2N = 26
+BYTES_PER_H = 100            # 16 fp32 read + 9 fp32 written
+FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+
+def workload_config(n, world):
+    return {"workload": "C3: general-position 4-point sets, batch 2^%d per GPU, fp32 SoA, ACA" % LOG2N
+            if n == 1 << LOG2N else "C3-like, batch %d per GPU, fp32 SoA, ACA" % n,
+            "sets_per_gpu": n, "layout": "SoA float[8][n] x2 -> float[9][n]", "arith": "fp64 internal, fp32 I/O",
+            "norm": "none (raw ACA scale)", "l2": "inputs_larger_than_l2 (6.7 GB per step)",
+            "parallelism": "dp%d (independent shards, no collective)" % world, "seed": 240218008 + 3}
+
+
+# ---- clocks during the timed region (NVML in a thread; nvidia-smi is too coarse for a 50 ms region) ----
+class ClockSampler:
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index):
+        self.samples, self.reasons, self._stop, self._thr, self.max_mhz = [], set(), threading.Event(), None, None
+        self.error = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = self._handle(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:      # no NVML: report that instead of a number
+            self.nv, self.error = None, repr(e)
+
+    def _handle(self, index):
+        uuid = None
+        try:
+            uuid = str(torch.cuda.get_device_properties(index).uuid)
+        except Exception:
+            pass
+        if uuid:
+            for cand in (uuid, "GPU-" + uuid):
+                try:
+                    return self.nv.nvmlDeviceGetHandleByUUID(cand.encode() if isinstance(cand, str) else cand)
+                except Exception:
+                    continue
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+        return self.nv.nvmlDeviceGetHandleByIndex(phys)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                bits = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for b, name in self.REASONS.items():
+                    if bits & b:
+                        self.reasons.add(name)
+            except Exception as e:
+                self.error = repr(e)
+                return
+            time.sleep(0.002)
+
+    def start(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr:
+            self._stop.set()
+            self._thr.join()
+        out = {"sm_mhz": statistics.median(self.samples) if self.samples else None, "sm_max_mhz": self.max_mhz,
+               "reasons": sorted(self.reasons), "samples": len(self.samples)}
+        if self.error:
+            out["error"] = self.error
+        return out
+
+
+def measured_peak_gbs():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return float(json.loads(p.read_text())["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "B200_PROFILING.md fallback (of fallback)"
+
+
+def event_time_ms(fn, reps, stream=None):
+    """Total device time of `reps` back-to-back calls, CUDA events on the current stream."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)
+
+
+# ---- the oracle on the host cores -------------------------------------------------------------------
+def oracle_rate(src_aos, dst_aos, passes, warm=1):
+    """ACA-fp64 oracle, all host cores (OpenMP): homographies/s over `passes` passes of the sample."""
+    import oracle
+    for _ in range(warm):
+        oracle.aca(src_aos, dst_aos)
+    t0 = time.perf_counter()
+    for _ in range(passes):
+        oracle.aca(src_aos, dst_aos)
+    dt = time.perf_counter() - t0
+    return src_aos.shape[0] * passes / dt, oracle.num_threads(), dt
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    import hg_workloads as W
+    n_s = 1 << 22
+    src, dst = W.general_sets(n_s, seed=W.SEED_BASE + 3)
+    s, d = src.numpy(), dst.numpy()
+    warm = max(args.warmup, 1)
+    rate, cores, dt = oracle_rate(s, d, passes=max(args.steps, 1), warm=warm)
+    sample = "each step = the first 2^22 sets of the C3 generator (CPU stream), ACA-fp64 oracle, OpenMP over all host cores"
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": warm, "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(1 << LOG2N, 1),
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---- extras: the other rows of the hot path at BASELINE sizes -----------------------------------------
+def run_extras(hg, W, dev, src, dst, H, peak):
+    n = src.shape[1]
+    ex = {}
+    for name, fn in (("sks_c3", hg.hg_sks_batched),):
+        ms = event_time_ms(lambda: fn(src, dst, H=H), 5) / 5
+        ex[name] = {"ms": ms, "homographies_per_s": n / ms * 1e3, "GBps": n * BYTES_PER_H / ms / 1e6,
+                    "frac_of_peak": n * BYTES_PER_H / ms / 1e6 / peak}
+    ms = event_time_ms(lambda: hg.hg_aca_batched(src, dst, H=H, prec=hg.PREC_F32), 5) / 5
+    ex["aca_c3_plain_fp32"] = {"ms": ms, "GBps": n * BYTES_PER_H / ms / 1e6, "note": "HG_PREC_F32: fails the parity tolerance, measurement only"}
+    # C5: offsets -> H -> grid, 8192 x 128 x 128 x 2 fp32 = 1.07 GB written per call (> L2)
+    off = W.offsets_workload(8192, seed=W.SEED_BASE + 5, device=dev)
+    Hh = torch.empty((8192, 3, 3), dtype=torch.float32, device=dev)
+    grid = torch.empty((8192, 128, 128, 2), dtype=torch.float32, device=dev)
+    f5 = lambda: hg.hg_offsets_to_grid(off, 0.0, 0.0, 127.0, 127.0, 128, 128, H=Hh, grid=grid)
+    f5(); f5(); f5()
+    ms = event_time_ms(f5, 10) / 10
+    by = grid.numel() * 4 + off.numel() * 4 + Hh.numel() * 4
+    ex["grid_c5"] = {"ms": ms, "GBps_written": by / ms / 1e6, "frac_of_peak": by / ms / 1e6 / peak,
+                     "grids_per_s": 8192 / ms * 1e3}
+    del grid
+    # C1: 1024 offsets -> H, launch-latency bound: us per call, plain launches and CUDA-graph replay
+    off1 = W.offsets_workload(1024, seed=W.SEED_BASE + 1, device=dev)
+    H1 = torch.empty((1024, 3, 3), dtype=torch.float32, device=dev)
+    f1 = lambda: hg.hg_offsets_to_grid(off1, 0.0, 0.0, 127.0, 127.0, 128, 128, H=H1, want_grid=False)
+    for _ in range(5):
+        f1()
+    ms = event_time_ms(f1, 200) / 200
+    ex["c1_offsets_to_h_1024"] = {"us_per_call_launch": ms * 1e3}
+    try:
+        st = torch.cuda.Stream()
+        st.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(st):
+            f1()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                for _ in range(20):
+                    f1()
+        torch.cuda.current_stream().wait_stream(st)
+        g.replay()
+        ms = event_time_ms(g.replay, 20) / (20 * 20)
+        ex["c1_offsets_to_h_1024"]["us_per_call_graph"] = ms * 1e3
+    except Exception as e:          # graph capture is a convenience measurement, never the headline
+        ex["c1_offsets_to_h_1024"]["graph_error"] = repr(e)[:200]
+    # C4: fused RANSAC, 4096 correspondences x 2^20 hypotheses, 3 px
+    wl = W.ransac_workload(device=dev)
+    ws = torch.empty(hg.hg_ransac_workspace_bytes(4096, 1 << 20), dtype=torch.uint8, device=dev)
+    cnt = torch.empty(1 << 20, dtype=torch.int32, device=dev)
+    f4 = lambda: hg.hg_ransac_hypothesize_score(wl["src_xy"], wl["dst_xy"], wl["hyp_idx"], 3.0, counts=cnt, workspace=ws)
+    out = f4(); f4(); f4()
+    ms = event_time_ms(f4, 5) / 5
+    stats = hg.ransac_stats(ws)
+    pairs = 4096 * (1 << 20)
+    props = torch.cuda.get_device_properties(dev)
+    ex["ransac_c4"] = {"ms": ms, "pairs_per_s": pairs / ms * 1e3, "hypotheses_per_s": (1 << 20) / ms * 1e3,
+                       "best_count": int(out["best_count"]), "fixup_hypotheses": stats["n_fixup"],
+                       "pairs_decided_in_fp64": stats["n_pairs_f64"],
+                       "fp32_lane_instr_per_pair": 14, "alu_peak_instr_per_s": props.multi_processor_count * 128 * 1.965e9,
+                       "frac_of_fp32_issue_peak": pairs * 14 / (ms * 1e-3) / (props.multi_processor_count * 128 * 1.965e9)}
+    return ex
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--log2n", type=int, default=LOG2N, help="sets per GPU = 2^log2n (default: the BASELINE size)")
+    ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libhg has no CPU path")
+    import torch.distributed as dist
+    import hg_workloads as W
+    import paper_2402_18008_b200 as hg
+
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    barrier = (lambda: dist.barrier()) if world > 1 else (lambda: None)
+
+    n = 1 << args.log2n
+    warm = max(args.warmup, 3)
+    steps = max(args.steps, 1)
+    hg.lib()
+    src, dst = W.general_sets(n, seed=W.SEED_BASE + 3 + 1000 * rank, device=dev, soa=True)
+    H = torch.empty((9, n), dtype=torch.float32, device=dev)
+    step = lambda: hg.hg_aca_batched(src, dst, H=H, layout=hg.SOA, norm=hg.NORM_NONE, prec=hg.PREC_F64)
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    for _ in range(warm):
+        step()
+    barrier()
+    ms_total = event_time_ms(step, steps)
+    barrier()
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / steps
+    value = world * n / (ms_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry point ------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        hs = torch.empty((8, n), dtype=torch.float32, pin_memory=True)
+        hd = torch.empty((8, n), dtype=torch.float32, pin_memory=True)
+        hH = torch.empty((9, n), dtype=torch.float32, pin_memory=True)
+        hs.copy_(src)
+        hd.copy_(dst)
+        torch.cuda.synchronize()
+        e_steps = min(steps, 5)
+        hg.hg_aca_batched_host(hs, hd, H=hH)                  # warm-up (allocations, page faults)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e_steps):
+            hg.hg_aca_batched_host(hs, hd, H=hH)              # synchronous: returns with H in host memory
+        dt = time.perf_counter() - t0
+        barrier()
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        same = bool(torch.equal(hH[:, :: 4097], H[:, :: 4097].cpu()))
+        e2e = {"value": world * n * e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 64 * n, "d2h_bytes_per_step": 36 * n,
+               "steps": e_steps, "ms_per_step": dt / e_steps * 1e3, "api": "hg_aca_batched_host (pinned host buffers)",
+               "matches_device_result": same}
+        del hs, hd, hH
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = measured_peak_gbs()
+    achieved = n * BYTES_PER_H / (ms_step * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(n, world),
+            "clocks": clocks, "gpu_launches": steps,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "hg::solve_soa_kernel<ACA,double,4>", "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": n * BYTES_PER_H, "frac_of_8000_datasheet": achieved / 8000.0},
+            "pct_of_peak_hbm": 100.0 * achieved / peak}
+    if e2e is not None:
+        line["e2e"] = e2e
+    if world == 1 and not args.no_cpu:
+        n_s = min(n, 1 << 24)
+        s_aos = W.to_aos(src[:, :n_s].contiguous()).cpu().numpy()
+        d_aos = W.to_aos(dst[:, :n_s].contiguous()).cpu().numpy()
+        rate, cores, dt = oracle_rate(s_aos, d_aos, passes=3)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": "first 2^%d sets of the timed workload, 3 passes of the ACA-fp64 oracle (OpenMP, %.1f s)"
+                                          % (n_s.bit_length() - 1, dt)}
+        del s_aos, d_aos
+    if world == 1 and not args.no_extras:
+        try:
+            line["extras"] = run_extras(hg, W, dev, src, dst, H, peak)
+        except Exception as e:
+            line["extras"] = {"error": repr(e)[:300]}
+    # traffic from the committed ncu capture, if one is recorded
+    tfile = ROOT / "profiles" / "roofline_traffic.json"
+    if tfile.exists():
+        try:
+            line["roofline"]["traffic"] = json.loads(tfile.read_text()).get("aca_c3_dram_bytes_per_launch")
+        except Exception:
+            pass
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

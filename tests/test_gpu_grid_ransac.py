@@ -59,16 +59,22 @@ def test_grid_config5_corners_and_h_only_and_grid_only():
     assert (g0[..., 1] - xs[None, :, None]).abs().max().item() <= 1e-4
 
 
-def test_grid_config1_h_only_matches_general_solver():
-    """C1 through the offsets entry point (H only, thread per item) = general ACA on the same corners."""
+def test_grid_config1_h_only_matches_oracle_and_general_solver():
+    """C1 through the offsets entry point (H only, thread per item): equals the oracle's offsets->H,
+    and the general ACA solver on the fp32-rounded corners up to that rounding."""
     off = W.offsets_workload(1024, seed=W.SEED_BASE + 1)
     H, _ = hg.hg_offsets_to_grid(off.to(DEV), 0.0, 0.0, 127.0, 127.0, 128, 128, want_grid=False, norm=hg.NORM_FROBENIUS)
-    s, d = W.offsets_to_sets(off)
-    Hg = hg.hg_aca_batched(s.to(DEV), d.to(DEV), layout=hg.AOS, norm=hg.NORM_FROBENIUS)
-    assert torch.equal(H, Hg)
-    Hr = oracle.aca(s.numpy(), d.numpy())
+    Hr, _ = oracle.offsets_to_grid(off.numpy(), 0.0, 0.0, 127.0, 127.0, 128, 128, want_grid=False)
     a, b = align_to(H.cpu().numpy().astype(np.float64), Hr)
     assert (np.abs(a - b) <= 1e-4 * np.abs(b) + 1e-7).all()
+    assert np.abs(a - b).max() <= 2e-7
+    s, d = W.offsets_to_sets(off)                       # corner + offset rounded to fp32
+    Hg = hg.hg_aca_batched(s.to(DEV), d.to(DEV), layout=hg.AOS, norm=hg.NORM_FROBENIUS)
+    assert (H - Hg).abs().max().item() <= 1e-5
+    # Algorithm 1 (TensorACA-rect, P:568-591) evaluated by the oracle gives the same H
+    Ha = oracle.aca_rect(off.numpy(), 0.0, 0.0, 127.0, 127.0)
+    a2, b2 = align_to(H.cpu().numpy().astype(np.float64), Ha)
+    assert np.abs(a2 - b2).max() <= 2e-7
 
 
 def test_grid_full_config5_sampled():

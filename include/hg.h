@@ -131,7 +131,7 @@ HG_API int hg_offsets_to_grid(const float* offsets, float x0, float y0, float w,
  * the correspondences whose forward transfer error ||pi(H*s) - d||_2 <= threshold_px
  * (reading R9: inclusive, W == 0 -> outlier, no degeneracy test, no local optimisation).
  * Scoring runs in fp32 with a per-hypothesis rigorous error band; every pair that falls inside
- * the band is re-decided in fp64, so counts equal an fp64 evaluation.
+ * the band is decided in fp64 inside the same sweep, so counts equal an fp64 evaluation.
  *   src_xy, dst_xy : float[n_pts][2] correspondences                  (read)
  *   hyp_idx        : int32[n_hyp][4], the 4 indices of a row distinct and in [0,n_pts)
  *                    (out-of-range indices are undefined behaviour)   (read, 16 B per hyp.)
@@ -154,7 +154,7 @@ HG_API int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy,
 
 /* After hg_ransac_hypothesize_score has completed on its stream, the first 4 int64 words of
  * the workspace hold statistics of that call (device memory; copy them out to read):
- *   [0] packed best key, [1] number of hypotheses re-scored by the fp64 fix-up pass,
+ *   [0] packed best key, [1] number of hypotheses that had at least one pair decided in fp64,
  *   [2] number of (hypothesis, point) pairs decided in fp64, [3] reserved.                      */
 #define HG_RANSAC_STAT_WORDS 4
 

@@ -1,18 +1,18 @@
 // hg_ransac.cu -- hg_ransac_hypothesize_score: RANSAC hypothesis generation fused with inlier
 // scoring (rows a-R0..a-R5 of SURVEY.md section 8(a)).
 //
-// Four launches on the caller's stream, no host synchronisation:
+// Three launches on the caller's stream, no host synchronisation:
 //   1. prep     : correspondence table -> packed, threshold-folded fp32 table in the workspace
 //                 (+ coordinate bounds for the error band)
 //   2. score    : one thread per hypothesis: gather 4 correspondences, fp64 ACA solve, fold the
 //                 threshold into H, then sweep the whole table from shared memory (staged by
 //                 bulk-async copies / mbarrier) with packed FFMA2 arithmetic, two points per
-//                 instruction.  Counts "surely inlier" and "surely outlier" pairs against a
-//                 rigorous per-hypothesis fp32 error band.
-//   3. fix-up   : hypotheses that had at least one pair inside the band are re-swept by one warp
-//                 each; the in-band pairs are decided in fp64 by the definition (reading R9).
-//   4. finalize : decode the packed (count, index) maximum, re-solve that hypothesis, emit best_H.
-// Compute-bound on the FP32 pipe: 14 packed instructions per two (hypothesis, point) pairs.
+//                 instruction.  One value per pair, a = (ex^2 + ey^2 - W^2) + Bc, against a rigorous
+//                 per-hypothesis fp32 error band Bc: a < 0 is a
+//                 sure inlier, a > 2 Bc a sure outlier; the rare pair in between is decided on the
+//                 spot in fp64 by the definition (reading R9) from the fp64 H kept in shared memory.
+//   3. finalize : decode the packed (count, index) maximum, re-solve that hypothesis, emit best_H.
+// Compute-bound on the FP32 pipe: 11 packed instructions per two (hypothesis, point) pairs.
 #include "hg_device.cuh"
 #include "hg_host.h"
 
@@ -21,12 +21,11 @@ namespace hg {
 constexpr int kRBlock     = 512;    // threads (= hypotheses) per scoring CTA
 constexpr int kChunkPairs = 1024;   // point pairs per shared-memory stage: 1024 * 32 B = 32 KB
 constexpr int kStages     = 2;
-constexpr int kFixBlock   = 256;
 constexpr size_t kHeaderBytes = 64;
 
 struct RansacHeader {               // first 64 bytes of the workspace
     unsigned long long best_key;    // (count << 32) | (0xFFFFFFFF - hypothesis index)
-    unsigned long long n_fixup;     // length of the fix-up worklist
+    unsigned long long n_fixup;     // hypotheses with at least one pair decided in fp64
     unsigned long long n_pairs_f64; // (hypothesis, point) pairs decided in fp64
     unsigned long long reserved;
     unsigned int bound_bits[4];     // float bits of max|sx|, max|sy|, max|dx/t|, max|dy/t|
@@ -37,38 +36,33 @@ static_assert(sizeof(RansacHeader) == kHeaderBytes, "header layout");
 // Per-hypothesis constants of the fp32 sweep.
 struct HypConst {
     float h[9];     // rows 1,2 of H scaled by 1/(t*max|h|), row 3 by 1/max|h|
-    float K;        // band slope:  |computed - exact| of (ex^2 + ey^2 - W^2) <= K*|W| + K0 whenever it matters
-    float K0;       // band offset
-    float K0x2;
+    float Bc;       // band: |computed - exact| of (ex^2 + ey^2 - W^2) < Bc for every table point whenever it matters
+    unsigned thr;   // float bits of 2*Bc
+    float K, K0;    // per-pair band K|W| + K0 <= Bc, used only by the cold path
 };
 
 // ---- packed fp32 helpers -------------------------------------------------------------------
 __device__ __forceinline__ float2 f2(float v) { return make_float2(v, v); }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
-__device__ __forceinline__ float2 abs2(float2 a) { return make_float2(fabsf(a.x), fabsf(a.y)); }
 
-// Two points against one hypothesis.  Outputs a < 0 <=> surely inlier, nb < 0 <=> surely outlier.
-// ndx, ndy hold -d/t.  14 packed FP32 instructions.
-__device__ __forceinline__ void score2(const HypConst& c, float2 sx, float2 sy, float2 ndx, float2 ndy,
-                                       float2& a, float2& nb)
+// Two points against one hypothesis: a = (ex^2 + ey^2 - W^2) + Bc, 11 packed FP32 instructions.
+//   a < 0         <=> surely inlier;   a > 2*Bc  <=> surely outlier;   0 <= a <= 2*Bc: decide in fp64.
+// ndx, ndy hold -d/t.
+__device__ __forceinline__ float2 score2(const HypConst& c, float2 sx, float2 sy, float2 ndx, float2 ndy)
 {
     const float2 X = __ffma2_rn(f2(c.h[0]), sx, __ffma2_rn(f2(c.h[1]), sy, f2(c.h[2])));
     const float2 Y = __ffma2_rn(f2(c.h[3]), sx, __ffma2_rn(f2(c.h[4]), sy, f2(c.h[5])));
     const float2 W = __ffma2_rn(f2(c.h[6]), sx, __ffma2_rn(f2(c.h[7]), sy, f2(c.h[8])));
     const float2 ex = __ffma2_rn(ndx, W, X);                     // X/t - (dx/t) W
     const float2 ey = __ffma2_rn(ndy, W, Y);
-    const float2 w2 = __ffma2_rn(W, W, f2(-c.K0));               // W^2 - K0
+    const float2 w2 = __ffma2_rn(W, W, f2(-c.Bc));               // W^2 - Bc
     const float2 p  = __ffma2_rn(ex, ex, neg2(w2));
-    const float2 dp = __ffma2_rn(ey, ey, p);                     // ex^2 + ey^2 - W^2 + K0
-    const float2 aw = abs2(W);
-    a = __ffma2_rn(f2(c.K), aw, dp);                             // diff + (K|W| + K0)
-    const float2 g2 = __ffma2_rn(f2(c.K), aw, f2(c.K0x2));       // K|W| + 2 K0
-    nb = __fadd2_rn(g2, neg2(dp));                               // (K|W| + K0) - diff
+    return __ffma2_rn(ey, ey, p);                                // ex^2 + ey^2 - W^2 + Bc
 }
 
 __device__ __forceinline__ unsigned sign_bit(float v) { return __float_as_uint(v) >> 31; }
 
-// ---- hypothesis set-up (shared by score, fix-up and finalize) --------------------------------
+// ---- hypothesis set-up (shared by score and finalize) --------------------------------
 __device__ __forceinline__ void gather_sets(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy,
                                             const int4 id, double s[8], double d[8])
 {
@@ -112,9 +106,16 @@ __device__ __forceinline__ bool make_hypothesis(const double s[8], const double 
     const double C = u * (3.0 * A1 + 4.0 * Dx * A3) + u * (3.0 * A2 + 4.0 * Dy * A3) + 3.0 * u * A3;
     const double Kd = (4.0 * C + 16.0 * u * A3) * 1.000001;
     const double K0d = 32.0 * C * C * 1.000001;
+    // One band for the whole table: |W^| <= A3 (1 + 3u) for every point, so Bc >= K |W^| + K0.
     c.K = __double2float_ru(Kd);
     c.K0 = __double2float_ru(K0d);
-    c.K0x2 = 2.0f * c.K0;
+    c.Bc = __double2float_ru(Kd * A3 * 1.000001 + K0d);
+    c.thr = __float_as_uint(2.0f * c.Bc);
+    if (!ok) {                          // unusable H: every point a sure outlier (X = 1, W = 0 => a = 1 > 0)
+#pragma unroll
+        for (int k = 0; k < 9; ++k) c.h[k] = 0.f;
+        c.h[2] = 1.f; c.Bc = 0.f; c.thr = 0u;
+    }
     return ok;
 }
 
@@ -206,15 +207,95 @@ __device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v)
     return v;
 }
 
+// Context of the cold path inside the sweep.
+struct SlowCtx {
+    const double* Hs;        // this thread's fp64 H (max-abs normalised) in shared memory, stride kRBlock
+    const float*  Ks;        // this thread's per-pair band constants K, K0 in shared memory, stride kRBlock
+    const float2* src_xy;
+    const float2* dst_xy;
+    double t;
+};
+
+// The definition in fp64 for one pair (rare: a few pairs per ten thousand).
+__device__ __noinline__ unsigned resolve_pair_f64(const SlowCtx& cx, int pt)
+{
+    double H[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) H[k] = cx.Hs[k * kRBlock];
+    const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
+    return inlier_f64(H, sp.x, sp.y, dq.x, dq.y, cx.t) ? 1u : 0u;
+}
+
+// A pair whose fp32 value fell inside the table-wide band Bc: apply the tighter per-pair band
+// K|W| + K0 to the same fp32 arithmetic (bit-identical X, Y, W, ex, ey: same operands and FMA nesting
+// as score2).  Returns 1 = surely inlier, 0 = surely outlier, 2 = still undecided.
+__device__ __forceinline__ unsigned recheck_f32(const HypConst& c, float K, float K0, float sx, float sy, float ndx, float ndy)
+{
+    const float X = __fmaf_rn(c.h[0], sx, __fmaf_rn(c.h[1], sy, c.h[2]));
+    const float Y = __fmaf_rn(c.h[3], sx, __fmaf_rn(c.h[4], sy, c.h[5]));
+    const float W = __fmaf_rn(c.h[6], sx, __fmaf_rn(c.h[7], sy, c.h[8]));
+    const float ex = __fmaf_rn(ndx, W, X), ey = __fmaf_rn(ndy, W, Y);
+    const float w2 = __fmaf_rn(W, W, -K0);
+    const float dp = __fmaf_rn(ey, ey, __fmaf_rn(ex, ex, -w2));          // diff + K0
+    const float aw = fabsf(W);
+    if (__fmaf_rn(K, aw, dp) < 0.f) return 1u;                            // diff + (K|W| + K0) < 0
+    if (__fmaf_rn(K, aw, 2.0f * K0) - dp < 0.f) return 0u;                // (K|W| + K0) - diff < 0
+    return 2u;
+}
+
+// G consecutive table entries (2G points) against one hypothesis.  `pt0` = index of the first point.
+// Fast path: 11 FFMA2 + 2 sign-bit adds + one 3-input unsigned min per entry; the cold branch is taken
+// by a warp only when one of its lanes has a pair inside the band.
+template <int G, bool ONLY_X>
+__device__ __forceinline__ void sweep_group(const HypConst& hc, const float4* __restrict__ tb, int pt0,
+                                            const SlowCtx& cx, unsigned& n_in, unsigned& n64)
+{
+    float2 a[G];
+    bool amb = false;
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        const float4 A = tb[2 * g], B = tb[2 * g + 1];
+        a[g] = score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w));
+        n_in += sign_bit(a[g].x);
+        amb |= (__float_as_uint(a[g].x) <= hc.thr);
+        if (!ONLY_X) {
+            n_in += sign_bit(a[g].y);
+            amb |= (__float_as_uint(a[g].y) <= hc.thr);
+        }
+    }
+    if (amb) {
+        unsigned mask = 0u;                                   // bit 2g + j: lane j of entry g is in the band
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            mask |= (__float_as_uint(a[g].x) <= hc.thr) ? (1u << (2 * g)) : 0u;
+            if (!ONLY_X) mask |= (__float_as_uint(a[g].y) <= hc.thr) ? (2u << (2 * g)) : 0u;
+        }
+        const float K = cx.Ks[0], K0 = cx.Ks[kRBlock];
+#pragma unroll 1
+        while (mask) {
+            const int i = __ffs(mask) - 1;
+            mask &= mask - 1u;
+            const float4 A = tb[i & ~1], B = tb[i | 1];       // entry g = i >> 1 lives at tb[2g], tb[2g + 1]
+            const bool hi = i & 1;
+            unsigned r = recheck_f32(hc, K, K0, hi ? A.y : A.x, hi ? A.w : A.z, hi ? B.y : B.x, hi ? B.w : B.z);
+            if (r == 2u) { r = resolve_pair_f64(cx, pt0 + i); ++n64; }
+            n_in += r;
+        }
+    }
+}
+
+constexpr int kGroup = 4;     // table entries per slow-path check
+
 __global__ void __launch_bounds__(kRBlock, 2)
 ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts,
                     const float4* __restrict__ table, int n_pairs, const int4* __restrict__ hyp_idx,
-                    int n_hyp, double inv_t, int* __restrict__ counts, RansacHeader* __restrict__ hdr,
-                    unsigned* __restrict__ worklist)
+                    int n_hyp, double inv_t, double t, int* __restrict__ counts, RansacHeader* __restrict__ hdr)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4* stage_buf = reinterpret_cast<float4*>(smem_raw);                       // kStages * kChunkPairs * 2 float4
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(kStages) * kChunkPairs * 32);
+    double* Hstash = reinterpret_cast<double*>(smem_raw + size_t(kStages) * kChunkPairs * 32);   // [9][kRBlock]
+    float* Kstash = reinterpret_cast<float*>(Hstash + 9 * kRBlock);                               // [2][kRBlock]
+    uint64_t* full = reinterpret_cast<uint64_t*>(Kstash + 2 * kRBlock);
 
     const int n_chunks = (n_pairs + kChunkPairs - 1) / kChunkPairs;
     if (threadIdx.x == 0) {
@@ -239,36 +320,34 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
         const float bounds[4] = { __uint_as_float(hdr->bound_bits[0]), __uint_as_float(hdr->bound_bits[1]),
                                   __uint_as_float(hdr->bound_bits[2]), __uint_as_float(hdr->bound_bits[3]) };
         double s[8], d[8], Hn[9];
-        const int4 id = active ? __ldg(hyp_idx + hidx) : make_int4(0, 1, 2, 3);
+        const int4 id = active ? __ldg(hyp_idx + hidx) : make_int4(0, 0, 0, 0);    // inactive: degenerate => sure outliers
         gather_sets(src_xy, dst_xy, id, s, d);
         ok = make_hypothesis(s, d, inv_t, bounds, Hn, hc) && active;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) Hstash[k * kRBlock + threadIdx.x] = Hn[k];
+        Kstash[threadIdx.x] = hc.K; Kstash[kRBlock + threadIdx.x] = hc.K0;
     }
+    SlowCtx cx;
+    cx.Hs = Hstash + threadIdx.x; cx.Ks = Kstash + threadIdx.x; cx.src_xy = src_xy; cx.dst_xy = dst_xy; cx.t = t;
 
-    unsigned n_in = 0, n_out = 0;
-    const int full_pairs = n_pts >> 1;                     // pairs holding two distinct points
+    unsigned n_in = 0, n64 = 0;
+    const int full_pairs = n_pts >> 1;                     // entries holding two distinct points
     for (int c = 0; c < n_chunks; ++c) {
         const int st = c % kStages;
         mbar_wait(&full[st], (c / kStages) & 1);
         const float4* tb = stage_buf + size_t(st) * kChunkPairs * 2;
         const int first = c * kChunkPairs;
         const int pairs = min(kChunkPairs, full_pairs - first);          // may be <= 0 in a tail-only chunk
-#pragma unroll 4
-        for (int k = 0; k < pairs; ++k) {
-            const float4 A = tb[2 * k], B = tb[2 * k + 1];
-            float2 a, nb;
-            score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w), a, nb);
-            n_in += sign_bit(a.x) + sign_bit(a.y);
-            n_out += sign_bit(nb.x) + sign_bit(nb.y);
-        }
-        // odd tail point: the duplicated pair counts once
-        if ((n_pts & 1) && full_pairs >= first && full_pairs < first + kChunkPairs) {
-            const int k = full_pairs - first;
-            const float4 A = tb[2 * k], B = tb[2 * k + 1];
-            float2 a, nb;
-            score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w), a, nb);
-            n_in += sign_bit(a.x);
-            n_out += sign_bit(nb.x);
-        }
+        int k = 0;
+#pragma unroll 1
+        for (; k + kGroup <= pairs; k += kGroup)
+            sweep_group<kGroup, false>(hc, tb + 2 * k, 2 * (first + k), cx, n_in, n64);
+#pragma unroll 1
+        for (; k < pairs; ++k)
+            sweep_group<1, false>(hc, tb + 2 * k, 2 * (first + k), cx, n_in, n64);
+        // odd tail point: the duplicated entry counts once
+        if ((n_pts & 1) && full_pairs >= first && full_pairs < first + kChunkPairs)
+            sweep_group<1, true>(hc, tb + 2 * (full_pairs - first), 2 * full_pairs, cx, n_in, n64);
         if (c + kStages < n_chunks) {                      // refill this stage (uniform branch)
             __syncthreads();
             if (threadIdx.x == 0) {
@@ -280,74 +359,21 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
         }
     }
 
-    // results: exact when no pair fell in the band; otherwise queue for the fix-up pass
-    const bool ambiguous = ok && (n_in + n_out != static_cast<unsigned>(n_pts));
     const unsigned count = ok ? n_in : 0u;
     unsigned long long key = 0ull;
-    if (active && !ambiguous) {
+    if (active) {
         if (counts) counts[hidx] = static_cast<int>(count);
         key = pack_key(count, static_cast<unsigned>(hidx));
     }
     key = warp_max_u64(key);
     if ((threadIdx.x & 31) == 0 && key != 0ull) atomicMax(&hdr->best_key, key);
-    const unsigned amb_mask = __ballot_sync(0xffffffffu, ambiguous);
+    // statistics: hypotheses that needed fp64 decisions, and how many pairs
+    const unsigned amb_mask = __ballot_sync(0xffffffffu, n64 != 0u);
     if (amb_mask) {
-        const int lane = threadIdx.x & 31;
-        unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(&hdr->n_fixup, static_cast<unsigned long long>(__popc(amb_mask)));
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if (ambiguous) worklist[base + __popc(amb_mask & ((1u << lane) - 1u))] = static_cast<unsigned>(hidx);
-    }
-}
-
-// ---- 3. fix-up -------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kFixBlock)
-ransac_fixup_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts,
-                    const float4* __restrict__ table, const int4* __restrict__ hyp_idx, double inv_t, double t,
-                    int* __restrict__ counts, RansacHeader* __restrict__ hdr, const unsigned* __restrict__ worklist)
-{
-    const int lane = threadIdx.x & 31;
-    const int warp = (blockIdx.x * kFixBlock + threadIdx.x) >> 5;
-    const int n_warps = (gridDim.x * kFixBlock) >> 5;
-    const unsigned long long n_work = hdr->n_fixup;
-    const float bounds[4] = { __uint_as_float(hdr->bound_bits[0]), __uint_as_float(hdr->bound_bits[1]),
-                              __uint_as_float(hdr->bound_bits[2]), __uint_as_float(hdr->bound_bits[3]) };
-    const int full_pairs = n_pts >> 1;
-    for (unsigned long long w = warp; w < n_work; w += n_warps) {
-        const unsigned hidx = worklist[w];
-        HypConst hc;
-        double s[8], d[8], Hn[9];
-        gather_sets(src_xy, dst_xy, __ldg(hyp_idx + hidx), s, d);
-        make_hypothesis(s, d, inv_t, bounds, Hn, hc);
-        unsigned cnt = 0, n64 = 0;
-        const int n_pairs = (n_pts + 1) >> 1;
-        for (int k = lane; k < n_pairs; k += 32) {
-            const float4 A = __ldg(table + 2 * k), B = __ldg(table + 2 * k + 1);
-            float2 a, nb;
-            score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w), a, nb);
-            const bool two = k < full_pairs;
-            // lane .x
-            if (sign_bit(a.x)) ++cnt;
-            else if (!sign_bit(nb.x)) {
-                const float2 sp = __ldg(src_xy + 2 * k), dq = __ldg(dst_xy + 2 * k);
-                cnt += inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, t) ? 1u : 0u;
-                ++n64;
-            }
-            if (two) {
-                if (sign_bit(a.y)) ++cnt;
-                else if (!sign_bit(nb.y)) {
-                    const float2 sp = __ldg(src_xy + 2 * k + 1), dq = __ldg(dst_xy + 2 * k + 1);
-                    cnt += inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, t) ? 1u : 0u;
-                    ++n64;
-                }
-            }
-        }
-        cnt = __reduce_add_sync(0xffffffffu, cnt);
-        n64 = __reduce_add_sync(0xffffffffu, n64);
-        if (lane == 0) {
-            if (counts) counts[hidx] = static_cast<int>(cnt);
-            atomicMax(&hdr->best_key, pack_key(cnt, hidx));
-            atomicAdd(&hdr->n_pairs_f64, static_cast<unsigned long long>(n64));
+        const unsigned tot = __reduce_add_sync(0xffffffffu, n64);
+        if ((threadIdx.x & 31) == 0) {
+            atomicAdd(&hdr->n_fixup, static_cast<unsigned long long>(__popc(amb_mask)));
+            atomicAdd(&hdr->n_pairs_f64, static_cast<unsigned long long>(tot));
         }
     }
 }
@@ -381,7 +407,8 @@ static size_t table_bytes(int32_t n_pts) { return size_t((n_pts + 1) / 2) * 32; 
 extern "C" size_t hg_ransac_workspace_bytes(int32_t n_pts, int64_t n_hyp)
 {
     if (n_pts < 0 || n_hyp < 0) return 0;
-    return hg::kHeaderBytes + hg::align16(hg::table_bytes(n_pts)) + hg::align16(size_t(n_hyp) * sizeof(unsigned));
+    (void)n_hyp;                                   // no per-hypothesis scratch
+    return hg::kHeaderBytes + hg::align16(hg::table_bytes(n_pts));
 }
 
 extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy, int32_t n_pts,
@@ -406,7 +433,6 @@ extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst
     unsigned char* ws = static_cast<unsigned char*>(workspace);
     RansacHeader* hdr = reinterpret_cast<RansacHeader*>(ws);
     float4* table = reinterpret_cast<float4*>(ws + kHeaderBytes);
-    unsigned* worklist = reinterpret_cast<unsigned*>(ws + kHeaderBytes + align16(table_bytes(n_pts)));
     const float2* s2 = reinterpret_cast<const float2*>(src_xy);
     const float2* d2 = reinterpret_cast<const float2*>(dst_xy);
     const int4* idx4 = reinterpret_cast<const int4*>(hyp_idx);
@@ -422,7 +448,8 @@ extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst
         if (launch_status() != HG_OK) return HG_ERR_CUDA;
     }
     {
-        const size_t smem = size_t(kStages) * kChunkPairs * 32 + kStages * sizeof(uint64_t);
+        const size_t smem = size_t(kStages) * kChunkPairs * 32 + size_t(9) * kRBlock * sizeof(double) + size_t(2) * kRBlock * sizeof(float) +
+                            kStages * sizeof(uint64_t);
         static bool attr_set = false;          // idempotent; a race only repeats the same call
         if (!attr_set) {
             if (cudaFuncSetAttribute(ransac_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
@@ -430,16 +457,8 @@ extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst
             attr_set = true;
         }
         const unsigned blocks = static_cast<unsigned>((n_hyp + kRBlock - 1) / kRBlock);
-        ransac_score_kernel<<<blocks, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, idx4, int(n_hyp), inv_t,
-                                                           counts, hdr, worklist);
-        if (launch_status() != HG_OK) return HG_ERR_CUDA;
-    }
-    {
-        int64_t warps = n_hyp;                                   // at most one warp per hypothesis
-        int64_t blocks = (warps * 32 + kFixBlock - 1) / kFixBlock;
-        if (blocks > 148 * 8) blocks = 148 * 8;
-        ransac_fixup_kernel<<<static_cast<unsigned>(blocks), kFixBlock, 0, st>>>(s2, d2, n_pts, table, idx4, inv_t, t,
-                                                                                 counts, hdr, worklist);
+        ransac_score_kernel<<<blocks, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, idx4, int(n_hyp), inv_t, t,
+                                                           counts, hdr);
         if (launch_status() != HG_OK) return HG_ERR_CUDA;
     }
     if (best_H || best_index || best_count) {

@@ -84,8 +84,8 @@ def test_grid_argument_validation():
 def test_ransac_argument_validation_and_workspace():
     L = hg.lib()
     ws = L.hg_ransac_workspace_bytes
-    assert ws(4096, 1 << 20) >= 64 + 4096 * 16 + 4 * (1 << 20)
-    assert ws(4097, 10) >= 64 + 2049 * 32 + 40
+    assert ws(4096, 1 << 20) >= 64 + 4096 * 16
+    assert ws(4097, 10) >= 64 + 2049 * 32
     assert ws(4096, 1 << 20) % 16 == 0
     f = L.hg_ransac_hypothesize_score
     args_ok = [FAKE, FAKE, 100, FAKE, 10, 3.0, FAKE, FAKE, FAKE, FAKE, FAKE, 1 << 30, None]

@@ -125,6 +125,24 @@ HG_API int hg_offsets_to_grid(const float* offsets, float x0, float y0, float w,
                        hg_norm_t norm, void* cuda_stream);
 
 /* --------------------------------------------------------------------------------------------
+ * hg_aca_rect_batched -- TensorACA for a rectangular source (Sec. 5.3, Eq. 42-45, Algorithm 1,
+ * P:540-591): the source quadrangle is the fixed rectangle TL = (x0,y0), extents (w,h), shared by
+ * the whole batch, so H_A1 is trivial, Q3 = (1,1,1) and H follows from the target corners alone
+ * (47 FLOPs; 44 for a square).  Only the offsets are read: 32 B in + 36 B out per homography.
+ *   offsets : corner offsets, target corner = source corner + offset, corner order TL,TR,BR,BL
+ *             (roles M=TL, N=TR, Q=BR, P=BL, reading R6);
+ *             HG_SOA: float[8][n] planes TL.x,TL.y,TR.x,...,BL.y;  HG_AOS: float[n][4][2]   (read)
+ *   H       : HG_SOA float[9][n] / HG_AOS float[n][3][3], scaled per `norm`; HG_NORM_NONE returns
+ *             Eq. 45's scale (a degree-2 polynomial of the target coordinates times w)       (write)
+ * The same H (up to scale) as hg_aca_batched on the explicit corners.  Errors: HG_ERR_INVALID_ARG
+ * (NULL with n > 0, n < 0, w == 0 or h == 0, bad enum), HG_ERR_ALIGNMENT (offsets or H not 16-byte
+ * aligned), HG_ERR_CUDA.
+ * -------------------------------------------------------------------------------------------- */
+HG_API int hg_aca_rect_batched(const float* offsets, float x0, float y0, float w, float h, float* H,
+                        int64_t n, hg_layout_t layout, hg_norm_t norm, hg_precision_t prec,
+                        void* cuda_stream);
+
+/* --------------------------------------------------------------------------------------------
  * hg_ransac_hypothesize_score -- RANSAC hypothesis generation fused with inlier scoring
  * (hypothesise-and-verify loop, Sec. 2.2; parallel hypotheses P:703).
  * For every hypothesis: gather its 4 correspondences, ACA solve (fp64 internal), then count

@@ -91,7 +91,7 @@ void hgo_normal_form(double* H, int64_t n)
     for (int64_t i = 0; i < n; ++i) hgo::normal_form(H + 9 * i);
 }
 
-// Paper-style operation counts of one evaluation.  method: 1 = ACA, 2 = SKS.
+// Paper-style operation counts of one evaluation.  method: 1 = ACA, 2 = SKS, 3 = Algorithm 1.
 // out = { add/sub, mul, div, FLOPs = add + mul + 4*div }.
 void hgo_op_counts(int method, int64_t out[4])
 {
@@ -102,8 +102,10 @@ void hgo_op_counts(int method, int64_t out[4])
     Counted s[8], d[8], H[9];
     for (int i = 0; i < 8; ++i) { s[i] = Counted(sv[i]); d[i] = Counted(dv[i]); }
     Counted::reset();
-    if (method == 1) hgo::aca<Counted>(s, d, H);
-    else             hgo::sks<Counted>(s, d, H);
+    if (method == 1)      hgo::aca<Counted>(s, d, H);
+    else if (method == 2) hgo::sks<Counted>(s, d, H);
+    else                  // 3 = Algorithm 1 (TensorACA-rect) on a 300 x 240 rectangle, r_rec = 1.25
+        hgo::aca_rect<Counted>(Counted(10.0), Counted(20.0), Counted(300.0), Counted(1.25), d, d + 2, d + 6, d + 4, H);
     out[0] = Counted::n_add;
     out[1] = Counted::n_mul;
     out[2] = Counted::n_div;

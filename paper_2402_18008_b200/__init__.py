@@ -19,7 +19,7 @@ from . import _build
 __all__ = [
     "HgError", "lib", "lib_path", "SOA", "AOS", "NORM_NONE", "NORM_H33", "NORM_FROBENIUS",
     "PREC_F64", "PREC_F32", "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host",
-    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_ransac_workspace_bytes",
+    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_ransac_workspace_bytes",
     "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_status_string",
     "hg_version", "hg_built_for_sm", "EXPORTS",
 ]
@@ -34,7 +34,7 @@ RANSAC_STAT_WORDS = 4
 # every symbol include/hg.h declares
 EXPORTS = [
     "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-    "hg_offsets_to_grid", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
+    "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
     "hg_ransac_hypothesize_score_host", "hg_status_string", "hg_version", "hg_built_for_sm",
 ]
 
@@ -68,6 +68,7 @@ def lib() -> ctypes.CDLL:
         L.hg_sks_batched_host.argtypes = host_args
         L.hg_offsets_to_grid.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _c_i32, _c_i32, _vp, _vp,
                                          _c_i64, _c_int, _vp]
+        L.hg_aca_rect_batched.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
         L.hg_ransac_workspace_bytes.argtypes = [_c_i32, _c_i64]
         L.hg_ransac_workspace_bytes.restype = ctypes.c_size_t
         L.hg_ransac_hypothesize_score.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp,
@@ -76,7 +77,8 @@ def lib() -> ctypes.CDLL:
         L.hg_status_string.argtypes = [_c_int]
         L.hg_status_string.restype = ctypes.c_char_p
         for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-                     "hg_offsets_to_grid", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host",
+                     "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_ransac_hypothesize_score",
+                     "hg_ransac_hypothesize_score_host",
                      "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
         _lib = L
@@ -214,6 +216,21 @@ def hg_offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w
                                       _ptr(grid, torch.float32, "cuda", "grid"), n, int(norm), _stream(stream))
     _check(st, "hg_offsets_to_grid")
     return H, grid
+
+
+def hg_aca_rect_batched(offsets, x0: float, y0: float, w: float, h: float, H=None, layout: int = AOS,
+                        norm: int = NORM_NONE, prec: int = PREC_F64, stream=None) -> torch.Tensor:
+    """Algorithm 1 (rectangular source).  AoS: offsets [n,4,2] -> H [n,3,3]; SoA: [8,n] -> [9,n]."""
+    n = _n_sets(offsets, layout)
+    if H is None:
+        H = torch.empty(_h_shape(n, layout), dtype=torch.float32, device=offsets.device)
+    elif tuple(H.shape) != _h_shape(n, layout):
+        raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
+    po, ph = _ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(H, torch.float32, "cuda", "H")
+    with torch.cuda.device(offsets.device):
+        st = lib().hg_aca_rect_batched(po, x0, y0, w, h, ph, n, int(layout), int(norm), int(prec), _stream(stream))
+    _check(st, "hg_aca_rect_batched")
+    return H
 
 
 def hg_ransac_workspace_bytes(n_pts: int, n_hyp: int) -> int:

@@ -1,0 +1,142 @@
+// hg_rect.cu -- hg_aca_rect_batched: TensorACA for a rectangular source.
+//
+// Deep-homography pipelines predict the offsets of the four corners of a FIXED source rectangle
+// (P:25).  For a rectangle H_A1 is trivial and Q3 = (1,1,1) (Eq. 42-43),
+// so H follows from the target quadrangle alone (Eq. 44-45; Algorithm 1):
+// 47 FLOPs, and only the 8 offsets are read -- 32 B in + 36 B out = 68 B per homography instead of
+// the general solver's 100 B.  Same streaming skeleton as hg_batched.cu; fp64 registers, fp32 I/O.
+#include "hg_device.cuh"
+#include "hg_host.h"
+
+namespace hg {
+
+constexpr int kRectBlock = 256;
+
+struct RectSrc {            // the source rectangle {M1.x, M1.y, w_rec, r_rec} of P:544 plus its height
+    double x0, y0, w, h, r; // r = w / h  (reading R6)
+};
+
+// Eq. 45 evaluated column by column, as Algorithm 1 does:
+//   col1 = Q4.x * n2 + t2 * m2,   col2 = r_rec * (Q4.y * p2 + t2 * m2),
+//   col3 = -M1.x * col1 - M1.y * col2 - w_rec * t2 * m2          (m2, n2, p2 homogeneous, weight 1)
+// with Q4 = f_A2-scaled fourth point of the target quadrangle in its affine frame (Eq. 28) and
+// t2 = f_A2 - Q4.x - Q4.y (Eq. 30).  Corner order of `o` is TL,TR,BR,BL; roles M=TL, N=TR, Q=BR, P=BL.
+// The scale is Eq. 45's (the negative of Algorithm 1's printed cross-product convention, R6).
+template <class T>
+__device__ __forceinline__ void aca_rect_solve(const RectSrc& rs, const T o[8], T H[9])
+{
+    const T x0 = T(rs.x0), y0 = T(rs.y0), w = T(rs.w), h = T(rs.h), r = T(rs.r);
+    const T m2x = x0 + o[0],     m2y = y0 + o[1];
+    const T n2x = x0 + w + o[2], n2y = y0 + o[3];
+    const T q2x = x0 + w + o[4], q2y = y0 + h + o[5];
+    const T p2x = x0 + o[6],     p2y = y0 + h + o[7];
+    const T ax = n2x - m2x, ay = n2y - m2y;            // M2N2
+    const T bx = p2x - m2x, by = p2y - m2y;            // M2P2
+    const T qx = q2x - m2x, qy = q2y - m2y;            // M2Q2
+    const T fA2 = det2(ax, ay, bx, by);
+    const T Q4x = det2(qx, qy, bx, by);
+    const T Q4y = det2(ax, ay, qx, qy);
+    const T t2 = fA2 - Q4x - Q4y;
+    const T bx3 = t2 * m2x, by3 = t2 * m2y;            // b = t2 * m2 (Algorithm 1 step 3)
+    const T h11 = K<T>::fma(Q4x, n2x, bx3), h21 = K<T>::fma(Q4x, n2y, by3), h31 = Q4x + t2;
+    const T h12 = r * K<T>::fma(Q4y, p2x, bx3), h22 = r * K<T>::fma(Q4y, p2y, by3), h32 = r * (Q4y + t2);
+    H[0] = h11; H[1] = h12; H[2] = -K<T>::fma(x0, h11, K<T>::fma(y0, h12, w * bx3));
+    H[3] = h21; H[4] = h22; H[5] = -K<T>::fma(x0, h21, K<T>::fma(y0, h22, w * by3));
+    H[6] = h31; H[7] = h32; H[8] = -K<T>::fma(x0, h31, K<T>::fma(y0, h32, w * t2));
+}
+
+// SoA: offsets = float[8][n] planes (TL.x, TL.y, TR.x, ..., BL.y), H = float[9][n]; thread per V items.
+template <class T, int V>
+__global__ void __launch_bounds__(kRectBlock)
+rect_soa_kernel(const float* __restrict__ offsets, RectSrc rs, float* __restrict__ H, int64_t n_vec, int64_t stride, int norm)
+{
+    const int64_t t = static_cast<int64_t>(blockIdx.x) * kRectBlock + threadIdx.x;
+    if (t >= n_vec) return;
+    const int64_t off = t * V;
+    Vec<V> o[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) o[k] = ld_stream<V>(offsets + k * stride + off);
+    Vec<V> hv[9];
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        T ov[8], Hv[9];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) ov[k] = static_cast<T>(o[k].v[v]);
+        aca_rect_solve<T>(rs, ov, Hv);
+        normalise<T>(Hv, norm);
+#pragma unroll
+        for (int k = 0; k < 9; ++k) hv[k].v[v] = static_cast<float>(Hv[k]);
+    }
+#pragma unroll
+    for (int k = 0; k < 9; ++k) st_stream<V>(H + k * stride + off, hv[k]);
+}
+
+// AoS: offsets = float[n][4][2] (what a regression head emits), H = float[n][3][3].  A thread reads its
+// own 32 B record with two 128-bit loads; the 36-byte H records go through shared memory so the block
+// writes one contiguous 128-bit-vectorised span.
+template <class T>
+__global__ void __launch_bounds__(kRectBlock)
+rect_aos_kernel(const float* __restrict__ offsets, RectSrc rs, float* __restrict__ H, int64_t n, int norm)
+{
+    __shared__ __align__(16) float stage[kRectBlock * 9];
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * kRectBlock;
+    const int64_t i = base + threadIdx.x;
+    if (i < n) {
+        const float4* op = reinterpret_cast<const float4*>(offsets + 8 * i);
+        const float4 o0 = __ldcs(op), o1 = __ldcs(op + 1);
+        const T ov[8] = { T(o0.x), T(o0.y), T(o0.z), T(o0.w), T(o1.x), T(o1.y), T(o1.z), T(o1.w) };
+        T Hv[9];
+        aca_rect_solve<T>(rs, ov, Hv);
+        normalise<T>(Hv, norm);
+#pragma unroll
+        for (int k = 0; k < 9; ++k) stage[threadIdx.x * 9 + k] = static_cast<float>(Hv[k]);
+    }
+    __syncthreads();
+    const int64_t rem = n - base;
+    const int cnt = static_cast<int>(rem < kRectBlock ? rem : kRectBlock) * 9;
+    float* out = H + 9 * base;
+    const int n4 = cnt >> 2;
+    for (int j = threadIdx.x; j < n4; j += kRectBlock)
+        __stcs(reinterpret_cast<float4*>(out) + j, reinterpret_cast<const float4*>(stage)[j]);
+    for (int j = (n4 << 2) + threadIdx.x; j < cnt; j += kRectBlock) out[j] = stage[j];
+}
+
+template <class T>
+static int rect_dispatch(const float* offsets, const RectSrc& rs, float* H, int64_t n, hg_layout_t layout, int norm, cudaStream_t st)
+{
+    if (layout == HG_SOA) {
+        if (n % 4 == 0) {
+            const int64_t nv = n / 4, blocks = (nv + kRectBlock - 1) / kRectBlock;
+            rect_soa_kernel<T, 4><<<static_cast<unsigned>(blocks), kRectBlock, 0, st>>>(offsets, rs, H, nv, n, norm);
+        } else {
+            const int64_t blocks = (n + kRectBlock - 1) / kRectBlock;
+            rect_soa_kernel<T, 1><<<static_cast<unsigned>(blocks), kRectBlock, 0, st>>>(offsets, rs, H, n, n, norm);
+        }
+    } else {
+        const int64_t blocks = (n + kRectBlock - 1) / kRectBlock;
+        rect_aos_kernel<T><<<static_cast<unsigned>(blocks), kRectBlock, 0, st>>>(offsets, rs, H, n, norm);
+    }
+    return launch_status();
+}
+
+}  // namespace hg
+
+extern "C" int hg_aca_rect_batched(const float* offsets, float x0, float y0, float w, float h, float* H, int64_t n,
+                                   hg_layout_t layout, hg_norm_t norm, hg_precision_t prec, void* cuda_stream)
+{
+    using namespace hg;
+    if (n < 0) return HG_ERR_INVALID_ARG;
+    if (layout != HG_SOA && layout != HG_AOS) return HG_ERR_INVALID_ARG;
+    if (norm != HG_NORM_NONE && norm != HG_NORM_H33 && norm != HG_NORM_FROBENIUS) return HG_ERR_INVALID_ARG;
+    if (prec != HG_PREC_F64 && prec != HG_PREC_F32) return HG_ERR_INVALID_ARG;
+    if (!(w != 0.0f) || !(h != 0.0f) || !(w == w) || !(h == h)) return HG_ERR_INVALID_ARG;
+    if (n == 0) return HG_OK;
+    if (!offsets || !H) return HG_ERR_INVALID_ARG;
+    if (!aligned16(offsets) || !aligned16(H)) return HG_ERR_ALIGNMENT;
+    if ((n + kRectBlock - 1) / kRectBlock > 0x7fffffffLL) return HG_ERR_INVALID_ARG;
+    RectSrc rs;
+    rs.x0 = x0; rs.y0 = y0; rs.w = w; rs.h = h; rs.r = double(w) / double(h);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    return prec == HG_PREC_F64 ? rect_dispatch<double>(offsets, rs, H, n, layout, int(norm), st)
+                               : rect_dispatch<float>(offsets, rs, H, n, layout, int(norm), st);
+}

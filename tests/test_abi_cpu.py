@@ -81,6 +81,25 @@ def test_grid_argument_validation():
     assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE, -5, hg.NORM_H33, None) == -1
 
 
+def test_rect_argument_validation():
+    f = hg.lib().hg_aca_rect_batched
+    ok = [FAKE, 0.0, 0.0, 127.0, 127.0, FAKE, 8, hg.AOS, hg.NORM_H33, hg.PREC_F64, None]
+
+    def call(**kw):
+        a = list(ok)
+        names = ["off", "x0", "y0", "w", "h", "H", "n", "layout", "norm", "prec", "st"]
+        for k, v in kw.items():
+            a[names.index(k)] = v
+        return f(*a)
+
+    assert call(n=0) == 0
+    assert call(n=-1) == -1
+    assert call(w=0.0) == -1 and call(h=0.0) == -1 and call(w=float("nan")) == -1
+    assert call(layout=7) == -1 and call(norm=9) == -1 and call(prec=3) == -1
+    assert call(off=None) == -1 and call(H=None) == -1
+    assert call(off=FAKE + 4) == -2 and call(H=FAKE + 8) == -2
+
+
 def test_ransac_argument_validation_and_workspace():
     L = hg.lib()
     ws = L.hg_ransac_workspace_bytes

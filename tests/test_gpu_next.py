@@ -1,0 +1,71 @@
+"""GPU parity of the SURVEY.md 8(f) rows against the fp64 oracle (same tolerances as the general
+solvers: reading R12 for H)."""
+import numpy as np
+import pytest
+import torch
+
+import hg_workloads as W
+import oracle
+import paper_2402_18008_b200 as hg
+from util import align_to, project
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+# ---- 8(f)-1: hg_aca_rect_batched (Algorithm 1) ----------------------------------------
+@pytest.mark.parametrize("rect,n,max_off", [((0.0, 0.0, 127.0, 127.0), 1024, 32.0),      # C1
+                                            ((16.0, 40.0, 300.0, 120.0), 4099, 30.0),     # ragged tail, r_rec = 2.5
+                                            ((-50.0, 7.0, 64.0, 200.0), 777, 12.0),
+                                            ((0.0, 0.0, 1.0, 1.0), 5, 0.2),
+                                            ((0.0, 0.0, 127.0, 127.0), 1, 32.0)])
+@pytest.mark.parametrize("layout", ["aos", "soa"])
+def test_aca_rect_matches_oracle(rect, n, max_off, layout):
+    x0, y0, w, h = rect
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 1 + n, max_offset=max_off)
+    H_ref = oracle.aca_rect(off.numpy(), x0, y0, w, h)
+    if layout == "aos":
+        H = hg.hg_aca_rect_batched(off.to(DEV), x0, y0, w, h, layout=hg.AOS, norm=hg.NORM_FROBENIUS).cpu().numpy()
+    else:
+        o_soa = off.reshape(n, 8).t().contiguous()
+        H = hg.hg_aca_rect_batched(o_soa.to(DEV), x0, y0, w, h, layout=hg.SOA, norm=hg.NORM_FROBENIUS)
+        H = H.t().reshape(n, 3, 3).cpu().numpy()
+    a, b = align_to(H.astype(np.float64), H_ref)
+    assert (np.abs(a - b) <= 1e-4 * np.abs(b) + 1e-7).all()
+    assert np.abs(a - b).max() <= 2e-7
+    # defining property on the fp32 result: corners map to corner + offset within the north_star tolerance
+    src = np.broadcast_to(W.patch_corners(x0, y0, w, h).numpy().astype(np.float64), (n, 4, 2))
+    dst = src + off.numpy().astype(np.float64)
+    assert np.abs(project(H.astype(np.float64), src) - dst).max() <= 1e-3
+
+
+def test_aca_rect_norms_scale_and_agreement_with_general_entry_points():
+    n = 4096
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 5).to(DEV)
+    Hn = hg.hg_aca_rect_batched(off, 0.0, 0.0, 127.0, 127.0, norm=hg.NORM_NONE)
+    H1 = hg.hg_aca_rect_batched(off, 0.0, 0.0, 127.0, 127.0, norm=hg.NORM_H33)
+    Hf = hg.hg_aca_rect_batched(off, 0.0, 0.0, 127.0, 127.0, norm=hg.NORM_FROBENIUS)
+    assert torch.all(H1[:, 2, 2] == 1.0)
+    assert ((Hf.double() ** 2).sum(dim=(1, 2)).sqrt() - 1.0).abs().max().item() <= 3e-7
+    # raw scale: Eq. 45, i.e. minus Algorithm 1's printed scale (reading R6) -- compare with the oracle's raw H
+    H_ref = oracle.aca_rect(off.cpu().numpy(), 0.0, 0.0, 127.0, 127.0)
+    raw = Hn.cpu().numpy().astype(np.float64)
+    assert (np.abs(raw + H_ref) <= 1e-6 * np.abs(H_ref).max(axis=(1, 2), keepdims=True)).all()
+    # the general offsets entry point (full ACA on the explicit corners) gives the same H
+    Hg, _ = hg.hg_offsets_to_grid(off, 0.0, 0.0, 127.0, 127.0, 128, 128, want_grid=False, norm=hg.NORM_H33)
+    assert (Hg - H1).abs().max().item() <= 2e-5 * H1.abs().max().item()
+    # fp32 arithmetic: sanity only (not a parity configuration)
+    H32 = hg.hg_aca_rect_batched(off, 0.0, 0.0, 127.0, 127.0, norm=hg.NORM_H33, prec=hg.PREC_F32)
+    assert (H32 - H1).abs().max().item() <= 1e-2 * H1.abs().max().item()
+
+
+def test_aca_rect_large_batch_sampled():
+    """2^22 items in the launch configuration bench.py times (AoS in, AoS out); the oracle checks a strided sample."""
+    n = 1 << 22
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 6, device=DEV)
+    H = hg.hg_aca_rect_batched(off, 0.0, 0.0, 127.0, 127.0, norm=hg.NORM_H33)
+    sel = torch.arange(0, n, 4099, device=DEV)
+    H_ref = oracle.aca_rect(off[sel].cpu().numpy(), 0.0, 0.0, 127.0, 127.0)
+    a, b = align_to(H[sel].cpu().numpy().astype(np.float64), H_ref)
+    assert (np.abs(a - b) <= 1e-4 * np.abs(b) + 1e-7).all()
+    assert torch.isfinite(H).all()

@@ -225,6 +225,10 @@ def test_operation_counts():
     # Table 3 prints 157; the formulas as printed (Eq. 6-16) evaluate in 160 with 5 reciprocals --
     # DESIGN.md reading R15.  11 of the 14 step counts of Table 3 are matched exactly.
     assert sks["div"] == 5 and sks["flops"] == 160
+    # Algorithm 1 for a rectangle: 47 FLOPs; the 3 multiplications by r_rec vanish for a square (44)
+    rect = oracle.op_counts(3)
+    assert rect["flops"] == paper["aca_rect_flops"]["rectangle"] == 47 and rect["div"] == 0
+    assert rect["flops"] - 3 == paper["aca_rect_flops"]["square"]
 
 
 # ---- (vii) homogeneity degrees of the raw ACA output, Eq. 35 ------------------------

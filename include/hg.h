@@ -142,6 +142,19 @@ HG_API int hg_aca_rect_batched(const float* offsets, float x0, float y0, float w
                         int64_t n, hg_layout_t layout, hg_norm_t norm, hg_precision_t prec,
                         void* cuda_stream);
 
+/* hg_aca_rect_backward -- backward pass of the deep-homography module (the training use of
+ * TensorACA: "ACA only uses basic arithmetic operations which are naturally differential").
+ * The forward map is G(offsets) = hg_aca_rect_batched(offsets, ..., HG_AOS, HG_NORM_H33), i.e. H/h33
+ * of Algorithm 1.  Given grad_H = dL/dG, writes grad_offsets[b][k] = sum_ij grad_H[b][i][j] *
+ * dG_ij/d offsets[b][k] (reverse mode through Algorithm 1 and the division by h33, fp64 internal).
+ *   offsets      : float[n][4][2], corner order TL,TR,BR,BL               (read,  32 B per item)
+ *   grad_H       : float[n][3][3]; entry (3,3) is ignored (G33 == 1)      (read,  36 B per item)
+ *   grad_offsets : float[n][4][2]                                         (write, 32 B per item)
+ * Errors: HG_ERR_INVALID_ARG (NULL with n > 0, n < 0, w == 0 or h == 0), HG_ERR_ALIGNMENT (any
+ * pointer not 16-byte aligned), HG_ERR_CUDA.                                                      */
+HG_API int hg_aca_rect_backward(const float* offsets, float x0, float y0, float w, float h,
+                         const float* grad_H, float* grad_offsets, int64_t n, void* cuda_stream);
+
 /* --------------------------------------------------------------------------------------------
  * hg_ransac_hypothesize_score -- RANSAC hypothesis generation fused with inlier scoring
  * (hypothesise-and-verify loop, Sec. 2.2; parallel hypotheses P:703).

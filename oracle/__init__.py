@@ -140,6 +140,20 @@ def aca_rect(offsets, x0: float, y0: float, w: float, h: float) -> np.ndarray:
     return H
 
 
+def aca_rect_backward(offsets, x0: float, y0: float, w: float, h: float, grad_G, want_jac: bool = False):
+    """dL/d offsets [n,4,2] (float64) of G = H/h33 (Algorithm 1) given dL/dG [n,3,3]; optionally the
+    Jacobian dG/d offsets [n,9,8]."""
+    o = _f32(offsets, (4, 2))
+    n = o.shape[0]
+    g = np.ascontiguousarray(np.asarray(grad_G, dtype=np.float64)).reshape(n, 9)
+    go = np.empty((n, 4, 2), dtype=np.float64)
+    jac = np.empty((n, 9, 8), dtype=np.float64) if want_jac else None
+    lib().hgo_aca_rect_backward(_p(o), ctypes.c_float(x0), ctypes.c_float(y0), ctypes.c_float(w),
+                                ctypes.c_float(h), _p(g), _p(go), _p(jac) if want_jac else None,
+                                ctypes.c_int64(n))
+    return (go, jac) if want_jac else go
+
+
 def offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w: int, grid_h: int,
                     want_grid: bool = True):
     """(H float64 [n,3,3] raw scale, grid float64 [n,grid_h,grid_w,2] or None)."""

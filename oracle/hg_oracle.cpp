@@ -130,6 +130,39 @@ void hgo_aca_rect(const float* offsets, float x0, float y0, float w, float h, do
     }
 }
 
+// Backward pass of the deep-homography module: G(offsets) = H / h33 with H from
+// Algorithm 1 (what hg_aca_rect_batched returns under HG_NORM_H33).  Given grad_G = dL/dG
+// (double [n][9], the (3,3) entry is ignored because G33 == 1), returns
+// grad_off[k] = sum_ij grad_G[ij] * dG_ij / d offsets[k]   (double [n][8]),
+// the Jacobian taken by forward-mode dual numbers through aca_rect<> and the division by h33.
+// jac (nullable): double [n][9][8], dG_ij / d offsets[k].
+void hgo_aca_rect_backward(const float* offsets, float x0, float y0, float w, float h,
+                           const double* grad_G, double* grad_off, double* jac, int64_t n)
+{
+    using D = hgo::Dual<8>;
+    const double X0 = x0, Y0 = y0, Wd = w, Hd = h;
+    const double cx[4] = { X0, X0 + Wd, X0 + Wd, X0 };
+    const double cy[4] = { Y0, Y0, Y0 + Hd, Y0 + Hd };
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        D t[4][2];
+        for (int k = 0; k < 4; ++k) {
+            t[k][0] = D(cx[k]) + D::variable(static_cast<double>(offsets[8 * i + 2 * k]), 2 * k);
+            t[k][1] = D(cy[k]) + D::variable(static_cast<double>(offsets[8 * i + 2 * k + 1]), 2 * k + 1);
+        }
+        D H[9];
+        hgo::aca_rect<D>(D(X0), D(Y0), D(Wd), D(Wd / Hd), t[0], t[1], t[3], t[2], H);
+        double go[8] = { 0, 0, 0, 0, 0, 0, 0, 0 };
+        for (int e = 0; e < 9; ++e) {
+            const D G = H[e] / H[8];
+            if (jac) for (int k = 0; k < 8; ++k) jac[(9 * i + e) * 8 + k] = G.g[k];
+            if (e == 8) continue;
+            for (int k = 0; k < 8; ++k) go[k] += grad_G[9 * i + e] * G.g[k];
+        }
+        if (grad_off) for (int k = 0; k < 8; ++k) grad_off[8 * i + k] = go[k];
+    }
+}
+
 // Offsets -> H -> dense grid (reading R10).  General ACA on corners in API order
 // (M,N,P,Q = TL,TR,BR,BL), then grid[b][j][i] = pi(H_b * (x_i, y_j, 1)) with
 // x_i = x0 + i*w/(grid_w-1), y_j = y0 + j*h/(grid_h-1) (x_i = x0 when grid_w == 1).

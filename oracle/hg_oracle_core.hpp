@@ -348,4 +348,30 @@ inline Counted operator*(Counted a, Counted b) { ++Counted::n_mul; return Counte
 inline Counted operator/(Counted a, Counted b) { ++Counted::n_div; return Counted(a.v / b.v); }
 inline Counted operator-(Counted a) { return Counted(-a.v); }
 
+// ---------------------------------------------------------------------------
+// Forward-mode dual number with N partial derivatives: evaluating any of the
+// templated solvers above on Dual<N> differentiates the paper's formulas step by
+// step (sum, product and quotient rules only).  Used for the backward pass of the
+// offsets -> H map ("ACA only uses basic arithmetic operations which are naturally
+// differential").
+// ---------------------------------------------------------------------------
+template <int N>
+struct Dual {
+    double v;
+    double g[N];
+    Dual() : v(0.0) { for (int i = 0; i < N; ++i) g[i] = 0.0; }
+    Dual(double x) : v(x) { for (int i = 0; i < N; ++i) g[i] = 0.0; }
+    static Dual variable(double x, int k) { Dual r(x); r.g[k] = 1.0; return r; }
+};
+template <int N> inline Dual<N> operator+(const Dual<N>& a, const Dual<N>& b)
+{ Dual<N> r(a.v + b.v); for (int i = 0; i < N; ++i) r.g[i] = a.g[i] + b.g[i]; return r; }
+template <int N> inline Dual<N> operator-(const Dual<N>& a, const Dual<N>& b)
+{ Dual<N> r(a.v - b.v); for (int i = 0; i < N; ++i) r.g[i] = a.g[i] - b.g[i]; return r; }
+template <int N> inline Dual<N> operator*(const Dual<N>& a, const Dual<N>& b)
+{ Dual<N> r(a.v * b.v); for (int i = 0; i < N; ++i) r.g[i] = a.g[i] * b.v + a.v * b.g[i]; return r; }
+template <int N> inline Dual<N> operator/(const Dual<N>& a, const Dual<N>& b)
+{ Dual<N> r(a.v / b.v); for (int i = 0; i < N; ++i) r.g[i] = (a.g[i] - r.v * b.g[i]) / b.v; return r; }
+template <int N> inline Dual<N> operator-(const Dual<N>& a)
+{ Dual<N> r(-a.v); for (int i = 0; i < N; ++i) r.g[i] = -a.g[i]; return r; }
+
 }  // namespace hgo

@@ -19,8 +19,8 @@ from . import _build
 __all__ = [
     "HgError", "lib", "lib_path", "SOA", "AOS", "NORM_NONE", "NORM_H33", "NORM_FROBENIUS",
     "PREC_F64", "PREC_F32", "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host",
-    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_ransac_workspace_bytes",
-    "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_status_string",
+    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward",
+    "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_status_string",
     "hg_version", "hg_built_for_sm", "EXPORTS",
 ]
 
@@ -34,7 +34,8 @@ RANSAC_STAT_WORDS = 4
 # every symbol include/hg.h declares
 EXPORTS = [
     "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-    "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
+    "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_ransac_workspace_bytes",
+    "hg_ransac_hypothesize_score",
     "hg_ransac_hypothesize_score_host", "hg_status_string", "hg_version", "hg_built_for_sm",
 ]
 
@@ -69,6 +70,7 @@ def lib() -> ctypes.CDLL:
         L.hg_offsets_to_grid.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _c_i32, _c_i32, _vp, _vp,
                                          _c_i64, _c_int, _vp]
         L.hg_aca_rect_batched.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
+        L.hg_aca_rect_backward.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _vp, _c_i64, _vp]
         L.hg_ransac_workspace_bytes.argtypes = [_c_i32, _c_i64]
         L.hg_ransac_workspace_bytes.restype = ctypes.c_size_t
         L.hg_ransac_hypothesize_score.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp,
@@ -77,8 +79,8 @@ def lib() -> ctypes.CDLL:
         L.hg_status_string.argtypes = [_c_int]
         L.hg_status_string.restype = ctypes.c_char_p
         for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-                     "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_ransac_hypothesize_score",
-                     "hg_ransac_hypothesize_score_host",
+                     "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward",
+                     "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host",
                      "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
         _lib = L
@@ -231,6 +233,24 @@ def hg_aca_rect_batched(offsets, x0: float, y0: float, w: float, h: float, H=Non
         st = lib().hg_aca_rect_batched(po, x0, y0, w, h, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, "hg_aca_rect_batched")
     return H
+
+
+def hg_aca_rect_backward(offsets, x0: float, y0: float, w: float, h: float, grad_H, grad_offsets=None,
+                         stream=None) -> torch.Tensor:
+    """dL/d offsets [n,4,2] of G = H/h33 (Algorithm 1) given dL/dG [n,3,3]."""
+    n = _n_sets(offsets, AOS)
+    if tuple(grad_H.shape) != (n, 3, 3):
+        raise ValueError("grad_H must be [n,3,3]")
+    if grad_offsets is None:
+        grad_offsets = torch.empty((n, 4, 2), dtype=torch.float32, device=offsets.device)
+    elif tuple(grad_offsets.shape) != (n, 4, 2):
+        raise ValueError("grad_offsets must be [n,4,2]")
+    po, pg, pr = (_ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(grad_H, torch.float32, "cuda", "grad_H"),
+                  _ptr(grad_offsets, torch.float32, "cuda", "grad_offsets"))
+    with torch.cuda.device(offsets.device):
+        st = lib().hg_aca_rect_backward(po, x0, y0, w, h, pg, pr, n, _stream(stream))
+    _check(st, "hg_aca_rect_backward")
+    return grad_offsets
 
 
 def hg_ransac_workspace_bytes(n_pts: int, n_hyp: int) -> int:

@@ -101,6 +101,98 @@ rect_aos_kernel(const float* __restrict__ offsets, RectSrc rs, float* __restrict
     for (int j = (n4 << 2) + threadIdx.x; j < cnt; j += kRectBlock) out[j] = stage[j];
 }
 
+// ------------------------------------------------------------------------------------------
+// Backward of G(offsets) = H / h33 ("naturally differential"): reverse mode
+// through aca_rect_solve and the h33 normalisation, by hand, in fp64.  g[9] = dL/dG (g[8] ignored:
+// G33 == 1), go[8] = dL/d offsets.  ~130 FLOPs.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void aca_rect_backward(const RectSrc& rs, const double o[8], const double g[9], double go[8])
+{
+    const double x0 = rs.x0, y0 = rs.y0, w = rs.w, h = rs.h, r = rs.r;
+    // forward (same steps as aca_rect_solve)
+    const double m2x = x0 + o[0],     m2y = y0 + o[1];
+    const double n2x = x0 + w + o[2], n2y = y0 + o[3];
+    const double q2x = x0 + w + o[4], q2y = y0 + h + o[5];
+    const double p2x = x0 + o[6],     p2y = y0 + h + o[7];
+    const double ax = n2x - m2x, ay = n2y - m2y, bx = p2x - m2x, by = p2y - m2y, qx = q2x - m2x, qy = q2y - m2y;
+    const double fA2 = det2(ax, ay, bx, by), Q4x = det2(qx, qy, bx, by), Q4y = det2(ax, ay, qx, qy);
+    const double t2 = fA2 - Q4x - Q4y;
+    const double Bx = t2 * m2x, By = t2 * m2y;
+    const double h11 = fma(Q4x, n2x, Bx), h21 = fma(Q4x, n2y, By), h31 = Q4x + t2;
+    const double u12 = fma(Q4y, p2x, Bx), u22 = fma(Q4y, p2y, By), u32 = Q4y + t2;
+    const double h12 = r * u12, h22 = r * u22, h32 = r * u32;
+    const double h13 = -fma(x0, h11, fma(y0, h12, w * Bx));
+    const double h23 = -fma(x0, h21, fma(y0, h22, w * By));
+    const double h33 = -fma(x0, h31, fma(y0, h32, w * t2));
+    // G = H / h33:  dL/dh_ij = g_ij / h33 (ij != 33),  dL/dh33 = -sum g_ij h_ij / h33^2
+    const double inv = K<double>::rcp(h33);
+    double g11 = g[0] * inv, g12 = g[1] * inv, g13 = g[2] * inv;
+    double g21 = g[3] * inv, g22 = g[4] * inv, g23 = g[5] * inv;
+    double g31 = g[6] * inv, g32 = g[7] * inv;
+    const double dot = fma(g11, h11, fma(g12, h12, fma(g13, h13, fma(g21, h21, fma(g22, h22, fma(g23, h23, fma(g31, h31, g32 * h32)))))));
+    const double g33 = -dot * inv;
+    // third column: h_i3 = -(x0 h_i1 + y0 h_i2 + w {Bx, By, t2})
+    g11 = fma(-x0, g13, g11); g12 = fma(-y0, g13, g12);
+    g21 = fma(-x0, g23, g21); g22 = fma(-y0, g23, g22);
+    g31 = fma(-x0, g33, g31); g32 = fma(-y0, g33, g32);
+    double gBx = -w * g13, gBy = -w * g23, gt2 = -w * g33;
+    // second column: h_i2 = r * u_i2, u = Q4y * p2 + B
+    const double gu12 = r * g12, gu22 = r * g22, gu32 = r * g32;
+    double gQ4y = fma(gu12, p2x, fma(gu22, p2y, gu32));
+    double gp2x = gu12 * Q4y, gp2y = gu22 * Q4y;
+    gBx += gu12; gBy += gu22; gt2 += gu32;
+    // first column: h_i1 = Q4x * n2 + B
+    double gQ4x = fma(g11, n2x, fma(g21, n2y, g31));
+    double gn2x = g11 * Q4x, gn2y = g21 * Q4x;
+    gBx += g11; gBy += g21; gt2 += g31;
+    // B = t2 * m2
+    gt2 = fma(gBx, m2x, fma(gBy, m2y, gt2));
+    double gm2x = gBx * t2, gm2y = gBy * t2;
+    // t2 = fA2 - Q4x - Q4y
+    const double gfA2 = gt2;
+    gQ4x -= gt2; gQ4y -= gt2;
+    // the three determinants
+    double gax = fma(gQ4y, qy, gfA2 * by),  gay = -fma(gQ4y, qx, gfA2 * bx);
+    double gbx = -fma(gQ4x, qy, gfA2 * ay), gby = fma(gQ4x, qx, gfA2 * ax);
+    double gqx = fma(gQ4x, by, -gQ4y * ay), gqy = fma(gQ4y, ax, -gQ4x * bx);
+    // a = n2 - m2, b = p2 - m2, q = q2 - m2
+    gn2x += gax; gn2y += gay; gp2x += gbx; gp2y += gby;
+    gm2x -= gax + gbx + gqx; gm2y -= gay + gby + gqy;
+    go[0] = gm2x; go[1] = gm2y; go[2] = gn2x; go[3] = gn2y; go[4] = gqx; go[5] = gqy; go[6] = gp2x; go[7] = gp2y;
+}
+
+// offsets float[n][4][2], grad_G float[n][3][3] (staged through shared memory: 36-byte records), grad_off float[n][4][2].
+__global__ void __launch_bounds__(kRectBlock)
+rect_backward_kernel(const float* __restrict__ offsets, RectSrc rs, const float* __restrict__ grad_G,
+                     float* __restrict__ grad_off, int64_t n)
+{
+    __shared__ __align__(16) float stage[kRectBlock * 9];
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * kRectBlock;
+    const int64_t rem = n - base;
+    const int cnt = static_cast<int>(rem < kRectBlock ? rem : kRectBlock) * 9;
+    const float* gin = grad_G + 9 * base;                       // 9*256*4 B per block: 16-byte aligned
+    const int n4 = cnt >> 2;
+    for (int j = threadIdx.x; j < n4; j += kRectBlock)
+        reinterpret_cast<float4*>(stage)[j] = __ldcs(reinterpret_cast<const float4*>(gin) + j);
+    for (int j = (n4 << 2) + threadIdx.x; j < cnt; j += kRectBlock) stage[j] = gin[j];
+    const int64_t i = base + threadIdx.x;
+    float4 o0 = make_float4(0.f, 0.f, 0.f, 0.f), o1 = o0;
+    if (i < n) {
+        const float4* op = reinterpret_cast<const float4*>(offsets + 8 * i);
+        o0 = __ldcs(op); o1 = __ldcs(op + 1);
+    }
+    __syncthreads();
+    if (i >= n) return;
+    const double ov[8] = { o0.x, o0.y, o0.z, o0.w, o1.x, o1.y, o1.z, o1.w };
+    double g[9], go[8];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) g[k] = static_cast<double>(stage[threadIdx.x * 9 + k]);
+    aca_rect_backward(rs, ov, g, go);
+    float4* out = reinterpret_cast<float4*>(grad_off + 8 * i);
+    __stcs(out, make_float4(float(go[0]), float(go[1]), float(go[2]), float(go[3])));
+    __stcs(out + 1, make_float4(float(go[4]), float(go[5]), float(go[6]), float(go[7])));
+}
+
 template <class T>
 static int rect_dispatch(const float* offsets, const RectSrc& rs, float* H, int64_t n, hg_layout_t layout, int norm, cudaStream_t st)
 {
@@ -139,4 +231,22 @@ extern "C" int hg_aca_rect_batched(const float* offsets, float x0, float y0, flo
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     return prec == HG_PREC_F64 ? rect_dispatch<double>(offsets, rs, H, n, layout, int(norm), st)
                                : rect_dispatch<float>(offsets, rs, H, n, layout, int(norm), st);
+}
+
+extern "C" int hg_aca_rect_backward(const float* offsets, float x0, float y0, float w, float h, const float* grad_H,
+                                    float* grad_offsets, int64_t n, void* cuda_stream)
+{
+    using namespace hg;
+    if (n < 0) return HG_ERR_INVALID_ARG;
+    if (!(w != 0.0f) || !(h != 0.0f) || !(w == w) || !(h == h)) return HG_ERR_INVALID_ARG;
+    if (n == 0) return HG_OK;
+    if (!offsets || !grad_H || !grad_offsets) return HG_ERR_INVALID_ARG;
+    if (!aligned16(offsets) || !aligned16(grad_H) || !aligned16(grad_offsets)) return HG_ERR_ALIGNMENT;
+    if ((n + kRectBlock - 1) / kRectBlock > 0x7fffffffLL) return HG_ERR_INVALID_ARG;
+    RectSrc rs;
+    rs.x0 = x0; rs.y0 = y0; rs.w = w; rs.h = h; rs.r = double(w) / double(h);
+    const int64_t blocks = (n + kRectBlock - 1) / kRectBlock;
+    rect_backward_kernel<<<static_cast<unsigned>(blocks), kRectBlock, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        offsets, rs, grad_H, grad_offsets, n);
+    return launch_status();
 }

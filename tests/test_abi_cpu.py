@@ -100,6 +100,18 @@ def test_rect_argument_validation():
     assert call(off=FAKE + 4) == -2 and call(H=FAKE + 8) == -2
 
 
+def test_rect_backward_argument_validation():
+    f = hg.lib().hg_aca_rect_backward
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, FAKE, FAKE, 0, None) == 0
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, FAKE, FAKE, -2, None) == -1
+    assert f(FAKE, 0.0, 0.0, 0.0, 127.0, FAKE, FAKE, 4, None) == -1
+    assert f(None, 0.0, 0.0, 127.0, 127.0, FAKE, FAKE, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, None, FAKE, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, FAKE, None, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, FAKE + 4, FAKE, 4, None) == -2
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, FAKE, FAKE + 8, 4, None) == -2
+
+
 def test_ransac_argument_validation_and_workspace():
     L = hg.lib()
     ws = L.hg_ransac_workspace_bytes

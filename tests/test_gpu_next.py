@@ -69,3 +69,34 @@ def test_aca_rect_large_batch_sampled():
     a, b = align_to(H[sel].cpu().numpy().astype(np.float64), H_ref)
     assert (np.abs(a - b) <= 1e-4 * np.abs(b) + 1e-7).all()
     assert torch.isfinite(H).all()
+
+
+# ---- 8(f)-2: hg_aca_rect_backward ----------------------------------------------------------------
+# Tolerance: the kernel evaluates the reverse-mode chain in fp64 and rounds once to fp32; against the fp64
+# dual-number oracle each gradient is within a few fp32 ulps of the item's largest gradient entry.
+@pytest.mark.parametrize("rect,n,max_off", [((0.0, 0.0, 127.0, 127.0), 1024, 32.0),
+                                            ((16.0, 40.0, 300.0, 120.0), 4099, 30.0),
+                                            ((-50.0, 7.0, 64.0, 200.0), 3, 12.0)])
+def test_rect_backward_matches_oracle(rect, n, max_off):
+    x0, y0, w, h = rect
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 21 + n, max_offset=max_off)
+    g = torch.randn((n, 3, 3), generator=torch.Generator().manual_seed(n), dtype=torch.float32)
+    go = hg.hg_aca_rect_backward(off.to(DEV), x0, y0, w, h, g.to(DEV)).cpu().numpy().astype(np.float64)
+    ref = oracle.aca_rect_backward(off.numpy(), x0, y0, w, h, g.numpy().astype(np.float64))
+    scale = np.abs(ref).reshape(n, 8).max(axis=1)[:, None, None]
+    assert (np.abs(go - ref) <= 4e-7 * scale + 1e-30).all(), (np.abs(go - ref) / scale).max()
+
+
+def test_rect_backward_is_the_gradient_of_the_forward_entry_point():
+    """Directional derivative of the library's own forward (H33-normalised) against <grad, direction>."""
+    n = 512
+    rect = (0.0, 0.0, 127.0, 127.0)
+    off = (W.offsets_workload(n, seed=77) * 16).round() / 16          # exact +-2^-5 steps in fp32
+    d = torch.randn((n, 4, 2), generator=torch.Generator().manual_seed(1)).sign() * 2.0 ** -5
+    g = torch.randn((n, 3, 3), generator=torch.Generator().manual_seed(2))
+    go = hg.hg_aca_rect_backward(off.to(DEV), *rect, g.to(DEV)).double().cpu()
+    Hp = hg.hg_aca_rect_batched((off + d).to(DEV), *rect, norm=hg.NORM_H33).double().cpu()
+    Hm = hg.hg_aca_rect_batched((off - d).to(DEV), *rect, norm=hg.NORM_H33).double().cpu()
+    lhs = ((Hp - Hm) * g.double()).sum(dim=(1, 2)) / 2.0
+    rhs = (go * d.double()).sum(dim=(1, 2))
+    assert ((lhs - rhs).abs() <= 2e-3 * rhs.abs() + 1e-5 * go.abs().amax(dim=(1, 2)) * 2.0 ** -5 * 8).all()

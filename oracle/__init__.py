@@ -154,6 +154,23 @@ def aca_rect_backward(offsets, x0: float, y0: float, w: float, h: float, grad_G,
     return (go, jac) if want_jac else go
 
 
+def affine(src3, dst3) -> np.ndarray:
+    """H_A = H_A2^-1 H_A1 (Eq. 41) from three correspondences: float32 [n,3,2] x2 -> float64 [n,3,3]."""
+    s, d = _f32(src3, (3, 2)), _f32(dst3, (3, 2))
+    H = np.empty((s.shape[0], 3, 3), dtype=np.float64)
+    lib().hgo_affine(_p(s), _p(d), _p(H), ctypes.c_int64(s.shape[0]))
+    return H
+
+
+def sk(P3, Q3, dst) -> np.ndarray:
+    """Simplified SK (Eq. 17): pattern points P3, Q3 (x,y) in the anchor frame, dst float32 [n,4,2] -> Hbar [n,3,3]."""
+    d = _f32(dst, (4, 2))
+    H = np.empty((d.shape[0], 3, 3), dtype=np.float64)
+    lib().hgo_sk(ctypes.c_double(P3[0]), ctypes.c_double(P3[1]), ctypes.c_double(Q3[0]), ctypes.c_double(Q3[1]),
+                 _p(d), _p(H), ctypes.c_int64(d.shape[0]))
+    return H
+
+
 def offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w: int, grid_h: int,
                     want_grid: bool = True):
     """(H float64 [n,3,3] raw scale, grid float64 [n,grid_h,grid_w,2] or None)."""

@@ -91,7 +91,7 @@ void hgo_normal_form(double* H, int64_t n)
     for (int64_t i = 0; i < n; ++i) hgo::normal_form(H + 9 * i);
 }
 
-// Paper-style operation counts of one evaluation.  method: 1 = ACA, 2 = SKS, 3 = Algorithm 1.
+// Paper-style operation counts of one evaluation.  method: 1 = ACA, 2 = SKS, 3 = Algorithm 1, 4 = affine, 5 = SK.
 // out = { add/sub, mul, div, FLOPs = add + mul + 4*div }.
 void hgo_op_counts(int method, int64_t out[4])
 {
@@ -104,8 +104,16 @@ void hgo_op_counts(int method, int64_t out[4])
     Counted::reset();
     if (method == 1)      hgo::aca<Counted>(s, d, H);
     else if (method == 2) hgo::sks<Counted>(s, d, H);
-    else                  // 3 = Algorithm 1 (TensorACA-rect) on a 300 x 240 rectangle, r_rec = 1.25
+    else if (method == 3) // Algorithm 1 (TensorACA-rect) on a 300 x 240 rectangle, r_rec = 1.25
         hgo::aca_rect<Counted>(Counted(10.0), Counted(20.0), Counted(300.0), Counted(1.25), d, d + 2, d + 6, d + 4, H);
+    else if (method == 4) // affine from the first three correspondences (Eq. 41)
+        hgo::affine<Counted>(s, d, H);
+    else {                // 5 = simplified SK (Eq. 17); the pattern constants are not counted (Table 3: 0)
+        Counted pat[5];
+        hgo::sk_pattern<Counted>(Counted(0.3), Counted(1.7), Counted(-0.6), Counted(-1.2), pat);
+        Counted::reset();
+        hgo::sk<Counted>(pat, d, H);
+    }
     out[0] = Counted::n_add;
     out[1] = Counted::n_mul;
     out[2] = Counted::n_div;
@@ -160,6 +168,30 @@ void hgo_aca_rect_backward(const float* offsets, float x0, float y0, float w, fl
             for (int k = 0; k < 8; ++k) go[k] += grad_G[9 * i + e] * G.g[k];
         }
         if (grad_off) for (int k = 0; k < 8; ++k) grad_off[8 * i + k] = go[k];
+    }
+}
+
+// Affine from three correspondences: src3, dst3 float [n][3][2] -> H double [n][3][3] (raw scale, h33 = f_A1).
+void hgo_affine(const float* src3, const float* dst3, double* H, int64_t n)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double s[6], d[6];
+        for (int k = 0; k < 6; ++k) { s[k] = static_cast<double>(src3[6 * i + k]); d[k] = static_cast<double>(dst3[6 * i + k]); }
+        hgo::affine<double>(s, d, H + 9 * i);
+    }
+}
+
+// Simplified SK: pattern points P3, Q3 in the anchor frame (doubles), dst float [n][4][2] -> Hbar double [n][3][3].
+void hgo_sk(double P3x, double P3y, double Q3x, double Q3y, const float* dst, double* H, int64_t n)
+{
+    double pat[5];
+    hgo::sk_pattern<double>(P3x, P3y, Q3x, Q3y, pat);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double d[8];
+        load_set(dst + 8 * i, d);
+        hgo::sk<double>(pat, d, H + 9 * i);
     }
 }
 

@@ -181,6 +181,89 @@ void sks(const T s[8], const T d[8], T H[9], T* kern = nullptr)
 }
 
 // ---------------------------------------------------------------------------
+// Simplified SK (object plane -> image, Eq. 17; Table 3 row "SK"):
+//   Hbar = H * H_S1^-1 = H_S2^-1 * H_K.
+// The object coordinates are expressed in the frame of the two anchors (M -> (-1,0), N -> (+1,0),
+// so H_S1 = I and f_S1 = 1); everything that depends only on the known pattern -- P5, Q7 and the
+// reciprocal of Eq. 14's determinant -- is computed once by sk_pattern() (zero per-image cost in
+// Table 3), the per-image work is the target-side half of sks().  Hbar maps (-1,0), (1,0), P3, Q3
+// to M2, N2, P2, Q2.
+// ---------------------------------------------------------------------------
+template <class T>
+void sk_pattern(T P3x, T P3y, T Q3x, T Q3y, T pat[5])
+{
+    const T one = T(1.0);
+    const T rP3 = one / P3y, rQ3 = one / Q3y;                  // Eq. 12 with f_S1 = 1
+    const T P5x = P3x * rP3, P5y = rP3;
+    const T Q5x = Q3x * rQ3, Q5y = rQ3;
+    const T Q7x = Q5x - P5x, Q7y = Q5y - P5y;                  // Eq. 13 (R3, R4)
+    pat[0] = P5x; pat[1] = P5y; pat[2] = Q7x; pat[3] = Q7y;
+    pat[4] = one / (Q7x * Q7x - Q7y * Q7y);                    // determinant of Eq. 14
+}
+
+template <class T>
+void sk(const T pat[5], const T d[8], T H[9])
+{
+    const T half = T(0.5), one = T(1.0);
+    const T P5x = pat[0], P5y = pat[1], Q7x = pat[2], Q7y = pat[3], rden = pat[4];
+    const T M2x = d[0], M2y = d[1], N2x = d[2], N2y = d[3];
+    const T P2x = d[4], P2y = d[5], Q2x = d[6], Q2y = d[7];
+    // H_S2: Eq. 6, 7, 9.  6 + 3 FLOPs.
+    const T O2x = half * (M2x + N2x), O2y = half * (M2y + N2y);
+    const T v2x = N2x - O2x, v2y = N2y - O2y;
+    const T fS2 = v2x * v2x + v2y * v2y;
+    // P4, Q4 (Eq. 8), then H_E and dehomogenisation (Eq. 12): P6, Q6.
+    const T eP2x = P2x - O2x, eP2y = P2y - O2y;
+    const T P4x = v2x * eP2x + v2y * eP2y;
+    const T P4y = v2x * eP2y - v2y * eP2x;
+    const T eQ2x = Q2x - O2x, eQ2y = Q2y - O2y;
+    const T Q4x = v2x * eQ2x + v2y * eQ2y;
+    const T Q4y = v2x * eQ2y - v2y * eQ2x;
+    const T rP4 = one / P4y;
+    const T P6x = P4x * rP4, P6y = fS2 * rP4;
+    const T rQ4 = one / Q4y;
+    const T Q6x = Q4x * rQ4, Q6y = fS2 * rQ4;
+    const T Q8x = Q6x - P6x, Q8y = Q6y - P6y;
+    // Eq. 14 with the pattern's determinant precomputed; Eq. 15.
+    const T aK = (Q8x * Q7x - Q8y * Q7y) * rden;
+    const T bK = (Q8y * Q7x - Q8x * Q7y) * rden;
+    const T uK = P6x - aK * P5x - bK * P5y;
+    const T vK = P6y - bK * P5x - aK * P5y;
+    // Hbar = H_S2^-1 * H_K (Eq. 17; Eq. 10, 11).  20 FLOPs.
+    H[0] = v2x * aK + O2x * bK;
+    H[1] = v2x * uK - v2y + O2x * vK;
+    H[2] = v2x * bK + O2x * aK;
+    H[3] = v2y * aK + O2y * bK;
+    H[4] = v2y * uK + v2x + O2y * vK;
+    H[5] = v2y * bK + O2y * aK;
+    H[6] = bK; H[7] = vK; H[8] = aK;
+}
+
+// ---------------------------------------------------------------------------
+// Affine transformation from three correspondences (Sec. 5.2, Eq. 41 first row):
+//   H_A = H_A2^-1 * H_A1   (the core transformation is the identity), 33 FLOPs.
+// s[], d[] hold x,y of M, N, P.  H_A1 per Eq. 23 (R2), H_A2^-1 per Eq. 25 (R1).
+// ---------------------------------------------------------------------------
+template <class T>
+void affine(const T s[6], const T d[6], T H[9])
+{
+    const T a1x = s[2] - s[0], a1y = s[3] - s[1];      // M1N1
+    const T b1x = s[4] - s[0], b1y = s[5] - s[1];      // M1P1
+    const T fA1 = a1x * b1y - a1y * b1x;
+    const T a2x = d[2] - d[0], a2y = d[3] - d[1];      // M2N2
+    const T b2x = d[4] - d[0], b2y = d[5] - d[1];      // M2P2
+    // [M2N2 M2P2] * [b1y -b1x; -a1y a1x]
+    const T h11 = a2x * b1y - b2x * a1y;
+    const T h12 = b2x * a1x - a2x * b1x;
+    const T h21 = a2y * b1y - b2y * a1y;
+    const T h22 = b2y * a1x - a2y * b1x;
+    // third column: f_A1 * M2 - L * M1
+    H[0] = h11; H[1] = h12; H[2] = fA1 * d[0] - h11 * s[0] - h12 * s[1];
+    H[3] = h21; H[4] = h22; H[5] = fA1 * d[1] - h21 * s[0] - h22 * s[1];
+    H[6] = T(0.0); H[7] = T(0.0); H[8] = fA1;
+}
+
+// ---------------------------------------------------------------------------
 // TensorACA for a rectangle: Algorithm 1, Eq. 42-45.
 // Roles (reading R6): M1 = upper-left vertex, N1, Q1, P1 follow
 // clockwise, i.e. M = TL, N = TR, Q = BR, P = BL; r_rec = w_rec / h_rec.

@@ -156,6 +156,46 @@ HG_API int hg_aca_rect_backward(const float* offsets, float x0, float y0, float 
                          const float* grad_H, float* grad_offsets, int64_t n, void* cuda_stream);
 
 /* --------------------------------------------------------------------------------------------
+ * hg_affine_batched -- 2D affine transformation from THREE correspondences by the ACA route
+ * (Sec. 5.2, Eq. 41 first row): H_A = H_A2^-1 * H_A1, the core transformation being the
+ * identity; 33 FLOPs, no division.  Returned as a 3x3 H "computed in the same way as projective
+ * transformations": h31 = h32 = 0 and, under HG_NORM_NONE, h33 = f_A1 (Eq. 24).
+ *   src3, dst3 : n sets of points M,N,P;  HG_SOA: float[6][n] planes x0,y0,x1,y1,x2,y2;
+ *                HG_AOS: float[n][3][2]                                  (read,  48 B per set)
+ *   H          : HG_SOA float[9][n] / HG_AOS float[n][3][3], per `norm`  (write, 36 B per set)
+ * Collinear source points give the singular H (h33 = 0).  Errors as hg_aca_batched.
+ * -------------------------------------------------------------------------------------------- */
+HG_API int hg_affine_batched(const float* src3, const float* dst3, float* H, int64_t n,
+                      hg_layout_t layout, hg_norm_t norm, hg_precision_t prec, void* cuda_stream);
+
+/* --------------------------------------------------------------------------------------------
+ * hg_sk_batched -- the simplified SK decomposition (Sec. 3.4 case ii, Eq. 17, Table 3 row "SK",
+ * P:303-318): homography from a known planar pattern (object plane) to each of n images,
+ * Hbar = H * H_S1^-1 = H_S2^-1 * H_K.  The pattern's coordinates are given in the frame of its two
+ * anchors, M -> (-1,0), N -> (+1,0) (H_S1 = I), so only P3, Q3 describe it; everything that depends
+ * on the pattern alone is computed once per call.  Hbar maps (-1,0), (1,0), P3, Q3 onto the image
+ * points M2, N2, P2, Q2.  Two reciprocals per image.
+ *   P3x..Q3y : the pattern's third and fourth point in the anchor frame (host doubles, by value)
+ *   dst      : n image quadruples M2,N2,P2,Q2 in `layout` (as hg_aca_batched's dst) (read, 32 B)
+ *   H        : Hbar in `layout`, per `norm`                                        (write, 36 B)
+ * P3.y == 0 or Q3.y == 0 (pattern point on the anchor line) or a zero determinant of Eq. 14 give
+ * non-finite output (reading R8).  Errors as hg_aca_batched, plus HG_ERR_INVALID_ARG for a NaN
+ * pattern coordinate.
+ * -------------------------------------------------------------------------------------------- */
+HG_API int hg_sk_batched(double P3x, double P3y, double Q3x, double Q3y, const float* dst, float* H,
+                  int64_t n, hg_layout_t layout, hg_norm_t norm, hg_precision_t prec,
+                  void* cuda_stream);
+
+/* hg_aca_batched_f64 / hg_sks_batched_f64 -- the two general solvers with fp64 STORAGE, the
+ * precision of the paper's own GPU experiment (Sec. 6.4).  Layouts as hg_layout_t with
+ * double in place of float (HG_SOA: double[8][n] -> double[9][n]); 128 B read + 72 B written per
+ * homography.  Arguments and errors otherwise as hg_aca_batched.                                */
+HG_API int hg_aca_batched_f64(const double* src, const double* dst, double* H, int64_t n,
+                       hg_layout_t layout, hg_norm_t norm, void* cuda_stream);
+HG_API int hg_sks_batched_f64(const double* src, const double* dst, double* H, int64_t n,
+                       hg_layout_t layout, hg_norm_t norm, void* cuda_stream);
+
+/* --------------------------------------------------------------------------------------------
  * hg_ransac_hypothesize_score -- RANSAC hypothesis generation fused with inlier scoring
  * (hypothesise-and-verify loop, Sec. 2.2; parallel hypotheses P:703).
  * For every hypothesis: gather its 4 correspondences, ACA solve (fp64 internal), then count

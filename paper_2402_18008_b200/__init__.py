@@ -20,6 +20,7 @@ __all__ = [
     "HgError", "lib", "lib_path", "SOA", "AOS", "NORM_NONE", "NORM_H33", "NORM_FROBENIUS",
     "PREC_F64", "PREC_F32", "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host",
     "hg_sks_batched_host", "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward",
+    "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
     "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_status_string",
     "hg_version", "hg_built_for_sm", "EXPORTS",
 ]
@@ -34,8 +35,8 @@ RANSAC_STAT_WORDS = 4
 # every symbol include/hg.h declares
 EXPORTS = [
     "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-    "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_ransac_workspace_bytes",
-    "hg_ransac_hypothesize_score",
+    "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_affine_batched", "hg_sk_batched",
+    "hg_aca_batched_f64", "hg_sks_batched_f64", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
     "hg_ransac_hypothesize_score_host", "hg_status_string", "hg_version", "hg_built_for_sm",
 ]
 
@@ -71,6 +72,11 @@ def lib() -> ctypes.CDLL:
                                          _c_i64, _c_int, _vp]
         L.hg_aca_rect_batched.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
         L.hg_aca_rect_backward.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _vp, _c_i64, _vp]
+        L.hg_affine_batched.argtypes = solve_args
+        _c_f64 = ctypes.c_double
+        L.hg_sk_batched.argtypes = [_c_f64, _c_f64, _c_f64, _c_f64, _vp, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
+        L.hg_aca_batched_f64.argtypes = [_vp, _vp, _vp, _c_i64, _c_int, _c_int, _vp]
+        L.hg_sks_batched_f64.argtypes = [_vp, _vp, _vp, _c_i64, _c_int, _c_int, _vp]
         L.hg_ransac_workspace_bytes.argtypes = [_c_i32, _c_i64]
         L.hg_ransac_workspace_bytes.restype = ctypes.c_size_t
         L.hg_ransac_hypothesize_score.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp,
@@ -79,7 +85,8 @@ def lib() -> ctypes.CDLL:
         L.hg_status_string.argtypes = [_c_int]
         L.hg_status_string.restype = ctypes.c_char_p
         for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-                     "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward",
+                     "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_affine_batched",
+                     "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
                      "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host",
                      "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
@@ -251,6 +258,75 @@ def hg_aca_rect_backward(offsets, x0: float, y0: float, w: float, h: float, grad
         st = lib().hg_aca_rect_backward(po, x0, y0, w, h, pg, pr, n, _stream(stream))
     _check(st, "hg_aca_rect_backward")
     return grad_offsets
+
+
+def _n_generic(t: torch.Tensor, layout: int, scalars: int, what: str) -> int:
+    if layout == SOA:
+        if t.dim() != 2 or t.shape[0] != scalars:
+            raise ValueError("SoA %s are [%d, n]" % (what, scalars))
+        return int(t.shape[1])
+    if t.dim() != 3 or tuple(t.shape[1:]) != (scalars // 2, 2):
+        raise ValueError("AoS %s are [n, %d, 2]" % (what, scalars // 2))
+    return int(t.shape[0])
+
+
+def hg_affine_batched(src3, dst3, H=None, layout: int = SOA, norm: int = NORM_NONE, prec: int = PREC_F64,
+                      stream=None) -> torch.Tensor:
+    """Affine H_A from three correspondences (Eq. 41).  SoA: [6,n] x2 -> [9,n]; AoS: [n,3,2] x2 -> [n,3,3]."""
+    n = _n_generic(src3, layout, 6, "3-point sets")
+    if tuple(dst3.shape) != tuple(src3.shape):
+        raise ValueError("src3 and dst3 shapes differ")
+    if H is None:
+        H = torch.empty(_h_shape(n, layout), dtype=torch.float32, device=src3.device)
+    elif tuple(H.shape) != _h_shape(n, layout):
+        raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
+    ps, pd, ph = (_ptr(src3, torch.float32, "cuda", "src3"), _ptr(dst3, torch.float32, "cuda", "dst3"),
+                  _ptr(H, torch.float32, "cuda", "H"))
+    with torch.cuda.device(src3.device):
+        st = lib().hg_affine_batched(ps, pd, ph, n, int(layout), int(norm), int(prec), _stream(stream))
+    _check(st, "hg_affine_batched")
+    return H
+
+
+def hg_sk_batched(P3, Q3, dst, H=None, layout: int = SOA, norm: int = NORM_NONE, prec: int = PREC_F64,
+                  stream=None) -> torch.Tensor:
+    """Simplified SK (Eq. 17): pattern points P3, Q3 = (x, y) in the anchor frame; dst as hg_aca_batched's dst."""
+    n = _n_sets(dst, layout)
+    if H is None:
+        H = torch.empty(_h_shape(n, layout), dtype=torch.float32, device=dst.device)
+    elif tuple(H.shape) != _h_shape(n, layout):
+        raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
+    pd, ph = _ptr(dst, torch.float32, "cuda", "dst"), _ptr(H, torch.float32, "cuda", "H")
+    with torch.cuda.device(dst.device):
+        st = lib().hg_sk_batched(float(P3[0]), float(P3[1]), float(Q3[0]), float(Q3[1]), pd, ph, n, int(layout),
+                                 int(norm), int(prec), _stream(stream))
+    _check(st, "hg_sk_batched")
+    return H
+
+
+def _solve_f64(fn_name: str, src, dst, H, layout, norm, stream):
+    n = _n_sets(src, layout)
+    if tuple(dst.shape) != tuple(src.shape):
+        raise ValueError("src and dst shapes differ")
+    if H is None:
+        H = torch.empty(_h_shape(n, layout), dtype=torch.float64, device=src.device)
+    elif tuple(H.shape) != _h_shape(n, layout):
+        raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
+    ps, pd, ph = (_ptr(src, torch.float64, "cuda", "src"), _ptr(dst, torch.float64, "cuda", "dst"),
+                  _ptr(H, torch.float64, "cuda", "H"))
+    with torch.cuda.device(src.device):
+        st = getattr(lib(), fn_name)(ps, pd, ph, n, int(layout), int(norm), _stream(stream))
+    _check(st, fn_name)
+    return H
+
+
+def hg_aca_batched_f64(src, dst, H=None, layout: int = SOA, norm: int = NORM_NONE, stream=None) -> torch.Tensor:
+    """ACA with float64 storage (the paper's GPU precision)."""
+    return _solve_f64("hg_aca_batched_f64", src, dst, H, layout, norm, stream)
+
+
+def hg_sks_batched_f64(src, dst, H=None, layout: int = SOA, norm: int = NORM_NONE, stream=None) -> torch.Tensor:
+    return _solve_f64("hg_sks_batched_f64", src, dst, H, layout, norm, stream)
 
 
 def hg_ransac_workspace_bytes(n_pts: int, n_hyp: int) -> int:

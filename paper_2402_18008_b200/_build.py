@@ -9,7 +9,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libhg.so"
-SOURCES = ["hg_api.cu", "hg_batched.cu", "hg_grid.cu", "hg_ransac.cu", "hg_rect.cu"]
+SOURCES = ["hg_api.cu", "hg_batched.cu", "hg_grid.cu", "hg_ransac.cu", "hg_rect.cu", "hg_variants.cu"]
 HEADERS = [CSRC / "hg_device.cuh", CSRC / "hg_host.h", PKG.parent / "include" / "hg.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-Xptxas", "-v"]

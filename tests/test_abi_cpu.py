@@ -112,6 +112,28 @@ def test_rect_backward_argument_validation():
     assert f(FAKE, 0.0, 0.0, 127.0, 127.0, FAKE, FAKE + 8, 4, None) == -2
 
 
+def test_variant_argument_validation():
+    L = hg.lib()
+    f = L.hg_affine_batched
+    assert f(FAKE, FAKE, FAKE, 0, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == 0
+    assert f(FAKE, FAKE, FAKE, -1, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -1
+    assert f(None, FAKE, FAKE, 4, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -1
+    assert f(FAKE, FAKE, FAKE, 4, 5, hg.NORM_NONE, hg.PREC_F64, None) == -1
+    assert f(FAKE, FAKE, FAKE, 4, hg.SOA, 7, hg.PREC_F64, None) == -1
+    assert f(FAKE, FAKE, FAKE, 4, hg.SOA, hg.NORM_NONE, 9, None) == -1
+    assert f(FAKE + 8, FAKE, FAKE, 4, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -2
+    g = L.hg_sk_batched
+    assert g(0.3, 1.5, -0.5, -1.0, FAKE, FAKE, 0, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == 0
+    assert g(float("nan"), 1.5, -0.5, -1.0, FAKE, FAKE, 4, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -1
+    assert g(0.3, 1.5, -0.5, -1.0, None, FAKE, 4, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -1
+    assert g(0.3, 1.5, -0.5, -1.0, FAKE, FAKE + 4, 4, hg.SOA, hg.NORM_NONE, hg.PREC_F64, None) == -2
+    for h in (L.hg_aca_batched_f64, L.hg_sks_batched_f64):
+        assert h(FAKE, FAKE, FAKE, 0, hg.SOA, hg.NORM_NONE, None) == 0
+        assert h(FAKE, FAKE, None, 4, hg.SOA, hg.NORM_NONE, None) == -1
+        assert h(FAKE, FAKE, FAKE, 4, 3, hg.NORM_NONE, None) == -1
+        assert h(FAKE, FAKE + 8, FAKE, 4, hg.SOA, hg.NORM_NONE, None) == -2
+
+
 def test_ransac_argument_validation_and_workspace():
     L = hg.lib()
     ws = L.hg_ransac_workspace_bytes

@@ -100,3 +100,73 @@ def test_rect_backward_is_the_gradient_of_the_forward_entry_point():
     lhs = ((Hp - Hm) * g.double()).sum(dim=(1, 2)) / 2.0
     rhs = (go * d.double()).sum(dim=(1, 2))
     assert ((lhs - rhs).abs() <= 2e-3 * rhs.abs() + 1e-5 * go.abs().amax(dim=(1, 2)) * 2.0 ** -5 * 8).all()
+
+
+# ---- 8(f)-3: hg_affine_batched (Eq. 41) -------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 1023, 4096, 50001])
+@pytest.mark.parametrize("layout", ["aos", "soa"])
+def test_affine_matches_oracle(n, layout):
+    s, d = W.general_sets(n, seed=W.SEED_BASE + 40 + n)
+    s3, d3 = s[:, :3].contiguous(), d[:, :3].contiguous()
+    H_ref = oracle.affine(s3.numpy(), d3.numpy())
+    if layout == "aos":
+        H = hg.hg_affine_batched(s3.to(DEV), d3.to(DEV), layout=hg.AOS, norm=hg.NORM_H33).cpu().numpy()
+    else:
+        a, b = s3.reshape(n, 6).t().contiguous(), d3.reshape(n, 6).t().contiguous()
+        H = hg.hg_affine_batched(a.to(DEV), b.to(DEV), layout=hg.SOA, norm=hg.NORM_H33).t().reshape(n, 3, 3).cpu().numpy()
+    assert np.all(H[:, 2, 0] == 0.0) and np.all(H[:, 2, 1] == 0.0) and np.all(H[:, 2, 2] == 1.0)
+    A_ref = H_ref / H_ref[:, 2:3, 2:3]
+    # fp64 internal, one rounding to fp32: each entry within fp32 rounding of its own magnitude (+ the translation's scale)
+    tol = 1.5e-7 * np.abs(A_ref) + 1e-7
+    assert (np.abs(H - A_ref) <= tol).all()
+    assert np.abs(project(H.astype(np.float64), s3.numpy()) - d3.numpy()).max() <= 1e-3
+    raw = hg.hg_affine_batched(s3.to(DEV), d3.to(DEV), layout=hg.AOS, norm=hg.NORM_NONE).cpu().numpy()
+    assert (np.abs(raw - H_ref) <= 1.5e-7 * np.abs(H_ref) + 1e-30).all()                 # raw scale: h33 = f_A1
+
+
+# ---- 8(f)-4: hg_sk_batched (Eq. 17) -----------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 777, 8192])
+@pytest.mark.parametrize("layout", ["aos", "soa"])
+def test_sk_matches_oracle(n, layout):
+    s, d = W.general_sets(n, seed=W.SEED_BASE + 50 + n)
+    P3, Q3 = (0.35, 1.6), (-0.8, -1.1)                      # a fixed pattern in its anchor frame
+    H_ref = oracle.sk(P3, Q3, d.numpy())
+    if layout == "aos":
+        H = hg.hg_sk_batched(P3, Q3, d.to(DEV), layout=hg.AOS, norm=hg.NORM_FROBENIUS).cpu().numpy()
+    else:
+        H = hg.hg_sk_batched(P3, Q3, W.to_soa(d).to(DEV), layout=hg.SOA, norm=hg.NORM_FROBENIUS)
+        H = H.t().reshape(n, 3, 3).cpu().numpy()
+    a, b = align_to(H.astype(np.float64), H_ref)
+    assert (np.abs(a - b) <= 1e-4 * np.abs(b) + 1e-7).all()
+    assert np.abs(a - b).max() <= 3e-7
+    obj = np.broadcast_to(np.array([[-1.0, 0.0], [1.0, 0.0], P3, Q3]), (n, 4, 2))
+    ok = np.isfinite(H_ref).all(axis=(1, 2))
+    assert ok.all()
+    # reprojection on the sets whose own fp32-rounding sensitivity is small (reading R12)
+    from util import rounding_sensitivity
+    good = rounding_sensitivity(H_ref, obj) <= 1e-3
+    assert n < 100 or good.mean() >= 0.7        # an arbitrary pattern against random quadrangles is strongly projective (77 %)
+    if good.any():
+        assert np.abs(project(H.astype(np.float64), obj) - d.numpy().astype(np.float64))[good].max() <= 1e-3
+
+
+# ---- 8(f)-3: fp64 storage --------------------------------------------------------------------
+@pytest.mark.parametrize("method", ["aca", "sks"])
+@pytest.mark.parametrize("n,layout", [(4096, "soa"), (4097, "soa"), (1000, "aos"), (1, "aos")])
+def test_f64_storage_matches_oracle(method, n, layout):
+    s, d = W.general_sets(n, seed=W.SEED_BASE + 60 + n)
+    s64, d64 = s.double(), d.double()
+    fn = hg.hg_aca_batched_f64 if method == "aca" else hg.hg_sks_batched_f64
+    if layout == "soa":
+        H = fn(W.to_soa(s64).to(DEV), W.to_soa(d64).to(DEV), layout=hg.SOA, norm=hg.NORM_FROBENIUS).t().reshape(n, 3, 3)
+    else:
+        H = fn(s64.to(DEV), d64.to(DEV), layout=hg.AOS, norm=hg.NORM_FROBENIUS)
+    H = H.cpu().numpy()
+    H_ref = oracle.solve_f64(oracle.METHOD_ACA if method == "aca" else oracle.METHOD_SKS, s64.numpy(), d64.numpy())
+    a, b = align_to(H, H_ref)
+    # both sides fp64; they differ by FMA contraction and the reciprocal's last ulp, amplified by conditioning
+    assert np.abs(a - b).max() <= (1e-11 if method == "aca" else 1e-9)
+    assert np.abs(project(H, s.numpy()) - d.numpy().astype(np.float64)).max() <= 1e-7
+    Hd = oracle.solve_f64(oracle.METHOD_DLT, s64.numpy(), d64.numpy())
+    a, b = align_to(H, Hd)
+    assert np.abs(a - b).max() <= 1e-9

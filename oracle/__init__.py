@@ -184,6 +184,19 @@ def offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w: i
     return H, grid
 
 
+def offsets_to_warp(offsets, x0: float, y0: float, w: float, h: float, out_w: int, out_h: int, image) -> np.ndarray:
+    """image float32 [n,C,img_h,img_w] sampled bilinearly (zero padding, pixel units) at the grid of H: float64 [n,C,out_h,out_w]."""
+    o = _f32(offsets, (4, 2))
+    img = np.ascontiguousarray(np.asarray(image), dtype=np.float32)
+    n, C, ih, iw = img.shape
+    assert n == o.shape[0]
+    out = np.empty((n, C, out_h, out_w), dtype=np.float64)
+    lib().hgo_offsets_to_warp(_p(o), ctypes.c_float(x0), ctypes.c_float(y0), ctypes.c_float(w), ctypes.c_float(h),
+                              ctypes.c_int32(out_w), ctypes.c_int32(out_h), _p(img), ctypes.c_int32(C),
+                              ctypes.c_int32(iw), ctypes.c_int32(ih), _p(out), ctypes.c_int64(n))
+    return out
+
+
 def ransac(src_xy, dst_xy, hyp_idx, threshold: float, band_rel: float = 1e-4, solver: int = METHOD_ACA):
     """Returns dict(counts int32 [n_hyp], band_counts, best_H [3,3] normal form, best_index, best_count)."""
     s = _f32(src_xy, (2,)); d = _f32(dst_xy, (2,))

@@ -226,6 +226,55 @@ void hgo_offsets_to_grid(const float* offsets, float x0, float y0, float w, floa
     }
 }
 
+// Offsets -> H -> warped image ("warp image with H"; reading R17):
+//   warped[b][c][j][i] = bilinear(image[b][c], pi(H_b * (x_i, y_j, 1)))
+// with the lattice (x_i, y_j) of hgo_offsets_to_grid.  The image is sampled in pixel units (pixel (col u,
+// row v) has centre (u, v)); u0 = floor(u), fu = u - u0, the four taps (u0,v0), (u0+1,v0), (u0,v0+1),
+// (u0+1,v0+1) carry weights (1-fu)(1-fv), fu(1-fv), (1-fu)fv, fu fv, and a tap outside the image
+// contributes zero (zero padding).  A non-finite sampling position gives 0.
+//   image  float  [n][channels][img_h][img_w];   warped double [n][channels][out_h][out_w]
+void hgo_offsets_to_warp(const float* offsets, float x0, float y0, float w, float h,
+                         int32_t out_w, int32_t out_h, const float* image, int32_t channels,
+                         int32_t img_w, int32_t img_h, double* warped, int64_t n)
+{
+    const double X0 = x0, Y0 = y0, Wd = w, Hd = h;
+    const double s[8] = { X0, Y0, X0 + Wd, Y0, X0 + Wd, Y0 + Hd, X0, Y0 + Hd };
+#pragma omp parallel for schedule(static)
+    for (int64_t b = 0; b < n; ++b) {
+        double d[8], H[9];
+        for (int k = 0; k < 8; ++k) d[k] = s[k] + static_cast<double>(offsets[8 * b + k]);
+        hgo::aca<double>(s, d, H);
+        for (int32_t j = 0; j < out_h; ++j) {
+            const double y = (out_h > 1) ? Y0 + j * Hd / (out_h - 1) : Y0;
+            for (int32_t i = 0; i < out_w; ++i) {
+                const double x = (out_w > 1) ? X0 + i * Wd / (out_w - 1) : X0;
+                const double X = H[0] * x + H[1] * y + H[2];
+                const double Y = H[3] * x + H[4] * y + H[5];
+                const double W = H[6] * x + H[7] * y + H[8];
+                const double u = X / W, v = Y / W;
+                const bool finite = std::isfinite(u) && std::isfinite(v);
+                const double u0 = std::floor(u), v0 = std::floor(v);
+                const double fu = u - u0, fv = v - v0;
+                for (int32_t c = 0; c < channels; ++c) {
+                    const float* img = image + (static_cast<int64_t>(b) * channels + c) * img_h * img_w;
+                    double acc = 0.0;
+                    if (finite && u0 >= -1.0 && u0 <= img_w && v0 >= -1.0 && v0 <= img_h) {
+                        const int64_t iu = static_cast<int64_t>(u0), iv = static_cast<int64_t>(v0);
+                        for (int dv = 0; dv < 2; ++dv)
+                            for (int du = 0; du < 2; ++du) {
+                                const int64_t tu = iu + du, tv = iv + dv;
+                                if (tu < 0 || tu >= img_w || tv < 0 || tv >= img_h) continue;
+                                const double wt = (du ? fu : 1.0 - fu) * (dv ? fv : 1.0 - fv);
+                                acc += wt * static_cast<double>(img[tv * img_w + tu]);
+                            }
+                    }
+                    warped[((static_cast<int64_t>(b) * channels + c) * out_h + j) * out_w + i] = acc;
+                }
+            }
+        }
+    }
+}
+
 // RANSAC hypothesise-and-score (reading R9).
 //   src_xy, dst_xy : float [n_pts][2];  hyp_idx : int32 [n_hyp][4]
 //   solver: 1 = ACA-fp64 (the parity reference), 0 = DLT-GE (cross-check)

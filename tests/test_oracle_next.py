@@ -156,3 +156,36 @@ def test_sk_defining_property_and_relation_to_complete_sks():
     c = oracle.op_counts(5)
     # Table 3 prints 73 for the simplified SK; the formulas as printed take 75 with two reciprocals (reading R15)
     assert c["div"] == 2 and c["flops"] == 75
+
+
+# ---- offsets -> H -> bilinear warp (reading R17) --------------------------------------------
+def test_warp_equals_library_grid_sample():
+    """torch.nn.functional.grid_sample (float64, bilinear, zeros, align_corners=True) on the oracle's own grid."""
+    import torch
+    n, C, ih, iw, ow, oh = 6, 2, 40, 56, 33, 21
+    rect = (3.0, 2.0, 45.0, 30.0)
+    off = W.offsets_workload(n, seed=91, max_offset=9.0).numpy()
+    rng = np.random.default_rng(91)
+    img = rng.random((n, C, ih, iw)).astype(np.float32)
+    out = oracle.offsets_to_warp(off, *rect, ow, oh, img)
+    _, grid = oracle.offsets_to_grid(off, *rect, ow, oh)
+    gn = np.empty_like(grid)
+    gn[..., 0] = 2.0 * grid[..., 0] / (iw - 1) - 1.0            # align_corners=True: pixel centre k <-> -1 + 2k/(size-1)
+    gn[..., 1] = 2.0 * grid[..., 1] / (ih - 1) - 1.0
+    ref = torch.nn.functional.grid_sample(torch.from_numpy(img).double(), torch.from_numpy(gn), mode="bilinear",
+                                          padding_mode="zeros", align_corners=True).numpy()
+    assert np.abs(out - ref).max() <= 1e-10
+    assert (out[:, :, 0, 0] != 0).any()
+
+
+def test_warp_identity_and_integer_translation_are_exact():
+    rng = np.random.default_rng(92)
+    img = rng.random((2, 1, 32, 32)).astype(np.float32)
+    zero = np.zeros((2, 4, 2), dtype=np.float32)
+    out = oracle.offsets_to_warp(zero, 0.0, 0.0, 31.0, 31.0, 32, 32, img)
+    assert np.abs(out - img).max() <= 1e-12                      # H = I on the pixel lattice (up to fp64 rounding of X/W)
+    sh = np.zeros((2, 4, 2), dtype=np.float32); sh[..., 0] = 3.0; sh[..., 1] = -2.0     # targets = corners + (3,-2)
+    out = oracle.offsets_to_warp(sh, 0.0, 0.0, 31.0, 31.0, 32, 32, img)
+    exp = np.zeros_like(out)
+    exp[:, :, 2:, :29] = img[:, :, :30, 3:]                       # out(x, y) = img(x + 3, y - 2), zero outside
+    assert np.abs(out - exp).max() <= 1e-10

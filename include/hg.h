@@ -125,6 +125,26 @@ HG_API int hg_offsets_to_grid(const float* offsets, float x0, float y0, float w,
                        hg_norm_t norm, void* cuda_stream);
 
 /* --------------------------------------------------------------------------------------------
+ * hg_offsets_to_warp -- offsets -> H -> warped image in one kernel ("warp image with H"): as
+ * hg_offsets_to_grid, but instead of writing the sampling grid the kernel samples `image` at it
+ * (reading R17):  warped[b][c][j][i] = bilinear(image[b][c], pi(H_b * (x_i, y_j, 1))),
+ * image coordinates in pixel units (pixel (col u, row v) has centre (u, v)), the four taps around
+ * (floor(u), floor(v)), a tap outside the image contributes zero, a non-finite position gives 0.
+ *   offsets, x0, y0, w, h : as hg_offsets_to_grid; out_w, out_h play the role of grid_w, grid_h
+ *   image   : float[n][channels][img_h][img_w]                       (read,  4 B per tap, L1-cached)
+ *   warped  : float[n][channels][out_h][out_w]                       (write, 4 B per pixel and channel)
+ *   H       : nullable, float[n][3][3] per `norm`
+ * Errors: HG_ERR_INVALID_ARG (NULL with n > 0, sizes < 1, w == 0 or h == 0, bad enum),
+ * HG_ERR_ALIGNMENT (offsets not 16-byte aligned; image, warped, H not 4-byte aligned), HG_ERR_CUDA.
+ * When the item's image (all channels) is at most 110 KB and 16-byte aligned it is staged in shared memory
+ * by one bulk-async copy per CTA; larger images are gathered through L1.
+ * -------------------------------------------------------------------------------------------- */
+HG_API int hg_offsets_to_warp(const float* offsets, float x0, float y0, float w, float h,
+                       int32_t out_w, int32_t out_h, const float* image, int32_t channels,
+                       int32_t img_w, int32_t img_h, float* warped, float* H, int64_t n,
+                       hg_norm_t norm, void* cuda_stream);
+
+/* --------------------------------------------------------------------------------------------
  * hg_aca_rect_batched -- TensorACA for a rectangular source (Sec. 5.3, Eq. 42-45, Algorithm 1,
  * P:540-591): the source quadrangle is the fixed rectangle TL = (x0,y0), extents (w,h), shared by
  * the whole batch, so H_A1 is trivial, Q3 = (1,1,1) and H follows from the target corners alone

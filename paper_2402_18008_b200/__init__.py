@@ -19,7 +19,7 @@ from . import _build
 __all__ = [
     "HgError", "lib", "lib_path", "SOA", "AOS", "NORM_NONE", "NORM_H33", "NORM_FROBENIUS",
     "PREC_F64", "PREC_F32", "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host",
-    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward",
+    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
     "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
     "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_status_string",
     "hg_version", "hg_built_for_sm", "EXPORTS",
@@ -35,8 +35,8 @@ RANSAC_STAT_WORDS = 4
 # every symbol include/hg.h declares
 EXPORTS = [
     "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-    "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_affine_batched", "hg_sk_batched",
-    "hg_aca_batched_f64", "hg_sks_batched_f64", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
+    "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_affine_batched",
+    "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
     "hg_ransac_hypothesize_score_host", "hg_status_string", "hg_version", "hg_built_for_sm",
 ]
 
@@ -72,6 +72,8 @@ def lib() -> ctypes.CDLL:
                                          _c_i64, _c_int, _vp]
         L.hg_aca_rect_batched.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
         L.hg_aca_rect_backward.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _vp, _c_i64, _vp]
+        L.hg_offsets_to_warp.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _c_i32, _c_i32, _vp, _c_i32, _c_i32, _c_i32,
+                                         _vp, _vp, _c_i64, _c_int, _vp]
         L.hg_affine_batched.argtypes = solve_args
         _c_f64 = ctypes.c_double
         L.hg_sk_batched.argtypes = [_c_f64, _c_f64, _c_f64, _c_f64, _vp, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
@@ -85,8 +87,8 @@ def lib() -> ctypes.CDLL:
         L.hg_status_string.argtypes = [_c_int]
         L.hg_status_string.restype = ctypes.c_char_p
         for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-                     "hg_offsets_to_grid", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_affine_batched",
-                     "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
+                     "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
+                     "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
                      "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host",
                      "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
@@ -225,6 +227,29 @@ def hg_offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w
                                       _ptr(grid, torch.float32, "cuda", "grid"), n, int(norm), _stream(stream))
     _check(st, "hg_offsets_to_grid")
     return H, grid
+
+
+def hg_offsets_to_warp(offsets, x0: float, y0: float, w: float, h: float, out_w: int, out_h: int, image,
+                       warped=None, want_H: bool = False, norm: int = NORM_H33, stream=None):
+    """offsets [n,4,2] + image [n,C,img_h,img_w] -> (warped [n,C,out_h,out_w], H [n,3,3] or None)."""
+    if offsets.dim() != 3 or tuple(offsets.shape[1:]) != (4, 2):
+        raise ValueError("offsets are float32 [n, 4, 2]")
+    n = int(offsets.shape[0])
+    if image.dim() != 4 or image.shape[0] != n:
+        raise ValueError("image is float32 [n, C, img_h, img_w]")
+    C, ih, iw = int(image.shape[1]), int(image.shape[2]), int(image.shape[3])
+    if warped is None:
+        warped = torch.empty((n, C, out_h, out_w), dtype=torch.float32, device=offsets.device)
+    elif tuple(warped.shape) != (n, C, out_h, out_w):
+        raise ValueError("warped must be [n,C,out_h,out_w]")
+    H = torch.empty((n, 3, 3), dtype=torch.float32, device=offsets.device) if want_H else None
+    with torch.cuda.device(offsets.device):
+        st = lib().hg_offsets_to_warp(_ptr(offsets, torch.float32, "cuda", "offsets"), x0, y0, w, h, int(out_w), int(out_h),
+                                      _ptr(image, torch.float32, "cuda", "image"), C, iw, ih,
+                                      _ptr(warped, torch.float32, "cuda", "warped"), _ptr(H, torch.float32, "cuda", "H"),
+                                      n, int(norm), _stream(stream))
+    _check(st, "hg_offsets_to_warp")
+    return warped, H
 
 
 def hg_aca_rect_batched(offsets, x0: float, y0: float, w: float, h: float, H=None, layout: int = AOS,

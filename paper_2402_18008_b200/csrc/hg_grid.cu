@@ -12,6 +12,7 @@
 namespace hg {
 
 constexpr int kGridBlock = 256;
+constexpr size_t kWarpStageBytes = 110 * 1024;   // staged image per CTA: two CTAs per SM
 
 struct RectParams {
     double x0, y0, w, h;      // source rectangle
@@ -131,6 +132,185 @@ offsets_to_h_kernel(const float* __restrict__ offsets, RectParams rp, float* __r
     for (int j = threadIdx.x; j < cnt; j += kGridBlock) out[j] = stage[j];
 }
 
+// ------------------------------------------------------------------------------------------
+// Offsets -> H -> warped image ("warp image with H"; reading R17): the
+// sampling grid never reaches HBM.  Lanes map to adjacent pixels of a row, so the four bilinear taps
+// of a warp fall into one or two lines each and every store instruction writes a full line.
+// Zero padding: a tap outside the image contributes 0; a non-finite position gives 0.
+// blockIdx.x = item, blockIdx.y = band of rows.  Per pixel and channel: 4 B read + 4 B written.
+// ------------------------------------------------------------------------------------------
+struct WarpGeom { int out_w, out_h, img_w, img_h, channels, rows_per_band; };
+
+// The four taps of one sampling position: element offsets into an image plane (always inside the plane)
+// and weights (zero for a tap that lies outside the image).  Branch-free: the position is first clamped to
+// [-1, size], where every tap is either valid or carries weight zero -- this also sends NaN to -1.
+struct Taps { int o00, o01, o10, o11; float w00, w01, w10, w11; };
+
+__device__ __forceinline__ Taps make_taps(float u, float v, int img_w, int img_h)
+{
+    const float uc = fminf(fmaxf(u, -1.f), static_cast<float>(img_w));
+    const float vc = fminf(fmaxf(v, -1.f), static_cast<float>(img_h));
+    const float u0 = floorf(uc), v0 = floorf(vc);
+    const float fu = uc - u0, fv = vc - v0;                                   // exact
+    const int iu = static_cast<int>(u0), iv = static_cast<int>(v0);           // [-1, img_w], [-1, img_h]
+    const float wx0 = (static_cast<unsigned>(iu) < static_cast<unsigned>(img_w)) ? 1.f - fu : 0.f;
+    const float wx1 = (static_cast<unsigned>(iu + 1) < static_cast<unsigned>(img_w)) ? fu : 0.f;
+    const float wy0 = (static_cast<unsigned>(iv) < static_cast<unsigned>(img_h)) ? 1.f - fv : 0.f;
+    const float wy1 = (static_cast<unsigned>(iv + 1) < static_cast<unsigned>(img_h)) ? fv : 0.f;
+    const int cx0 = min(max(iu, 0), img_w - 1), cx1 = min(iu + 1, img_w - 1);
+    const int r0 = min(max(iv, 0), img_h - 1) * img_w, r1 = min(iv + 1, img_h - 1) * img_w;
+    Taps t;
+    t.o00 = r0 + cx0; t.o01 = r0 + cx1; t.o10 = r1 + cx0; t.o11 = r1 + cx1;
+    t.w00 = wy0 * wx0; t.w01 = wy0 * wx1; t.w10 = wy1 * wx0; t.w11 = wy1 * wx1;
+    return t;
+}
+
+// SMEM: the image plane was staged in shared memory (plain loads); otherwise global memory, read-only path.
+template <bool SMEM> __device__ __forceinline__ float px(const float* p) { return SMEM ? *p : __ldg(p); }
+
+template <bool SMEM>
+__device__ __forceinline__ float gather(const float* __restrict__ img, const Taps& t)
+{
+    return fmaf(t.w11, px<SMEM>(img + t.o11), fmaf(t.w10, px<SMEM>(img + t.o10),
+           fmaf(t.w01, px<SMEM>(img + t.o01), t.w00 * px<SMEM>(img + t.o00))));
+}
+
+// All four taps inside the image: p points at tap (0,0) of the plane.
+template <bool SMEM>
+__device__ __forceinline__ float gather_interior(const float* __restrict__ p, int img_w, float fu, float fv)
+{
+    const float a = px<SMEM>(p), b = px<SMEM>(p + 1), c = px<SMEM>(p + img_w), d = px<SMEM>(p + img_w + 1);
+    const float gu = 1.f - fu, gv = 1.f - fv;
+    return fmaf(fv * fu, d, fmaf(fv * gu, c, fmaf(gv * fu, b, (gv * gu) * a)));   // same weighted sum as gather()
+}
+
+__device__ __forceinline__ float rcp_approx(float x)
+{ float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+// CH = compile-time channel count (0: read it from the geometry).  SMEM: the item's image (all channels) is
+// staged in shared memory by bulk-async copies issued before the solve, so the HBM read is one deep transfer
+// per CTA instead of latency-bound gathers; used when the image fits (the host decides).
+template <int CH, bool SMEM>
+__global__ void __launch_bounds__(kGridBlock, SMEM ? 3 : 4)
+offsets_to_warp_kernel(const float* __restrict__ offsets, RectParams rp, WarpGeom g, int tx_count,
+                       const float* __restrict__ image, float* __restrict__ warped, float* __restrict__ H_out, int norm)
+{
+    __shared__ float hs[9];
+    __shared__ uint64_t img_bar;
+    extern __shared__ __align__(128) float img_s[];
+    const int64_t b = blockIdx.x;
+    if (SMEM) {
+        if (threadIdx.x == 0) { mbar_init(&img_bar, 1); fence_barrier_init(); }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const uint32_t bytes = static_cast<uint32_t>(g.channels) * g.img_w * g.img_h * 4u;
+            const char* src = reinterpret_cast<const char*>(image) + b * static_cast<int64_t>(bytes);
+            mbar_arrive_expect_tx(&img_bar, bytes);
+            for (uint32_t off = 0; off < bytes; off += 32768u)
+                bulk_copy_g2s(reinterpret_cast<char*>(img_s) + off, src + off, min(32768u, bytes - off), &img_bar);
+        }
+    }
+    if (threadIdx.x < 32) {
+        const float4* op = reinterpret_cast<const float4*>(offsets + 8 * b);
+        const float4 o0 = __ldg(op), o1 = __ldg(op + 1);
+        double s[8], d[8], Hd[9];
+        corners_from_offsets(rp, o0, o1, s, d);
+        aca_solve<double>(s, d, Hd);
+        double m = 0.0;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) m = fmax(m, fabs(Hd[k]));
+        const double r = K<double>::rcp(m);
+        if (H_out != nullptr && blockIdx.y == 0) {
+            double Hn[9];
+#pragma unroll
+            for (int k = 0; k < 9; ++k) Hn[k] = Hd[k] * r;
+            normalise<double>(Hn, norm);
+            if (norm == 0) {
+#pragma unroll
+                for (int k = 0; k < 9; ++k) Hn[k] = Hd[k];
+            }
+            if (threadIdx.x == 0) {
+#pragma unroll
+                for (int k = 0; k < 9; ++k) H_out[9 * b + k] = static_cast<float>(Hn[k]);
+            }
+        }
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int row = 0; row < 3; ++row) {
+                const double a = Hd[3 * row] * r, bb = Hd[3 * row + 1] * r, c = Hd[3 * row + 2] * r;
+                hs[3 * row]     = static_cast<float>(a * rp.step_x);
+                hs[3 * row + 1] = static_cast<float>(bb * rp.step_y);
+                hs[3 * row + 2] = static_cast<float>(fma(a, rp.x0, fma(bb, rp.y0, c)));
+            }
+        }
+    }
+    __syncthreads();
+    const float l11 = hs[0], l12 = hs[1], l13 = hs[2];
+    const float l21 = hs[3], l22 = hs[4], l23 = hs[5];
+    const float l31 = hs[6], l32 = hs[7], l33 = hs[8];
+
+    const int tx = threadIdx.x & (tx_count - 1);
+    const int ty = threadIdx.x / tx_count;
+    const int rows_per_pass = kGridBlock / tx_count;
+    const int channels = CH > 0 ? CH : g.channels;
+    const int img_w = g.img_w, img_h = g.img_h, out_w = g.out_w;
+    const int img_plane = img_w * img_h;
+    const int out_plane = out_w * g.out_h;
+    const float wm1 = static_cast<float>(img_w - 1), hm1 = static_cast<float>(img_h - 1);
+    const float* img_b = SMEM ? img_s : image + b * channels * static_cast<int64_t>(img_plane);
+    float* out_b = warped + b * channels * static_cast<int64_t>(out_plane);
+    const int j_begin = blockIdx.y * g.rows_per_band;
+    const int j_end = min(g.out_h, j_begin + g.rows_per_band);
+    if (SMEM) mbar_wait(&img_bar, 0);
+
+    for (int i = tx; i < out_w; i += tx_count) {
+        const float fi = static_cast<float>(i);
+        const float cx = fmaf(l11, fi, l13), cy = fmaf(l21, fi, l23), cw = fmaf(l31, fi, l33);
+        float* out_col = out_b + i;
+#pragma unroll 2
+        for (int j = j_begin + ty; j < j_end; j += rows_per_pass) {
+            const float fj = static_cast<float>(j);
+            const float X = fmaf(l12, fj, cx), Y = fmaf(l22, fj, cy), Wv = fmaf(l32, fj, cw);
+            const float q = rcp_approx(Wv);
+            const float u = X * q, v = Y * q;
+            float* op = out_col + j * out_w;
+            // Interior fast path, decided per warp: all four taps of every lane inside the image -- no clamping,
+            // no weight selection, one address.  NaN fails the comparisons and takes the general path.
+            const bool interior = (u >= 0.f) && (u < wm1) && (v >= 0.f) && (v < hm1);
+            if (__all_sync(0xffffffffu, interior)) {
+                const float u0 = floorf(u), v0 = floorf(v);
+                const float fu = u - u0, fv = v - v0;
+                const float* p = img_b + (static_cast<int>(v0) * img_w + static_cast<int>(u0));
+                if (CH > 0) {
+#pragma unroll
+                    for (int c = 0; c < CH; ++c) { __stcs(op, gather_interior<SMEM>(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
+                } else {
+                    for (int c = 0; c < channels; ++c) { __stcs(op, gather_interior<SMEM>(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
+                }
+            } else {
+                const Taps t = make_taps(u, v, img_w, img_h);
+                const float* ip = img_b;
+                if (CH > 0) {
+#pragma unroll
+                    for (int c = 0; c < CH; ++c) { __stcs(op, gather<SMEM>(ip, t)); ip += img_plane; op += out_plane; }
+                } else {
+                    for (int c = 0; c < channels; ++c) { __stcs(op, gather<SMEM>(ip, t)); ip += img_plane; op += out_plane; }
+                }
+            }
+        }
+    }
+}
+
+template <int CH, bool SMEM>
+static int launch_warp(dim3 grid, size_t smem, cudaStream_t st, const float* offsets, const RectParams& rp, const WarpGeom& g,
+                       int tx_count, const float* image, float* warped, float* H, int norm)
+{
+    if (SMEM && cudaFuncSetAttribute(offsets_to_warp_kernel<CH, SMEM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     int(kWarpStageBytes)) != cudaSuccess) return HG_ERR_CUDA;
+    offsets_to_warp_kernel<CH, SMEM><<<grid, kGridBlock, smem, st>>>(offsets, rp, g, tx_count, image, warped, H, norm);
+    return launch_status();
+}
+
 static int pow2_at_least(int v) { int p = 1; while (p < v) p <<= 1; return p; }
 
 }  // namespace hg
@@ -169,4 +349,49 @@ extern "C" int hg_offsets_to_grid(const float* offsets, float x0, float y0, floa
     else
         offsets_to_grid_kernel<1><<<static_cast<unsigned>(n), kGridBlock, 0, st>>>(offsets, rp, grid_w, grid_h, tx_count, H, grid, int(norm));
     return launch_status();
+}
+
+extern "C" int hg_offsets_to_warp(const float* offsets, float x0, float y0, float w, float h,
+                                  int32_t out_w, int32_t out_h, const float* image, int32_t channels,
+                                  int32_t img_w, int32_t img_h, float* warped, float* H, int64_t n,
+                                  hg_norm_t norm, void* cuda_stream)
+{
+    using namespace hg;
+    if (n < 0) return HG_ERR_INVALID_ARG;
+    if (norm != HG_NORM_NONE && norm != HG_NORM_H33 && norm != HG_NORM_FROBENIUS) return HG_ERR_INVALID_ARG;
+    if (!(w != 0.0f) || !(h != 0.0f)) return HG_ERR_INVALID_ARG;
+    if (out_w < 1 || out_h < 1 || img_w < 1 || img_h < 1 || channels < 1) return HG_ERR_INVALID_ARG;
+    if (int64_t(img_w) * img_h > 0x3fffffffLL || int64_t(out_w) * out_h > 0x3fffffffLL) return HG_ERR_INVALID_ARG;
+    if (n == 0) return HG_OK;
+    if (!offsets || !image || !warped) return HG_ERR_INVALID_ARG;
+    if (!aligned16(offsets) || !aligned4(warped) || !aligned4(image) || (H != nullptr && !aligned4(H))) return HG_ERR_ALIGNMENT;
+    if (n > 0x7fffffffLL) return HG_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    RectParams rp;
+    rp.x0 = x0; rp.y0 = y0; rp.w = w; rp.h = h;
+    rp.step_x = (out_w > 1) ? double(w) / double(out_w - 1) : 0.0;
+    rp.step_y = (out_h > 1) ? double(h) / double(out_h - 1) : 0.0;
+    int tx_count = pow2_at_least(out_w < 32 ? 32 : out_w);
+    if (tx_count > kGridBlock) tx_count = kGridBlock;
+    // enough CTAs to fill the machine when the batch is small: split the rows into bands
+    int bands = 1;
+    const int rows_per_pass = kGridBlock / tx_count;
+    while (n * bands < 4 * 148 && (out_h + bands - 1) / bands > rows_per_pass) bands *= 2;
+    WarpGeom g;
+    g.out_w = out_w; g.out_h = out_h; g.img_w = img_w; g.img_h = img_h; g.channels = channels;
+    g.rows_per_band = (out_h + bands - 1) / bands;
+    bands = (out_h + g.rows_per_band - 1) / g.rows_per_band;
+    const dim3 grid(static_cast<unsigned>(n), static_cast<unsigned>(bands));
+    // Stage the item's image in shared memory when two CTAs fit on an SM and the bulk copy's 16-byte rules hold.
+    const size_t img_bytes = size_t(channels) * img_w * img_h * sizeof(float);
+    const bool staged = img_bytes <= kWarpStageBytes && img_bytes % 16 == 0 && aligned16(image);
+    const int nm = int(norm);
+    if (staged) {
+        if (channels == 1) return launch_warp<1, true>(grid, img_bytes, st, offsets, rp, g, tx_count, image, warped, H, nm);
+        if (channels == 3) return launch_warp<3, true>(grid, img_bytes, st, offsets, rp, g, tx_count, image, warped, H, nm);
+        return launch_warp<0, true>(grid, img_bytes, st, offsets, rp, g, tx_count, image, warped, H, nm);
+    }
+    if (channels == 1) return launch_warp<1, false>(grid, 0, st, offsets, rp, g, tx_count, image, warped, H, nm);
+    if (channels == 3) return launch_warp<3, false>(grid, 0, st, offsets, rp, g, tx_count, image, warped, H, nm);
+    return launch_warp<0, false>(grid, 0, st, offsets, rp, g, tx_count, image, warped, H, nm);
 }

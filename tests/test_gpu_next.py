@@ -170,3 +170,39 @@ def test_f64_storage_matches_oracle(method, n, layout):
     Hd = oracle.solve_f64(oracle.METHOD_DLT, s64.numpy(), d64.numpy())
     a, b = align_to(H, Hd)
     assert np.abs(a - b).max() <= 1e-9
+
+
+# ---- 8(f)-4: hg_offsets_to_warp (reading R17) ---------------------------------------------------
+# Tolerance: bilinear sampling is continuous in the sampling position with slope <= (max - min) of the image per
+# pixel and axis; the fp32 sampling positions are within the grid tolerance (1e-3 px, typically 1e-5) of the oracle's.
+@pytest.mark.parametrize("rect,ow,oh,iw,ih,C,n,max_off", [
+    ((0.0, 0.0, 127.0, 127.0), 128, 128, 128, 128, 1, 24, 32.0),        # C5-shaped patches
+    ((0.0, 0.0, 127.0, 127.0), 128, 128, 160, 144, 3, 5, 32.0),
+    ((3.0, 2.0, 45.0, 30.0), 33, 21, 56, 40, 2, 9, 9.0),                 # odd width: scalar stores
+    ((0.0, 0.0, 63.0, 31.0), 62, 30, 64, 32, 1, 3, 6.0),                 # width % 4 == 2
+    ((0.0, 0.0, 255.0, 255.0), 256, 256, 256, 256, 1, 2, 40.0)])         # small batch: row bands
+def test_warp_matches_oracle(rect, ow, oh, iw, ih, C, n, max_off):
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 70 + ow, max_offset=max_off)
+    img = torch.rand((n, C, ih, iw), generator=torch.Generator().manual_seed(ow), dtype=torch.float32)
+    out, H = hg.hg_offsets_to_warp(off.to(DEV), *rect, ow, oh, img.to(DEV), want_H=True)
+    ref = oracle.offsets_to_warp(off.numpy(), *rect, ow, oh, img.numpy())
+    err = np.abs(out.cpu().numpy().astype(np.float64) - ref)
+    assert err.max() <= 2e-3, err.max()                                  # 2 axes x 1e-3 px x range 1
+    assert np.median(err) <= 1e-5
+    Hg, _ = hg.hg_offsets_to_grid(off.to(DEV), *rect, ow, oh, want_grid=False)
+    assert torch.equal(H, Hg)
+    assert (ref != 0).mean() > 0.5
+
+
+def test_warp_identity_translation_and_outside():
+    img = torch.rand((3, 2, 128, 128), generator=torch.Generator().manual_seed(3)).to(DEV)
+    zero = torch.zeros((3, 4, 2), device=DEV)
+    out, _ = hg.hg_offsets_to_warp(zero, 0.0, 0.0, 127.0, 127.0, 128, 128, img)
+    assert (out - img).abs().max().item() <= 2e-5
+    sh = torch.zeros((3, 4, 2), device=DEV); sh[..., 0] = 5.0; sh[..., 1] = -7.0
+    out, _ = hg.hg_offsets_to_warp(sh, 0.0, 0.0, 127.0, 127.0, 128, 128, img)
+    exp = torch.zeros_like(img); exp[:, :, 7:, :123] = img[:, :, :121, 5:]
+    assert (out - exp).abs().max().item() <= 1e-4
+    far = torch.zeros((3, 4, 2), device=DEV); far[..., 0] = 1000.0
+    out, _ = hg.hg_offsets_to_warp(far, 0.0, 0.0, 127.0, 127.0, 128, 128, img)
+    assert torch.count_nonzero(out).item() == 0

@@ -15,7 +15,8 @@ step streams from HBM: no L2 flush is needed).  Rank 0 prints ONE JSON line.
              chunked H2D -> kernel -> D2H pipeline inside the timed region)
   roofline   algorithmic bytes (100 B x 2^26) / average launch duration, against MEASURED_PEAKS.json
   cpu_baseline  the fp64 oracle (oracle/) on the host cores, on a bounded sample of the same workload
-  extras     the other hot-path rows at their BASELINE sizes (SKS C3, grid C5, RANSAC C4, C1 latency)
+  extras     the other hot-path rows at their BASELINE sizes (SKS C3, grid C5, RANSAC C4, C1 latency) and the
+             SURVEY 8(f) rows (rectangle fast path, backward, affine, SK, fp64 storage, fused warp)
 
 `--impl reference` times the oracle alone (rank 0 only), same metric/unit/config.
 With N > 1 (torchrun, one rank per GPU) every rank solves its own 2^26 sets: weak scaling, no
@@ -138,16 +139,21 @@ def event_time_ms(fn, reps, stream=None):
 
 
 # ---- the oracle on the host cores -------------------------------------------------------------------
-def oracle_rate(src_aos, dst_aos, passes, warm=1):
-    """ACA-fp64 oracle, all host cores (OpenMP): homographies/s over `passes` passes of the sample."""
+def oracle_rate(src_aos, dst_aos, passes, warm=1, min_seconds=0.0):
+    """ACA-fp64 oracle, all host cores (OpenMP): homographies/s over at least `passes` passes of the sample
+    (and at least `min_seconds` of work)."""
     import oracle
     for _ in range(warm):
         oracle.aca(src_aos, dst_aos)
+    done = 0
     t0 = time.perf_counter()
-    for _ in range(passes):
+    while True:
         oracle.aca(src_aos, dst_aos)
-    dt = time.perf_counter() - t0
-    return src_aos.shape[0] * passes / dt, oracle.num_threads(), dt
+        done += 1
+        dt = time.perf_counter() - t0
+        if done >= passes and dt >= min_seconds:
+            break
+    return src_aos.shape[0] * done / dt, oracle.num_threads(), dt, done
 
 
 def run_reference(args, rank):
@@ -158,7 +164,7 @@ def run_reference(args, rank):
     src, dst = W.general_sets(n_s, seed=W.SEED_BASE + 3)
     s, d = src.numpy(), dst.numpy()
     warm = max(args.warmup, 1)
-    rate, cores, dt = oracle_rate(s, d, passes=max(args.steps, 1), warm=warm)
+    rate, cores, dt, done = oracle_rate(s, d, passes=max(args.steps, 1), warm=warm)
     sample = "each step = the first 2^22 sets of the C3 generator (CPU stream), ACA-fp64 oracle, OpenMP over all host cores"
     line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": warm, "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -228,6 +234,55 @@ def run_extras(hg, W, dev, src, dst, H, peak):
                        "pairs_decided_in_fp64": stats["n_pairs_f64"],
                        "fp32_lane_instr_per_pair": 11, "alu_peak_instr_per_s": props.multi_processor_count * 128 * 1.965e9,
                        "frac_of_fp32_issue_peak": pairs * 11 / (ms * 1e-3) / (props.multi_processor_count * 128 * 1.965e9)}
+    ex.update(run_next_rows(hg, W, dev, peak))
+    return ex
+
+
+def run_next_rows(hg, W, dev, peak):
+    """SURVEY.md 8(f) rows at 2^26 items (2^25 for fp64 storage): all streaming, HBM-bound."""
+    ex = {}
+    n = 1 << 26
+
+    def leg(name, fn, bytes_per_item, items, reps=10, **kw):
+        for _ in range(3):
+            fn()
+        ms = event_time_ms(fn, reps) / reps
+        gbs = items * bytes_per_item / ms / 1e6
+        ex[name] = dict({"ms": ms, "items_per_s": items / ms * 1e3, "GBps": gbs, "frac_of_peak": gbs / peak,
+                         "bytes_per_item": bytes_per_item}, **kw)
+
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 6, device=dev)
+    Haos = torch.empty((n, 3, 3), dtype=torch.float32, device=dev)
+    leg("rect_aos_2p26", lambda: hg.hg_aca_rect_batched(off, 0.0, 0.0, 127.0, 127.0, H=Haos, layout=hg.AOS, norm=hg.NORM_H33), 68, n)
+    g = torch.randn((n, 3, 3), device=dev)
+    go = torch.empty((n, 4, 2), dtype=torch.float32, device=dev)
+    leg("rect_backward_2p26", lambda: hg.hg_aca_rect_backward(off, 0.0, 0.0, 127.0, 127.0, g, grad_offsets=go), 100, n)
+    del g, go, Haos
+    osoa = off.reshape(n, 8).t().contiguous()
+    del off
+    Hsoa = torch.empty((9, n), dtype=torch.float32, device=dev)
+    leg("rect_soa_2p26", lambda: hg.hg_aca_rect_batched(osoa, 0.0, 0.0, 127.0, 127.0, H=Hsoa, layout=hg.SOA, norm=hg.NORM_H33), 68, n)
+    a = torch.rand((6, n), device=dev) * 600.0
+    b = torch.rand((6, n), device=dev) * 600.0
+    leg("affine_soa_2p26", lambda: hg.hg_affine_batched(a, b, H=Hsoa), 84, n)
+    del a, b
+    osoa.mul_(10.0).add_(300.0)                                  # reuse as image quadruples for the SK leg
+    leg("sk_soa_2p26", lambda: hg.hg_sk_batched((0.35, 1.6), (-0.8, -1.1), osoa, H=Hsoa), 68, n)
+    del osoa, Hsoa
+    m = 1 << 25
+    s64 = torch.rand((8, m), device=dev, dtype=torch.float64) * 600.0
+    d64 = torch.rand((8, m), device=dev, dtype=torch.float64) * 600.0
+    H64 = torch.empty((9, m), device=dev, dtype=torch.float64)
+    leg("aca_f64_soa_2p25", lambda: hg.hg_aca_batched_f64(s64, d64, H=H64), 200, m)
+    leg("sks_f64_soa_2p25", lambda: hg.hg_sks_batched_f64(s64, d64, H=H64), 200, m)
+    del s64, d64, H64
+    # offsets -> H -> bilinear warp of 8192 single-channel 128 x 128 patches (4 B read + 4 B written per pixel)
+    k = 8192
+    off5 = W.offsets_workload(k, seed=W.SEED_BASE + 5, device=dev)
+    img = torch.rand((k, 1, 128, 128), device=dev)
+    out = torch.empty_like(img)
+    leg("warp_c5_1ch", lambda: hg.hg_offsets_to_warp(off5, 0.0, 0.0, 127.0, 127.0, 128, 128, img, warped=out), 8, k * 128 * 128,
+        unit="pixels")
     return ex
 
 
@@ -336,10 +391,10 @@ def main():
         n_s = min(n, 1 << 24)
         s_aos = W.to_aos(src[:, :n_s].contiguous()).cpu().numpy()
         d_aos = W.to_aos(dst[:, :n_s].contiguous()).cpu().numpy()
-        rate, cores, dt = oracle_rate(s_aos, d_aos, passes=3)
+        rate, cores, dt, done = oracle_rate(s_aos, d_aos, passes=3, min_seconds=10.0)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": "first 2^%d sets of the timed workload, 3 passes of the ACA-fp64 oracle (OpenMP, %.1f s)"
-                                          % (n_s.bit_length() - 1, dt)}
+                                "sample": "first 2^%d sets of the timed workload, %d passes of the ACA-fp64 oracle (OpenMP, %.1f s)"
+                                          % (n_s.bit_length() - 1, done, dt)}
         del s_aos, d_aos
     if world == 1 and not args.no_extras:
         try:

@@ -218,6 +218,40 @@ def ransac(src_xy, dst_xy, hyp_idx, threshold: float, band_rel: float = 1e-4, so
             "best_index": int(best_index.value), "best_count": int(best_count.value)}
 
 
+def philox4x32_10(ctr, key) -> np.ndarray:
+    c = np.ascontiguousarray(ctr, dtype=np.uint32); k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.zeros(4, dtype=np.uint32)
+    lib().hgo_philox4x32_10(_p(c), _p(k), _p(out))
+    return out
+
+
+def ransac_sample(seed: int, h0: int, n: int, n_pts: int) -> np.ndarray:
+    idx = np.zeros((n, 4), dtype=np.int32)
+    lib().hgo_ransac_sample(ctypes.c_uint64(seed), ctypes.c_int64(h0), ctypes.c_int64(n), ctypes.c_int32(n_pts), _p(idx))
+    return idx
+
+
+def ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, threshold: float, confidence: float,
+                    band_rel: float = 1e-4):
+    """Sampling + rounds + adaptive termination (reading R19).  Returns dict(n_evaluated, hyp_idx [n_evaluated,4],
+    counts, band_counts, best_H, best_index, best_count, margins [rounds])."""
+    s = _f32(src_xy, (2,)); d = _f32(dst_xy, (2,))
+    n_pts = s.shape[0]
+    idx = np.zeros((max_hyp, 4), dtype=np.int32)
+    counts = np.zeros(max_hyp, dtype=np.int32); band = np.zeros(max_hyp, dtype=np.int32)
+    n_rounds = (max_hyp + round_hyp - 1) // round_hyp
+    margins = np.full(n_rounds, np.nan)
+    best_H = np.full((3, 3), np.nan)
+    bi, bc, ne = ctypes.c_int64(-1), ctypes.c_int32(-1), ctypes.c_int64(0)
+    lib().hgo_ransac_adaptive(_p(s), _p(d), ctypes.c_int32(n_pts), ctypes.c_uint64(seed), ctypes.c_int64(max_hyp),
+                              ctypes.c_int64(round_hyp), ctypes.c_double(float(np.float32(threshold))),
+                              ctypes.c_double(float(np.float32(confidence))), ctypes.c_double(band_rel), _p(idx), _p(counts),
+                              _p(band), _p(best_H), ctypes.byref(bi), ctypes.byref(bc), ctypes.byref(ne), _p(margins))
+    n = int(ne.value)
+    return {"n_evaluated": n, "hyp_idx": idx[:n], "counts": counts[:n], "band_counts": band[:n], "best_H": best_H,
+            "best_index": int(bi.value), "best_count": int(bc.value), "margins": margins}
+
+
 def residuals(H, src_xy, dst_xy) -> np.ndarray:
     Hc = np.ascontiguousarray(np.asarray(H, dtype=np.float64)).reshape(3, 3)
     s = _f32(src_xy, (2,)); d = _f32(dst_xy, (2,))

@@ -327,6 +327,61 @@ void hgo_ransac(const float* src_xy, const float* dst_xy, int32_t n_pts,
     }
 }
 
+// Known-answer access to the generator, and the sampled indices of hypotheses [h0, h0 + n).
+void hgo_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { hgo::philox4x32_10(ctr, key, out); }
+
+void hgo_ransac_sample(uint64_t seed, int64_t h0, int64_t n, int32_t n_pts, int32_t* idx)
+{
+    for (int64_t i = 0; i < n; ++i) hgo::sample4(seed, static_cast<uint64_t>(h0 + i), n_pts, idx + 4 * i);
+}
+
+// RANSAC with on-device-style sampling and adaptive termination ("99 %"; reading R19).
+// Hypotheses are scored in rounds of round_hyp; after a round with `done` hypotheses scored and best count c,
+//   w = c / n_pts,  s = done * log1p(-w^4) - log1p(-confidence);  stop iff s <= 0
+// (i.e. done >= log(1 - confidence) / log(1 - w^4), the standard number of samples for an all-inlier draw);
+// confidence <= 0 never stops early.  counts / idx_out / band_counts hold max_hyp entries (those past
+// n_evaluated are left untouched); margins[r] = s after round r (NaN when not computed).
+void hgo_ransac_adaptive(const float* src_xy, const float* dst_xy, int32_t n_pts, uint64_t seed,
+                         int64_t max_hyp, int64_t round_hyp, double t, double confidence, double band_rel,
+                         int32_t* idx_out, int32_t* counts, int32_t* band_counts, double* best_H,
+                         int64_t* best_index, int32_t* best_count, int64_t* n_evaluated, double* margins)
+{
+    int64_t bi = -1, done = 0, round = 0;
+    int32_t bc = -1;
+    while (done < max_hyp) {
+        const int64_t m = (max_hyp - done < round_hyp) ? (max_hyp - done) : round_hyp;
+        hgo_ransac_sample(seed, done, m, n_pts, idx_out + 4 * done);
+        int64_t rbi = -1;
+        int32_t rbc = -1;
+        hgo_ransac(src_xy, dst_xy, n_pts, idx_out + 4 * done, m, t, band_rel, 1, counts + done,
+                   band_counts ? band_counts + done : nullptr, nullptr, &rbi, &rbc);
+        if (rbc > bc) { bc = rbc; bi = done + rbi; }          // ties keep the lowest index
+        done += m;
+        double s = NAN;
+        if (confidence > 0.0) {
+            const double w = static_cast<double>(bc) / static_cast<double>(n_pts);
+            const double q = w * w * w * w;
+            s = static_cast<double>(done) * std::log1p(-q) - std::log1p(-confidence);
+        }
+        if (margins) margins[round] = s;
+        ++round;
+        if (confidence > 0.0 && s <= 0.0) break;
+    }
+    *n_evaluated = done;
+    *best_index = bi;
+    *best_count = bc;
+    if (best_H && bi >= 0) {
+        double sv[8], dv[8];
+        for (int k = 0; k < 4; ++k) {
+            const int32_t j = idx_out[4 * bi + k];
+            sv[2 * k] = src_xy[2 * j];     sv[2 * k + 1] = src_xy[2 * j + 1];
+            dv[2 * k] = dst_xy[2 * j];     dv[2 * k + 1] = dst_xy[2 * j + 1];
+        }
+        hgo::aca<double>(sv, dv, best_H);
+        hgo::normal_form(best_H);
+    }
+}
+
 // Residuals of one H against all correspondences (used by tests to look at single pairs).
 void hgo_residuals(const double* H, const float* src_xy, const float* dst_xy, int32_t n_pts, double* r)
 {

@@ -457,4 +457,49 @@ template <int N> inline Dual<N> operator/(const Dual<N>& a, const Dual<N>& b)
 template <int N> inline Dual<N> operator-(const Dual<N>& a)
 { Dual<N> r(-a.v); for (int i = 0; i < N; ++i) r.g[i] = -a.g[i]; return r; }
 
+// ---------------------------------------------------------------------------
+// Counter-based generator for on-device hypothesis sampling ("RANSAC extras"): the
+// published Philox4x32-10 (Salmon et al., SC'11), restated: 10 rounds of
+//   (c0, c1, c2, c3) <- (hi(M1*c2) ^ c1 ^ k0, lo(M1*c2), hi(M0*c0) ^ c3 ^ k1, lo(M0*c0)),  k += (W0, W1).
+// Pinned by the published known-answer vectors (tests/golden/philox4x32_10_kat.json).
+// ---------------------------------------------------------------------------
+inline void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    const uint64_t M0 = 0xD2511F53ull, M1 = 0xCD9E8D57ull;
+    const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = M0 * c0, p1 = M1 * c2;
+        const uint32_t n0 = static_cast<uint32_t>(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n1 = static_cast<uint32_t>(p1);
+        const uint32_t n2 = static_cast<uint32_t>(p0 >> 32) ^ c3 ^ k1;
+        const uint32_t n3 = static_cast<uint32_t>(p0);
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// The 4 indices of hypothesis h (reading R19 of DESIGN.md): attempt a = 0, 1, ... draws
+// Philox(counter = (lo32(h), hi32(h), a, 0), key = (lo32(seed), hi32(seed))) and maps each word r to
+// floor(r * n_pts / 2^32); the first attempt whose 4 indices are pairwise distinct is taken; after 32
+// failed attempts (only plausible for n_pts < 8) the sample is i, i+1, i+2, i+3 (mod n_pts), i = attempt 0's
+// first index.
+inline void sample4(uint64_t seed, uint64_t h, int32_t n_pts, int32_t idx[4])
+{
+    const uint32_t key[2] = { static_cast<uint32_t>(seed), static_cast<uint32_t>(seed >> 32) };
+    int32_t first = 0;
+    for (uint32_t a = 0; a < 32; ++a) {
+        const uint32_t ctr[4] = { static_cast<uint32_t>(h), static_cast<uint32_t>(h >> 32), a, 0u };
+        uint32_t r[4];
+        philox4x32_10(ctr, key, r);
+        for (int k = 0; k < 4; ++k)
+            idx[k] = static_cast<int32_t>((static_cast<uint64_t>(r[k]) * static_cast<uint64_t>(n_pts)) >> 32);
+        if (a == 0) first = idx[0];
+        if (idx[0] != idx[1] && idx[0] != idx[2] && idx[0] != idx[3] && idx[1] != idx[2] && idx[1] != idx[3] && idx[2] != idx[3])
+            return;
+    }
+    for (int k = 0; k < 4; ++k) idx[k] = (first + k) % n_pts;
+}
+
 }  // namespace hgo

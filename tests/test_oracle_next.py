@@ -189,3 +189,64 @@ def test_warp_identity_and_integer_translation_are_exact():
     exp = np.zeros_like(out)
     exp[:, :, 2:, :29] = img[:, :, :30, 3:]                       # out(x, y) = img(x + 3, y - 2), zero outside
     assert np.abs(out - exp).max() <= 1e-10
+
+
+# ---- RANSAC extras: counter-based sampling and adaptive termination (reading R19) ---------
+def test_philox_known_answers():
+    import json
+    from pathlib import Path
+    kat = json.loads((Path(__file__).parent / "golden" / "philox4x32_10_kat.json").read_text())
+    for v in kat["vectors"]:
+        out = oracle.philox4x32_10([int(x, 16) for x in v["ctr"]], [int(x, 16) for x in v["key"]])
+        assert [int(x) for x in out] == [int(x, 16) for x in v["out"]]
+
+
+def test_sampling_is_distinct_in_range_uniform_and_counter_based():
+    idx = oracle.ransac_sample(seed=0x1234567890ABCDEF, h0=0, n=200000, n_pts=4096)
+    assert idx.min() >= 0 and idx.max() < 4096
+    srt = np.sort(idx, axis=1)
+    assert (np.diff(srt, axis=1) > 0).all()                                   # pairwise distinct
+    hist = np.bincount(idx.reshape(-1), minlength=4096)
+    exp = idx.size / 4096.0
+    assert np.abs(hist - exp).max() <= 6.0 * np.sqrt(exp)                      # uniform (6 sigma over 4096 bins)
+    # counter-based: any sub-range reproduces the same rows; another seed does not
+    assert np.array_equal(oracle.ransac_sample(0x1234567890ABCDEF, 777, 100, 4096), idx[777:877])
+    assert not np.array_equal(oracle.ransac_sample(0x1234567890ABCDEE, 0, 100, 4096), idx[:100])
+    # the index map is floor(r * n / 2^32) of the four Philox words of attempt 0 (when they are distinct)
+    r = oracle.philox4x32_10([5, 0, 0, 0], [0x90ABCDEF, 0x12345678]).astype(np.uint64)
+    m = (r * np.uint64(4096)) >> np.uint64(32)
+    if len(set(m.tolist())) == 4:
+        assert np.array_equal(idx[5], m.astype(np.int32))
+    # tiny tables: still distinct and in range (rejection, then the consecutive fallback)
+    small = oracle.ransac_sample(3, 0, 5000, 4)
+    assert (np.sort(small, axis=1) == np.arange(4)).all()
+
+
+def test_adaptive_termination_rule():
+    """Planted model, zero noise, exactly half the points inliers: w^4 = 1/16, needed = log(0.01)/log(15/16) = 71.4
+    hypotheses once an all-inlier sample has been seen; rounds of 16 => stop after 80."""
+    rng = np.random.default_rng(5)
+    n = 200
+    src = (rng.random((n, 2)) * [640, 480]).astype(np.float32)
+    A = np.array([[1.0, 0.0, 16.0], [0.0, 1.0, -8.0]])                       # exact integer translation: inliers are exact in fp32
+    dst = src.copy(); dst[:, 0] += 16.0; dst[:, 1] -= 8.0
+    out_mask = np.arange(n) % 2 == 1
+    dst[out_mask] = (rng.random((out_mask.sum(), 2)) * [640, 480]).astype(np.float32)
+    res = oracle.ransac_adaptive(src, dst, seed=11, max_hyp=4096, round_hyp=16, threshold=3.0, confidence=0.99)
+    first_hit = int(np.argmax(res["counts"] >= 100)) if (res["counts"] >= 100).any() else None
+    assert first_hit is not None and res["best_count"] >= 100
+    w4 = (res["best_count"] / n) ** 4
+    needed = np.log(0.01) / np.log1p(-w4)
+    # the run stops at the first multiple of 16 that is >= needed and lies after the round in which the best was found
+    stop = res["n_evaluated"]
+    assert stop % 16 == 0 and stop >= needed and stop >= first_hit + 1
+    counts_by_round = [res["counts"][: k].max() for k in range(16, stop, 16)]
+    for k, c in zip(range(16, stop, 16), counts_by_round):                    # no earlier round satisfied the rule
+        assert k < np.log(0.01) / np.log1p(-((c / n) ** 4)) if c > 0 else True
+    # consistency with the plain scorer on the sampled indices, and the index of the best
+    ref = oracle.ransac(src, dst, res["hyp_idx"], 3.0)
+    assert np.array_equal(ref["counts"], res["counts"]) and ref["best_index"] == res["best_index"]
+    assert np.array_equal(res["hyp_idx"], oracle.ransac_sample(11, 0, stop, n))
+    # confidence 0: never stops early
+    full = oracle.ransac_adaptive(src, dst, seed=11, max_hyp=300, round_hyp=64, threshold=3.0, confidence=0.0)
+    assert full["n_evaluated"] == 300

@@ -243,10 +243,38 @@ HG_API int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy,
                                 int32_t* best_count, void* workspace, size_t workspace_bytes,
                                 void* cuda_stream);
 
+/* --------------------------------------------------------------------------------------------
+ * hg_ransac_adaptive -- the same fused gather-solve-score with the two "RANSAC extras" of the
+ * hypothesise-and-verify loop (Sec. 2.2; "99 %" sampling counts) done on the device
+ * (reading R19):
+ *  - sampling: hypothesis h takes its 4 indices from the counter-based generator Philox4x32-10,
+ *    counter = (lo32(h), hi32(h), attempt, 0), key = (lo32(seed), hi32(seed)); word r -> index
+ *    floor(r * n_pts / 2^32); the first attempt with 4 pairwise distinct indices is used (after 32
+ *    failed attempts: i, i+1, i+2, i+3 mod n_pts, i = attempt 0's first index);
+ *  - adaptive termination: hypotheses are scored in rounds of round_hyp; after a round with `done`
+ *    hypotheses scored and best count c, w = c / n_pts and the run stops iff
+ *    done * log1p(-w^4) <= log1p(-confidence) (fp64), i.e. done >= log(1-confidence)/log(1-w^4);
+ *    confidence <= 0 scores all max_hyp hypotheses.  No host synchronisation: every round is
+ *    enqueued, rounds after the stop return immediately.
+ *   seed, max_hyp, round_hyp : max_hyp <= 2^31-1, round_hyp >= 1, at most 65536 rounds
+ *   confidence     : < 1
+ *   counts         : nullable, int32[max_hyp]; entries >= *n_evaluated are not written
+ *   hyp_idx_out    : nullable, int32[max_hyp][4], 16-byte aligned: the sampled indices (same rule)
+ *   best_H, best_index, best_count : as hg_ransac_hypothesize_score, over the hypotheses scored
+ *   n_evaluated    : nullable, int64: hypotheses scored (a multiple of round_hyp, or max_hyp)
+ *   workspace      : >= hg_ransac_workspace_bytes(n_pts, max_hyp) bytes, 16-byte aligned
+ * Errors: as hg_ransac_hypothesize_score.
+ * -------------------------------------------------------------------------------------------- */
+HG_API int hg_ransac_adaptive(const float* src_xy, const float* dst_xy, int32_t n_pts, uint64_t seed,
+                       int64_t max_hyp, int64_t round_hyp, float threshold_px, float confidence,
+                       int32_t* counts, int32_t* hyp_idx_out, float* best_H, int64_t* best_index,
+                       int32_t* best_count, int64_t* n_evaluated, void* workspace,
+                       size_t workspace_bytes, void* cuda_stream);
+
 /* After hg_ransac_hypothesize_score has completed on its stream, the first 4 int64 words of
  * the workspace hold statistics of that call (device memory; copy them out to read):
  *   [0] packed best key, [1] number of hypotheses that had at least one pair decided in fp64,
- *   [2] number of (hypothesis, point) pairs decided in fp64, [3] reserved.                      */
+ *   [2] number of (hypothesis, point) pairs decided in fp64, [3] hypotheses scored (adaptive mode).                      */
 #define HG_RANSAC_STAT_WORDS 4
 
 /* Host-buffer form: all pointers are HOST pointers; the call allocates device memory and the

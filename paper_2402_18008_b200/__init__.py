@@ -21,7 +21,8 @@ __all__ = [
     "PREC_F64", "PREC_F32", "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host",
     "hg_sks_batched_host", "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
     "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
-    "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_status_string",
+    "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
+    "hg_status_string",
     "hg_version", "hg_built_for_sm", "EXPORTS",
 ]
 
@@ -37,7 +38,7 @@ EXPORTS = [
     "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
     "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_affine_batched",
     "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
-    "hg_ransac_hypothesize_score_host", "hg_status_string", "hg_version", "hg_built_for_sm",
+    "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive", "hg_status_string", "hg_version", "hg_built_for_sm",
 ]
 
 
@@ -83,13 +84,15 @@ def lib() -> ctypes.CDLL:
         L.hg_ransac_workspace_bytes.restype = ctypes.c_size_t
         L.hg_ransac_hypothesize_score.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp,
                                                   _vp, ctypes.c_size_t, _vp]
+        L.hg_ransac_adaptive.argtypes = [_vp, _vp, _c_i32, ctypes.c_uint64, _c_i64, _c_i64, _c_f32, _c_f32, _vp, _vp, _vp, _vp, _vp,
+                                         _vp, _vp, ctypes.c_size_t, _vp]
         L.hg_ransac_hypothesize_score_host.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp]
         L.hg_status_string.argtypes = [_c_int]
         L.hg_status_string.restype = ctypes.c_char_p
         for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
                      "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
                      "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
-                     "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host",
+                     "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
                      "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
         _lib = L
@@ -388,6 +391,34 @@ def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, co
     _check(st, "hg_ransac_hypothesize_score")
     return {"counts": counts, "best_H": best_H, "best_index": best_index, "best_count": best_count,
             "workspace": workspace}
+
+
+def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, threshold_px: float, confidence: float,
+                       want_counts: bool = True, want_idx: bool = False, workspace=None, stream=None):
+    """On-device sampling (Philox4x32-10) + rounds + adaptive termination.  Returns dict(counts [max_hyp] or None,
+    hyp_idx [max_hyp,4] or None, best_H [3,3], best_index [1], best_count [1], n_evaluated [1], workspace) -- device tensors."""
+    n_pts = int(src_xy.shape[0])
+    dev = src_xy.device
+    need = hg_ransac_workspace_bytes(n_pts, max_hyp)
+    if workspace is None:
+        workspace = torch.empty((max(need, 16),), dtype=torch.uint8, device=dev)
+    counts = torch.zeros((max_hyp,), dtype=torch.int32, device=dev) if want_counts else None
+    idx = torch.zeros((max_hyp, 4), dtype=torch.int32, device=dev) if want_idx else None
+    best_H = torch.empty((3, 3), dtype=torch.float32, device=dev)
+    best_index = torch.empty((1,), dtype=torch.int64, device=dev)
+    best_count = torch.empty((1,), dtype=torch.int32, device=dev)
+    n_eval = torch.empty((1,), dtype=torch.int64, device=dev)
+    with torch.cuda.device(dev):
+        st = lib().hg_ransac_adaptive(
+            _ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
+            int(seed) & 0xFFFFFFFFFFFFFFFF, int(max_hyp), int(round_hyp), float(threshold_px), float(confidence),
+            _ptr(counts, torch.int32, "cuda", "counts"), _ptr(idx, torch.int32, "cuda", "hyp_idx_out"),
+            _ptr(best_H, torch.float32, "cuda", "best_H"), _ptr(best_index, torch.int64, "cuda", "best_index"),
+            _ptr(best_count, torch.int32, "cuda", "best_count"), _ptr(n_eval, torch.int64, "cuda", "n_evaluated"),
+            _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()), _stream(stream))
+    _check(st, "hg_ransac_adaptive")
+    return {"counts": counts, "hyp_idx": idx, "best_H": best_H, "best_index": best_index, "best_count": best_count,
+            "n_evaluated": n_eval, "workspace": workspace}
 
 
 def ransac_stats(workspace: torch.Tensor) -> dict:

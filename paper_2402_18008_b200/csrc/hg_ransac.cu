@@ -27,9 +27,10 @@ struct RansacHeader {               // first 64 bytes of the workspace
     unsigned long long best_key;    // (count << 32) | (0xFFFFFFFF - hypothesis index)
     unsigned long long n_fixup;     // hypotheses with at least one pair decided in fp64
     unsigned long long n_pairs_f64; // (hypothesis, point) pairs decided in fp64
-    unsigned long long reserved;
+    unsigned long long n_evaluated; // adaptive mode: hypotheses scored when the run stopped
     unsigned int bound_bits[4];     // float bits of max|sx|, max|sy|, max|dx/t|, max|dy/t|
-    unsigned int pad[4];
+    unsigned int stop;              // adaptive mode: set by the round kernel, later rounds return at once
+    unsigned int pad[3];
 };
 static_assert(sizeof(RansacHeader) == kHeaderBytes, "header layout");
 
@@ -74,6 +75,53 @@ __device__ __forceinline__ void gather_sets(const float2* __restrict__ src_xy, c
         s[2 * k] = sp.x; s[2 * k + 1] = sp.y;
         d[2 * k] = dq.x; d[2 * k + 1] = dq.y;
     }
+}
+
+// ---- where the hypotheses of a launch come from ----------------------------------------------
+struct HypSource {
+    const int4* idx;            // caller-supplied indices [n_hyp][4], or nullptr: sample on the device
+    int4* idx_out;              // sampling mode, nullable: the sampled indices are written here
+    unsigned long long seed;    // sampling mode
+    int h0, h1;                 // this launch scores hypotheses [h0, h1)
+    int check_stop;             // 1: return at once when hdr->stop is set (adaptive termination)
+};
+
+// Philox4x32-10 (Salmon et al., SC'11), the counter-based generator of reading R19: 10 rounds of
+// (c0,c1,c2,c3) <- (hi(M1 c2) ^ c1 ^ k0, lo(M1 c2), hi(M0 c0) ^ c3 ^ k1, lo(M0 c0)), k += (W0, W1).
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+        const unsigned hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+        k.x += 0x9E3779B9u; k.y += 0xBB67AE85u;
+    }
+    return c;
+}
+
+// The 4 indices of hypothesis h: attempt a draws Philox(counter = (lo(h), hi(h), a, 0), key = seed), index =
+// floor(word * n_pts / 2^32); first attempt with pairwise distinct indices wins; after 32 failures
+// i, i+1, i+2, i+3 (mod n_pts) with i = attempt 0's first index.
+__device__ __forceinline__ int4 sample4(unsigned long long seed, unsigned long long h, int n_pts)
+{
+    const uint2 key = make_uint2(static_cast<unsigned>(seed), static_cast<unsigned>(seed >> 32));
+    int first = 0;
+    for (unsigned a = 0; a < 32u; ++a) {
+        const uint4 r = philox4x32_10(make_uint4(static_cast<unsigned>(h), static_cast<unsigned>(h >> 32), a, 0u), key);
+        const int4 id = make_int4(static_cast<int>(__umulhi(r.x, static_cast<unsigned>(n_pts))),
+                                  static_cast<int>(__umulhi(r.y, static_cast<unsigned>(n_pts))),
+                                  static_cast<int>(__umulhi(r.z, static_cast<unsigned>(n_pts))),
+                                  static_cast<int>(__umulhi(r.w, static_cast<unsigned>(n_pts))));
+        if (a == 0) first = id.x;
+        if (id.x != id.y && id.x != id.z && id.x != id.w && id.y != id.z && id.y != id.w && id.z != id.w) return id;
+    }
+    return make_int4(first % n_pts, (first + 1) % n_pts, (first + 2) % n_pts, (first + 3) % n_pts);
+}
+
+__device__ __forceinline__ int4 hypothesis_indices(const HypSource& hs, int hidx, int n_pts)
+{
+    return hs.idx ? __ldg(hs.idx + hidx) : sample4(hs.seed, static_cast<unsigned long long>(hidx), n_pts);
 }
 
 // fp64 ACA solve, max-abs normalisation, threshold folding and the error band.
@@ -262,9 +310,10 @@ constexpr int kGroup = 4;     // table entries per slow-path check
 
 __global__ void __launch_bounds__(kRBlock, 2)
 ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts,
-                    const float4* __restrict__ table, int n_pairs, const int4* __restrict__ hyp_idx,
-                    int n_hyp, double inv_t, double t, int* __restrict__ counts, RansacHeader* __restrict__ hdr)
+                    const float4* __restrict__ table, int n_pairs, HypSource hs,
+                    double inv_t, double t, int* __restrict__ counts, RansacHeader* __restrict__ hdr)
 {
+    if (hs.check_stop && hdr->stop) return;                 // uniform: written by an earlier launch on this stream
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4* stage_buf = reinterpret_cast<float4*>(smem_raw);                       // kStages * kChunkPairs * 2 float4
     double* Hstash = reinterpret_cast<double*>(smem_raw + size_t(kStages) * kChunkPairs * 32);   // [9][kRBlock]
@@ -286,15 +335,16 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     }
 
     // hypothesis set-up overlaps the first table copies
-    const int hidx = blockIdx.x * kRBlock + threadIdx.x;
-    const bool active = hidx < n_hyp;
+    const int hidx = hs.h0 + blockIdx.x * kRBlock + threadIdx.x;
+    const bool active = hidx < hs.h1;
     HypConst hc;
     bool ok = false;
     {
         const float bounds[4] = { __uint_as_float(hdr->bound_bits[0]), __uint_as_float(hdr->bound_bits[1]),
                                   __uint_as_float(hdr->bound_bits[2]), __uint_as_float(hdr->bound_bits[3]) };
         double s[8], d[8], Hn[9];
-        const int4 id = active ? __ldg(hyp_idx + hidx) : make_int4(0, 0, 0, 0);    // inactive: degenerate => sure outliers
+        const int4 id = active ? hypothesis_indices(hs, hidx, n_pts) : make_int4(0, 0, 0, 0);   // inactive: degenerate => sure outliers
+        if (active && hs.idx_out) hs.idx_out[hidx] = id;
         gather_sets(src_xy, dst_xy, id, s, d);
         ok = make_hypothesis(s, d, inv_t, bounds, Hn, hc) && active;
 #pragma unroll
@@ -352,20 +402,36 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     }
 }
 
+// ---- 3. round (adaptive mode): the termination rule after `done` hypotheses ----------------------
+// Reading R19: w = best_count / n_pts; stop iff done * log1p(-w^4) <= log1p(-confidence), i.e. once
+// done >= log(1 - confidence) / log(1 - w^4); confidence <= 0 never stops early.
+__global__ void ransac_round_kernel(RansacHeader* __restrict__ hdr, int n_pts, long long done, double confidence, int last)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0 || hdr->stop) return;
+    bool stop = last != 0;
+    if (confidence > 0.0) {
+        const double w = static_cast<double>(hdr->best_key >> 32) / static_cast<double>(n_pts);
+        const double q = w * w * w * w;
+        stop = stop || (static_cast<double>(done) * log1p(-q) - log1p(-confidence) <= 0.0);
+    }
+    if (stop) { hdr->n_evaluated = static_cast<unsigned long long>(done); hdr->stop = 1u; }
+}
+
 // ---- 4. finalize -----------------------------------------------------------------------------
-__global__ void ransac_finalize_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy,
-                                       const int4* __restrict__ hyp_idx, const RansacHeader* __restrict__ hdr,
+__global__ void ransac_finalize_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts,
+                                       HypSource hs, const RansacHeader* __restrict__ hdr,
                                        float* __restrict__ best_H, long long* __restrict__ best_index,
-                                       int* __restrict__ best_count)
+                                       int* __restrict__ best_count, long long* __restrict__ n_evaluated)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     const unsigned long long key = hdr->best_key;
     const unsigned idx = 0xFFFFFFFFu - static_cast<unsigned>(key & 0xFFFFFFFFull);
     if (best_index) *best_index = static_cast<long long>(idx);
     if (best_count) *best_count = static_cast<int>(key >> 32);
+    if (n_evaluated) *n_evaluated = static_cast<long long>(hdr->n_evaluated);
     if (best_H) {
         double s[8], d[8], H[9];
-        gather_sets(src_xy, dst_xy, __ldg(hyp_idx + idx), s, d);
+        gather_sets(src_xy, dst_xy, hypothesis_indices(hs, static_cast<int>(idx), n_pts), s, d);
         aca_solve<double>(s, d, H);
         normalise<double>(H, 2);
 #pragma unroll
@@ -385,6 +451,67 @@ extern "C" size_t hg_ransac_workspace_bytes(int32_t n_pts, int64_t n_hyp)
     return hg::kHeaderBytes + hg::align16(hg::table_bytes(n_pts));
 }
 
+namespace hg {
+
+// Shared by the two device entry points.  Sampling mode: hyp_idx == nullptr.  round_hyp == n_hyp and
+// confidence <= 0 give the single-launch behaviour of hg_ransac_hypothesize_score.
+static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, const int32_t* hyp_idx, int32_t* hyp_idx_out,
+                      unsigned long long seed, int64_t n_hyp, int64_t round_hyp, float threshold_px, double confidence,
+                      bool adaptive, int32_t* counts, float* best_H, int64_t* best_index, int32_t* best_count,
+                      int64_t* n_evaluated, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    RansacHeader* hdr = reinterpret_cast<RansacHeader*>(ws);
+    float4* table = reinterpret_cast<float4*>(ws + kHeaderBytes);
+    const float2* s2 = reinterpret_cast<const float2*>(src_xy);
+    const float2* d2 = reinterpret_cast<const float2*>(dst_xy);
+    const int n_pairs = (n_pts + 1) / 2;
+    const double t = static_cast<double>(threshold_px);
+    const double inv_t = 1.0 / t;
+    (void)workspace_bytes;
+
+    if (cudaMemsetAsync(hdr, 0, kHeaderBytes, st) != cudaSuccess) return HG_ERR_CUDA;
+    {
+        int blocks = (n_pairs + 255) / 256;
+        if (blocks > 1184) blocks = 1184;
+        ransac_prep_kernel<<<blocks, 256, 0, st>>>(s2, d2, n_pts, n_pairs, inv_t, table, hdr);
+        if (launch_status() != HG_OK) return HG_ERR_CUDA;
+    }
+    const size_t smem = size_t(kStages) * kChunkPairs * 32 + size_t(9) * kRBlock * sizeof(double) + size_t(2) * kRBlock * sizeof(float) +
+                        kStages * sizeof(uint64_t);
+    static bool attr_set = false;          // idempotent; a race only repeats the same call
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(ransac_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
+            return HG_ERR_CUDA;
+        attr_set = true;
+    }
+    HypSource hs;
+    hs.idx = reinterpret_cast<const int4*>(hyp_idx);
+    hs.idx_out = reinterpret_cast<int4*>(hyp_idx_out);
+    hs.seed = seed;
+    hs.check_stop = adaptive ? 1 : 0;
+    for (int64_t h0 = 0; h0 < n_hyp; h0 += round_hyp) {
+        const int64_t h1 = (h0 + round_hyp < n_hyp) ? h0 + round_hyp : n_hyp;
+        hs.h0 = static_cast<int>(h0); hs.h1 = static_cast<int>(h1);
+        const unsigned blocks = static_cast<unsigned>((h1 - h0 + kRBlock - 1) / kRBlock);
+        ransac_score_kernel<<<blocks, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, hs, inv_t, t, counts, hdr);
+        if (launch_status() != HG_OK) return HG_ERR_CUDA;
+        if (adaptive) {
+            ransac_round_kernel<<<1, 32, 0, st>>>(hdr, n_pts, static_cast<long long>(h1), confidence, h1 == n_hyp ? 1 : 0);
+            if (launch_status() != HG_OK) return HG_ERR_CUDA;
+        }
+    }
+    if (best_H || best_index || best_count || n_evaluated) {
+        ransac_finalize_kernel<<<1, 32, 0, st>>>(s2, d2, n_pts, hs, hdr, best_H, reinterpret_cast<long long*>(best_index), best_count,
+                                                 reinterpret_cast<long long*>(n_evaluated));
+        if (launch_status() != HG_OK) return HG_ERR_CUDA;
+    }
+    return HG_OK;
+}
+
+}  // namespace hg
+
 extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy, int32_t n_pts,
                                            const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
                                            int32_t* counts, float* best_H, int64_t* best_index,
@@ -402,44 +529,32 @@ extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst
         (best_index && (reinterpret_cast<uintptr_t>(best_index) & 7u)) || (best_count && !aligned4(best_count)))
         return HG_ERR_ALIGNMENT;
     if (workspace_bytes < hg_ransac_workspace_bytes(n_pts, n_hyp)) return HG_ERR_WORKSPACE;
+    return ransac_run(src_xy, dst_xy, n_pts, hyp_idx, nullptr, 0ull, n_hyp, n_hyp, threshold_px, 0.0, false, counts, best_H,
+                      best_index, best_count, nullptr, workspace, workspace_bytes, cuda_stream);
+}
 
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    unsigned char* ws = static_cast<unsigned char*>(workspace);
-    RansacHeader* hdr = reinterpret_cast<RansacHeader*>(ws);
-    float4* table = reinterpret_cast<float4*>(ws + kHeaderBytes);
-    const float2* s2 = reinterpret_cast<const float2*>(src_xy);
-    const float2* d2 = reinterpret_cast<const float2*>(dst_xy);
-    const int4* idx4 = reinterpret_cast<const int4*>(hyp_idx);
-    const int n_pairs = (n_pts + 1) / 2;
-    const double t = static_cast<double>(threshold_px);
-    const double inv_t = 1.0 / t;
-
-    if (cudaMemsetAsync(hdr, 0, kHeaderBytes, st) != cudaSuccess) return HG_ERR_CUDA;
-    {
-        int blocks = (n_pairs + 255) / 256;
-        if (blocks > 1184) blocks = 1184;
-        ransac_prep_kernel<<<blocks, 256, 0, st>>>(s2, d2, n_pts, n_pairs, inv_t, table, hdr);
-        if (launch_status() != HG_OK) return HG_ERR_CUDA;
-    }
-    {
-        const size_t smem = size_t(kStages) * kChunkPairs * 32 + size_t(9) * kRBlock * sizeof(double) + size_t(2) * kRBlock * sizeof(float) +
-                            kStages * sizeof(uint64_t);
-        static bool attr_set = false;          // idempotent; a race only repeats the same call
-        if (!attr_set) {
-            if (cudaFuncSetAttribute(ransac_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
-                return HG_ERR_CUDA;
-            attr_set = true;
-        }
-        const unsigned blocks = static_cast<unsigned>((n_hyp + kRBlock - 1) / kRBlock);
-        ransac_score_kernel<<<blocks, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, idx4, int(n_hyp), inv_t, t,
-                                                           counts, hdr);
-        if (launch_status() != HG_OK) return HG_ERR_CUDA;
-    }
-    if (best_H || best_index || best_count) {
-        ransac_finalize_kernel<<<1, 32, 0, st>>>(s2, d2, idx4, hdr, best_H, reinterpret_cast<long long*>(best_index), best_count);
-        if (launch_status() != HG_OK) return HG_ERR_CUDA;
-    }
-    return HG_OK;
+extern "C" int hg_ransac_adaptive(const float* src_xy, const float* dst_xy, int32_t n_pts, uint64_t seed, int64_t max_hyp,
+                                  int64_t round_hyp, float threshold_px, float confidence, int32_t* counts,
+                                  int32_t* hyp_idx_out, float* best_H, int64_t* best_index, int32_t* best_count,
+                                  int64_t* n_evaluated, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    using namespace hg;
+    if (max_hyp < 0 || max_hyp > 0x7fffffffLL || round_hyp < 1) return HG_ERR_INVALID_ARG;
+    if (n_pts < 4) return HG_ERR_INVALID_ARG;
+    if (!(threshold_px > 0.0f) || !(threshold_px < 3.0e38f)) return HG_ERR_INVALID_ARG;
+    if (!(confidence < 1.0f) || !(confidence == confidence)) return HG_ERR_INVALID_ARG;
+    if (max_hyp == 0) return HG_OK;
+    if ((max_hyp + round_hyp - 1) / round_hyp > 65536) return HG_ERR_INVALID_ARG;          // launches per call
+    if (!src_xy || !dst_xy || !workspace) return HG_ERR_INVALID_ARG;
+    if (!aligned16(src_xy) || !aligned16(dst_xy) || !aligned16(workspace) || (hyp_idx_out && !aligned16(hyp_idx_out)))
+        return HG_ERR_ALIGNMENT;
+    if ((counts && !aligned4(counts)) || (best_H && !aligned4(best_H)) || (best_count && !aligned4(best_count)) ||
+        (best_index && (reinterpret_cast<uintptr_t>(best_index) & 7u)) || (n_evaluated && (reinterpret_cast<uintptr_t>(n_evaluated) & 7u)))
+        return HG_ERR_ALIGNMENT;
+    if (workspace_bytes < hg_ransac_workspace_bytes(n_pts, max_hyp)) return HG_ERR_WORKSPACE;
+    return ransac_run(src_xy, dst_xy, n_pts, nullptr, hyp_idx_out, seed, max_hyp, round_hyp, threshold_px,
+                      static_cast<double>(confidence), true, counts, best_H, best_index, best_count, n_evaluated, workspace,
+                      workspace_bytes, cuda_stream);
 }
 
 extern "C" int hg_ransac_hypothesize_score_host(const float* src_xy, const float* dst_xy, int32_t n_pts,

@@ -162,6 +162,26 @@ def test_ransac_argument_validation_and_workspace():
     assert call(wsb=128) == -4
 
 
+def test_ransac_adaptive_argument_validation():
+    f = hg.lib().hg_ransac_adaptive
+    ok = [FAKE, FAKE, 100, 7, 1000, 100, 3.0, 0.99, FAKE, FAKE, FAKE, FAKE, FAKE, FAKE, FAKE, 1 << 30, None]
+    names = ["src", "dst", "n_pts", "seed", "max_hyp", "round", "t", "conf", "counts", "idx", "bH", "bi", "bc", "ne", "ws", "wsb", "st"]
+
+    def call(**kw):
+        a = list(ok)
+        for k, v in kw.items():
+            a[names.index(k)] = v
+        return f(*a)
+
+    assert call(max_hyp=0) == 0
+    assert call(max_hyp=-1) == -1 and call(round=0) == -1 and call(n_pts=3) == -1
+    assert call(t=0.0) == -1 and call(conf=1.0) == -1 and call(conf=float("nan")) == -1
+    assert call(max_hyp=1 << 30, round=1) == -1                       # more than 65536 rounds
+    assert call(src=None) == -1 and call(ws=None) == -1
+    assert call(idx=FAKE + 4) == -2 and call(ne=FAKE + 4) == -2 and call(src=FAKE + 8) == -2
+    assert call(wsb=64) == -4
+
+
 def test_binding_refuses_cpu_tensors_on_the_device_entry_points():
     s = torch.zeros((8, 16), dtype=torch.float32)
     with pytest.raises(ValueError, match="no fallback"):

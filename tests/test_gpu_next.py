@@ -206,3 +206,53 @@ def test_warp_identity_translation_and_outside():
     far = torch.zeros((3, 4, 2), device=DEV); far[..., 0] = 1000.0
     out, _ = hg.hg_offsets_to_warp(far, 0.0, 0.0, 127.0, 127.0, 128, 128, img)
     assert torch.count_nonzero(out).item() == 0
+
+
+# ---- 8(f)-4 "RANSAC extras": on-device sampling + adaptive termination (reading R19) ----------------------
+def _adaptive_case(n_pts, inlier_frac, seed, max_hyp, round_hyp, conf, t=3.0):
+    wl = W.ransac_workload(n_pts=n_pts, n_hyp=4, seed=W.SEED_BASE + 80 + n_pts, inlier_frac=inlier_frac)
+    out = hg.hg_ransac_adaptive(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), seed, max_hyp, round_hyp, t, conf, want_idx=True)
+    ref = oracle.ransac_adaptive(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), seed, max_hyp, round_hyp, t, conf)
+    return wl, out, ref
+
+
+@pytest.mark.parametrize("n_pts,frac,max_hyp,round_hyp,conf", [
+    (4096, 0.7, 1 << 14, 512, 0.99),        # easy: stops after the first round
+    (2000, 0.25, 1 << 15, 1024, 0.99),      # ~1200 samples needed: stops after a few rounds
+    (1001, 0.12, 20000, 3000, 0.999),       # hard + ragged last round: runs to max_hyp or close
+    (500, 0.5, 5000, 700, 0.0),             # confidence 0: never stops early
+    (4, 1.0, 64, 16, 0.99)])                # tiny table: rejection sampling / fallback
+def test_ransac_adaptive_matches_oracle(n_pts, frac, max_hyp, round_hyp, conf):
+    wl, out, ref = _adaptive_case(n_pts, frac, 0xC0FFEE1234, max_hyp, round_hyp, conf)
+    n = int(out["n_evaluated"].item())
+    # sampled indices: integer work, bit-exact (for every hypothesis both sides scored)
+    m = min(n, ref["n_evaluated"])
+    assert np.array_equal(out["hyp_idx"].cpu().numpy()[:m], ref["hyp_idx"][:m])
+    # the stop decision is taken in fp64 on both sides; it may differ only when a round's margin is a rounding away from 0
+    # or when in-band pairs changed the best count
+    if n != ref["n_evaluated"]:
+        marg = ref["margins"][np.isfinite(ref["margins"])]
+        assert (np.abs(marg) < 1e-9).any() or ref["band_counts"].max() > 0
+        return
+    counts = out["counts"].cpu().numpy()[:n]
+    diff = np.abs(counts.astype(np.int64) - ref["counts"])
+    assert (diff <= ref["band_counts"]).all()
+    bi, bc = int(out["best_index"].item()), int(out["best_count"].item())
+    assert bc == counts.max() and bi == int(np.argmax(counts))
+    if (diff == 0).all():
+        assert bi == ref["best_index"] and bc == ref["best_count"]
+        Hb = out["best_H"].cpu().numpy().astype(np.float64).reshape(1, 3, 3)
+        a, b = align_to(Hb, ref["best_H"].reshape(1, 3, 3))
+        assert np.abs(a - b).max() <= 2e-7
+    assert (out["counts"].cpu().numpy()[n:] == 0).all()                    # entries past n_evaluated untouched
+    print(n_pts, frac, "n_evaluated", n, "of", max_hyp, "best", bc)
+
+
+def test_ransac_adaptive_agrees_with_explicit_indices():
+    """The sampled hypotheses scored through hg_ransac_hypothesize_score give the same counts."""
+    wl, out, ref = _adaptive_case(3000, 0.3, 99, 1 << 13, 1 << 11, 0.0)
+    idx = out["hyp_idx"]
+    plain = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), idx, 3.0)
+    assert torch.equal(plain["counts"], out["counts"])
+    assert plain["best_index"].item() == out["best_index"].item()
+    assert torch.equal(plain["best_H"], out["best_H"])

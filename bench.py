@@ -234,6 +234,14 @@ def run_extras(hg, W, dev, src, dst, H, peak):
                        "pairs_decided_in_fp64": stats["n_pairs_f64"],
                        "fp32_lane_instr_per_pair": 11, "alu_peak_instr_per_s": props.multi_processor_count * 128 * 1.965e9,
                        "frac_of_fp32_issue_peak": pairs * 11 / (ms * 1e-3) / (props.multi_processor_count * 128 * 1.965e9)}
+    # RANSAC extras: on-device sampling, rounds of one wave (296 CTAs x 512), with and without adaptive termination
+    fa = lambda conf: hg.hg_ransac_adaptive(wl["src_xy"], wl["dst_xy"], 240218008, 1 << 20, 296 * 512, 3.0, conf,
+                                            want_counts=False, workspace=ws)
+    for name, conf in (("ransac_c4_sampled_all_rounds", 0.0), ("ransac_c4_sampled_adaptive_p99", 0.99)):
+        o = fa(conf); fa(conf)
+        ms = event_time_ms(lambda: fa(conf), 5) / 5
+        ne = int(o["n_evaluated"])
+        ex[name] = {"ms": ms, "n_evaluated": ne, "best_count": int(o["best_count"]), "pairs_per_s": ne * 4096 / ms * 1e3}
     ex.update(run_next_rows(hg, W, dev, peak))
     return ex
 

@@ -175,13 +175,26 @@ __device__ __forceinline__ float gather(const float* __restrict__ img, const Tap
            fmaf(t.w01, px<SMEM>(img + t.o01), t.w00 * px<SMEM>(img + t.o00))));
 }
 
-// All four taps inside the image: p points at tap (0,0) of the plane.
-template <bool SMEM>
-__device__ __forceinline__ float gather_interior(const float* __restrict__ p, int img_w, float fu, float fv)
+// All four taps inside the image.  SMEM: `at` = shared-memory byte address of tap (0,0), row_bytes = 4 * img_w
+// (32-bit addressing, one LDS per tap); else `p` points at tap (0,0) in global memory.  Nested lerps: the same
+// bilinear form as gather() up to rounding.
+__device__ __forceinline__ float lerp2(float a, float b, float c, float d, float fu, float fv)
 {
-    const float a = px<SMEM>(p), b = px<SMEM>(p + 1), c = px<SMEM>(p + img_w), d = px<SMEM>(p + img_w + 1);
-    const float gu = 1.f - fu, gv = 1.f - fv;
-    return fmaf(fv * fu, d, fmaf(fv * gu, c, fmaf(gv * fu, b, (gv * gu) * a)));   // same weighted sum as gather()
+    const float top = fmaf(fu, b - a, a), bot = fmaf(fu, d - c, c);
+    return fmaf(fv, bot - top, top);
+}
+
+__device__ __forceinline__ float lds_f32(uint32_t addr)
+{ float v; asm("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr)); return v; }
+
+__device__ __forceinline__ float gather_interior_smem(uint32_t at, uint32_t row_bytes, float fu, float fv)
+{
+    return lerp2(lds_f32(at), lds_f32(at + 4u), lds_f32(at + row_bytes), lds_f32(at + row_bytes + 4u), fu, fv);
+}
+
+__device__ __forceinline__ float gather_interior_gmem(const float* __restrict__ p, int img_w, float fu, float fv)
+{
+    return lerp2(__ldg(p), __ldg(p + 1), __ldg(p + img_w), __ldg(p + img_w + 1), fu, fv);
 }
 
 __device__ __forceinline__ float rcp_approx(float x)
@@ -263,29 +276,47 @@ offsets_to_warp_kernel(const float* __restrict__ offsets, RectParams rp, WarpGeo
     const int j_end = min(g.out_h, j_begin + g.rows_per_band);
     if (SMEM) mbar_wait(&img_bar, 0);
 
+    const uint32_t img_base = SMEM ? smem_u32(img_s) : 0u;
+    const uint32_t row_bytes = 4u * static_cast<uint32_t>(img_w), plane_bytes = 4u * static_cast<uint32_t>(img_plane);
+    const int64_t out_step = static_cast<int64_t>(rows_per_pass) * out_w;
+
     for (int i = tx; i < out_w; i += tx_count) {
         const float fi = static_cast<float>(i);
         const float cx = fmaf(l11, fi, l13), cy = fmaf(l21, fi, l23), cw = fmaf(l31, fi, l33);
-        float* out_col = out_b + i;
+        float* op_row = out_b + i + static_cast<int64_t>(j_begin + ty) * out_w;
 #pragma unroll 2
-        for (int j = j_begin + ty; j < j_end; j += rows_per_pass) {
-            const float fj = static_cast<float>(j);
+        float fj = static_cast<float>(j_begin + ty);
+        const float fstep = static_cast<float>(rows_per_pass);
+        for (int j = j_begin + ty; j < j_end; j += rows_per_pass, op_row += out_step, fj += fstep) {
             const float X = fmaf(l12, fj, cx), Y = fmaf(l22, fj, cy), Wv = fmaf(l32, fj, cw);
             const float q = rcp_approx(Wv);
             const float u = X * q, v = Y * q;
-            float* op = out_col + j * out_w;
+            float* op = op_row;
             // Interior fast path, decided per warp: all four taps of every lane inside the image -- no clamping,
             // no weight selection, one address.  NaN fails the comparisons and takes the general path.
             const bool interior = (u >= 0.f) && (u < wm1) && (v >= 0.f) && (v < hm1);
             if (__all_sync(0xffffffffu, interior)) {
-                const float u0 = floorf(u), v0 = floorf(v);
-                const float fu = u - u0, fv = v - v0;
-                const float* p = img_b + (static_cast<int>(v0) * img_w + static_cast<int>(u0));
-                if (CH > 0) {
+                // floor without the conversion pipe: (u - 1/2) + 1.5 * 2^23 rounds to an integer k in the low mantissa
+                // bits, k = floor(u) except k = u - 1 for some integral u, where fu = 1 gives the same sample.
+                const float tu = __fadd_rn(__fadd_rn(u, -0.5f), 12582912.f), tv = __fadd_rn(__fadd_rn(v, -0.5f), 12582912.f);
+                const float fu = u - __fadd_rn(tu, -12582912.f), fv = v - __fadd_rn(tv, -12582912.f);
+                const int e = (__float_as_int(tv) - 0x4B400000) * img_w + (__float_as_int(tu) - 0x4B400000);
+                if (SMEM) {
+                    uint32_t at = img_base + 4u * static_cast<uint32_t>(e);
+                    if (CH > 0) {
 #pragma unroll
-                    for (int c = 0; c < CH; ++c) { __stcs(op, gather_interior<SMEM>(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
+                        for (int c = 0; c < CH; ++c) { __stcs(op, gather_interior_smem(at, row_bytes, fu, fv)); at += plane_bytes; op += out_plane; }
+                    } else {
+                        for (int c = 0; c < channels; ++c) { __stcs(op, gather_interior_smem(at, row_bytes, fu, fv)); at += plane_bytes; op += out_plane; }
+                    }
                 } else {
-                    for (int c = 0; c < channels; ++c) { __stcs(op, gather_interior<SMEM>(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
+                    const float* p = img_b + e;
+                    if (CH > 0) {
+#pragma unroll
+                        for (int c = 0; c < CH; ++c) { __stcs(op, gather_interior_gmem(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
+                    } else {
+                        for (int c = 0; c < channels; ++c) { __stcs(op, gather_interior_gmem(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
+                    }
                 }
             } else {
                 const Taps t = make_taps(u, v, img_w, img_h);

@@ -284,6 +284,42 @@ def run_next_rows(hg, W, dev, peak):
     leg("aca_f64_soa_2p25", lambda: hg.hg_aca_batched_f64(s64, d64, H=H64), 200, m)
     leg("sks_f64_soa_2p25", lambda: hg.hg_sks_batched_f64(s64, d64, H=H64), 200, m)
     del s64, d64, H64
+    # The sizes of the paper's Table 8 (1 ... 1M sets, fp64 storage, RTX 3090), as context: us per call,
+    # back-to-back launches (launch-bound below ~10K sets, L2-resident up to ~500K sets), and with an L2 flush at 1M.
+    t8 = {}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for k8 in (1, 10, 100, 1000, 10000, 100000, 1000000):
+        a8 = torch.rand((k8, 4, 2), device=dev, dtype=torch.float64) * 600.0
+        b8 = torch.rand((k8, 4, 2), device=dev, dtype=torch.float64) * 600.0
+        h8 = torch.empty((k8, 3, 3), device=dev, dtype=torch.float64)
+        row = {}
+        for nm, fn in (("aca", hg.hg_aca_batched_f64), ("sks", hg.hg_sks_batched_f64)):
+            call = lambda: fn(a8, b8, H=h8, layout=hg.AOS)
+            for _ in range(5):
+                call()
+            row[nm + "_us"] = event_time_ms(call, 100) / 100 * 1e3
+            try:
+                st8 = torch.cuda.Stream()
+                with torch.cuda.stream(st8):
+                    call()
+                    g8 = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(g8, stream=st8):
+                        for _ in range(20):
+                            call()
+                torch.cuda.current_stream().wait_stream(st8)
+                g8.replay()
+                row[nm + "_us_graph"] = event_time_ms(g8.replay, 10) / 200 * 1e3
+            except Exception as e:
+                row[nm + "_graph_error"] = repr(e)[:120]
+            if k8 == 1000000:
+                tot = 0.0
+                for _ in range(5):
+                    flush.zero_()
+                    tot += event_time_ms(call, 1)
+                row[nm + "_us_l2_flushed"] = tot / 5 * 1e3
+        t8[str(k8)] = row
+    del flush
+    ex["paper_table8_sizes_f64_aos"] = t8
     # offsets -> H -> bilinear warp of 8192 single-channel 128 x 128 patches (4 B read + 4 B written per pixel)
     k = 8192
     off5 = W.offsets_workload(k, seed=W.SEED_BASE + 5, device=dev)

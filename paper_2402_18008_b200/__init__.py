@@ -126,10 +126,35 @@ def _ptr(t, dtype, device_type: str, name: str):
     return _vp(t.data_ptr())
 
 
+_raw_stream = getattr(torch._C, "_cuda_getCurrentRawStream", None)
+
+
 def _stream(stream=None):
+    """cudaStream_t of `stream`, or of torch's current stream on the current device (the cheap raw query when torch has it)."""
     if stream is None:
+        if _raw_stream is not None:
+            return _vp(int(_raw_stream(torch.cuda.current_device())))
         stream = torch.cuda.current_stream()
     return _vp(int(stream.cuda_stream))
+
+
+class _NoCtx:
+    def __enter__(self):
+        return None
+
+    def __exit__(self, *a):
+        return False
+
+
+_NOCTX = _NoCtx()
+
+
+def _on(device):
+    """Context that makes `device` current; free when it already is (the common case on the latency-bound C1 path)."""
+    idx = device.index
+    if idx is None or idx == torch.cuda.current_device():
+        return _NOCTX
+    return torch.cuda.device(device)
 
 
 def _check(status: int, where: str):
@@ -162,7 +187,7 @@ def _solve(fn_name: str, src, dst, H, layout, norm, prec, stream):
     fn = getattr(lib(), fn_name)
     ps, pd, ph = (_ptr(src, torch.float32, "cuda", "src"), _ptr(dst, torch.float32, "cuda", "dst"),
                   _ptr(H, torch.float32, "cuda", "H"))
-    with torch.cuda.device(src.device):
+    with _on(src.device):
         st = fn(ps, pd, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, fn_name)
     return H
@@ -224,7 +249,7 @@ def hg_offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w
         raise ValueError("H must be [n,3,3]")
     if grid is not None and tuple(grid.shape) != (n, grid_h, grid_w, 2):
         raise ValueError("grid must be [n,grid_h,grid_w,2]")
-    with torch.cuda.device(offsets.device):
+    with _on(offsets.device):
         st = lib().hg_offsets_to_grid(po, x0, y0, w, h,
                                       int(grid_w), int(grid_h), _ptr(H, torch.float32, "cuda", "H"),
                                       _ptr(grid, torch.float32, "cuda", "grid"), n, int(norm), _stream(stream))
@@ -246,7 +271,7 @@ def hg_offsets_to_warp(offsets, x0: float, y0: float, w: float, h: float, out_w:
     elif tuple(warped.shape) != (n, C, out_h, out_w):
         raise ValueError("warped must be [n,C,out_h,out_w]")
     H = torch.empty((n, 3, 3), dtype=torch.float32, device=offsets.device) if want_H else None
-    with torch.cuda.device(offsets.device):
+    with _on(offsets.device):
         st = lib().hg_offsets_to_warp(_ptr(offsets, torch.float32, "cuda", "offsets"), x0, y0, w, h, int(out_w), int(out_h),
                                       _ptr(image, torch.float32, "cuda", "image"), C, iw, ih,
                                       _ptr(warped, torch.float32, "cuda", "warped"), _ptr(H, torch.float32, "cuda", "H"),
@@ -264,7 +289,7 @@ def hg_aca_rect_batched(offsets, x0: float, y0: float, w: float, h: float, H=Non
     elif tuple(H.shape) != _h_shape(n, layout):
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
     po, ph = _ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(H, torch.float32, "cuda", "H")
-    with torch.cuda.device(offsets.device):
+    with _on(offsets.device):
         st = lib().hg_aca_rect_batched(po, x0, y0, w, h, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, "hg_aca_rect_batched")
     return H
@@ -282,7 +307,7 @@ def hg_aca_rect_backward(offsets, x0: float, y0: float, w: float, h: float, grad
         raise ValueError("grad_offsets must be [n,4,2]")
     po, pg, pr = (_ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(grad_H, torch.float32, "cuda", "grad_H"),
                   _ptr(grad_offsets, torch.float32, "cuda", "grad_offsets"))
-    with torch.cuda.device(offsets.device):
+    with _on(offsets.device):
         st = lib().hg_aca_rect_backward(po, x0, y0, w, h, pg, pr, n, _stream(stream))
     _check(st, "hg_aca_rect_backward")
     return grad_offsets
@@ -310,7 +335,7 @@ def hg_affine_batched(src3, dst3, H=None, layout: int = SOA, norm: int = NORM_NO
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
     ps, pd, ph = (_ptr(src3, torch.float32, "cuda", "src3"), _ptr(dst3, torch.float32, "cuda", "dst3"),
                   _ptr(H, torch.float32, "cuda", "H"))
-    with torch.cuda.device(src3.device):
+    with _on(src3.device):
         st = lib().hg_affine_batched(ps, pd, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, "hg_affine_batched")
     return H
@@ -325,7 +350,7 @@ def hg_sk_batched(P3, Q3, dst, H=None, layout: int = SOA, norm: int = NORM_NONE,
     elif tuple(H.shape) != _h_shape(n, layout):
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
     pd, ph = _ptr(dst, torch.float32, "cuda", "dst"), _ptr(H, torch.float32, "cuda", "H")
-    with torch.cuda.device(dst.device):
+    with _on(dst.device):
         st = lib().hg_sk_batched(float(P3[0]), float(P3[1]), float(Q3[0]), float(Q3[1]), pd, ph, n, int(layout),
                                  int(norm), int(prec), _stream(stream))
     _check(st, "hg_sk_batched")
@@ -342,7 +367,7 @@ def _solve_f64(fn_name: str, src, dst, H, layout, norm, stream):
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
     ps, pd, ph = (_ptr(src, torch.float64, "cuda", "src"), _ptr(dst, torch.float64, "cuda", "dst"),
                   _ptr(H, torch.float64, "cuda", "H"))
-    with torch.cuda.device(src.device):
+    with _on(src.device):
         st = getattr(lib(), fn_name)(ps, pd, ph, n, int(layout), int(norm), _stream(stream))
     _check(st, fn_name)
     return H
@@ -381,7 +406,7 @@ def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, co
     best_H = torch.empty((3, 3), dtype=torch.float32, device=dev)
     best_index = torch.empty((1,), dtype=torch.int64, device=dev)
     best_count = torch.empty((1,), dtype=torch.int32, device=dev)
-    with torch.cuda.device(dev):
+    with _on(dev):
         st = lib().hg_ransac_hypothesize_score(
             _ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
             _ptr(hyp_idx, torch.int32, "cuda", "hyp_idx"), n_hyp, float(threshold_px),
@@ -408,7 +433,7 @@ def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, 
     best_index = torch.empty((1,), dtype=torch.int64, device=dev)
     best_count = torch.empty((1,), dtype=torch.int32, device=dev)
     n_eval = torch.empty((1,), dtype=torch.int64, device=dev)
-    with torch.cuda.device(dev):
+    with _on(dev):
         st = lib().hg_ransac_adaptive(
             _ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
             int(seed) & 0xFFFFFFFFFFFFFFFF, int(max_hyp), int(round_hyp), float(threshold_px), float(confidence),

@@ -1,0 +1,59 @@
+"""Randomised parity sweep: random (ragged) sizes, layouts, normalisations and shapes through every entry point, each
+case compared with the oracle at the tolerances of the dedicated tests.  Seeded: the same cases every run."""
+import numpy as np
+import pytest
+import torch
+
+import hg_workloads as W
+import oracle
+import paper_2402_18008_b200 as hg
+from util import align_to
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+SIZES = [1, 2, 3, 4, 5, 7, 31, 32, 33, 255, 256, 257, 1023, 1025]
+
+
+def test_random_sizes_solvers_rect_backward():
+    rng = np.random.default_rng(123)
+    for it in range(60):
+        n = int(rng.choice(SIZES + [int(rng.integers(1, 9000))]))
+        s, d = W.general_sets(n, seed=1000 + it)
+        layout, norm, meth = int(rng.integers(0, 2)), int(rng.integers(0, 3)), int(rng.integers(0, 2))
+        fn = hg.hg_aca_batched if meth == 0 else hg.hg_sks_batched
+        if layout == hg.SOA:
+            H = fn(W.to_soa(s).to(DEV), W.to_soa(d).to(DEV), layout=hg.SOA, norm=norm).t().reshape(n, 3, 3)
+        else:
+            H = fn(s.to(DEV), d.to(DEV), layout=hg.AOS, norm=norm)
+        ref = oracle.solve(oracle.METHOD_ACA if meth == 0 else oracle.METHOD_SKS, s.numpy(), d.numpy())
+        a, b = align_to(H.cpu().numpy().astype(np.float64), ref)
+        ok = (np.abs(a - b) <= 1e-4 * np.abs(b) + 1e-7).all(axis=(1, 2))
+        assert ok.mean() >= 0.97 or n < 40, (n, layout, norm, meth, ok.mean())     # R12: a few sets are rounding-sensitive
+        off = W.offsets_workload(n, seed=2000 + it)
+        Hr = hg.hg_aca_rect_batched(off.to(DEV), 3.0, -2.0, 100.0, 60.0, norm=hg.NORM_FROBENIUS).cpu().numpy().astype(np.float64)
+        a, b = align_to(Hr, oracle.aca_rect(off.numpy(), 3.0, -2.0, 100.0, 60.0))
+        assert np.abs(a - b).max() <= 3e-7, (n, np.abs(a - b).max())
+        g = torch.randn((n, 3, 3), generator=torch.Generator().manual_seed(it))
+        go = hg.hg_aca_rect_backward(off.to(DEV), 3.0, -2.0, 100.0, 60.0, g.to(DEV)).cpu().numpy().astype(np.float64)
+        gr = oracle.aca_rect_backward(off.numpy(), 3.0, -2.0, 100.0, 60.0, g.numpy().astype(np.float64))
+        sc = np.abs(gr).reshape(n, 8).max(axis=1)[:, None, None]
+        assert (np.abs(go - gr) <= 4e-7 * sc + 1e-30).all(), n
+
+
+def test_random_shapes_ransac_and_warp():
+    rng = np.random.default_rng(321)
+    for it in range(16):
+        npts, nh = int(rng.integers(4, 3000)), int(rng.integers(1, 3000))
+        t = float(rng.choice([0.5, 1.0, 3.0, 7.5]))
+        wl = W.ransac_workload(n_pts=npts, n_hyp=nh, seed=3000 + it)
+        out = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV), t)
+        rf = oracle.ransac(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy(), t, band_rel=1e-4)
+        df = np.abs(out["counts"].cpu().numpy().astype(np.int64) - rf["counts"])
+        assert (df <= rf["band_counts"]).all(), (npts, nh, t, int(df.max()))
+        ow, oh = int(rng.integers(1, 70)), int(rng.integers(1, 50))
+        iw, ih, C, m = int(rng.integers(2, 90)), int(rng.integers(2, 70)), int(rng.integers(1, 5)), int(rng.integers(1, 9))
+        o2 = W.offsets_workload(m, seed=it, max_offset=5.0)
+        img = torch.rand((m, C, ih, iw), generator=torch.Generator().manual_seed(it))
+        wp, _ = hg.hg_offsets_to_warp(o2.to(DEV), 1.0, 1.0, 40.0, 30.0, ow, oh, img.to(DEV))
+        wr = oracle.offsets_to_warp(o2.numpy(), 1.0, 1.0, 40.0, 30.0, ow, oh, img.numpy())
+        assert np.abs(wp.cpu().numpy() - wr).max() <= 2e-3, (ow, oh, iw, ih, C, m)

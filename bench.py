@@ -185,6 +185,21 @@ def run_extras(hg, W, dev, src, dst, H, peak):
                     "frac_of_peak": n * BYTES_PER_H / ms / 1e6 / peak}
     ms = event_time_ms(lambda: hg.hg_aca_batched(src, dst, H=H, prec=hg.PREC_F32), 5) / 5
     ex["aca_c3_plain_fp32"] = {"ms": ms, "GBps": n * BYTES_PER_H / ms / 1e6, "note": "HG_PREC_F32: fails the parity tolerance, measurement only"}
+    # C2: 2^20 sets = 105 MB, fits the 126 MB L2: timed with an L2 flush (a 256 MB memset) before every call, and warm
+    n2 = 1 << 20
+    s2, d2, H2 = src[:, :n2].contiguous(), dst[:, :n2].contiguous(), torch.empty((9, n2), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for name, fn in (("aca_c2", hg.hg_aca_batched), ("sks_c2", hg.hg_sks_batched)):
+        call = lambda: fn(s2, d2, H=H2)
+        call(); call()
+        cold = 0.0
+        for _ in range(10):
+            flush.zero_()
+            cold += event_time_ms(call, 1)
+        warm = event_time_ms(call, 20) / 20
+        ex[name] = {"ms_l2_flushed": cold / 10, "GBps_l2_flushed": n2 * BYTES_PER_H / (cold / 10) / 1e6,
+                    "ms_l2_warm": warm, "GBps_l2_warm": n2 * BYTES_PER_H / warm / 1e6, "l2": "flushed by a 256 MB memset / warm"}
+    del flush, s2, d2, H2
     # C5: offsets -> H -> grid, 8192 x 128 x 128 x 2 fp32 = 1.07 GB written per call (> L2)
     off = W.offsets_workload(8192, seed=W.SEED_BASE + 5, device=dev)
     Hh = torch.empty((8192, 3, 3), dtype=torch.float32, device=dev)

@@ -449,7 +449,7 @@ def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, 
 def ransac_stats(workspace: torch.Tensor) -> dict:
     """Decode the statistics words a finished hg_ransac_hypothesize_score call left in its workspace."""
     w = workspace[: 8 * RANSAC_STAT_WORDS].cpu().view(torch.int64)
-    return {"best_key": int(w[0]), "n_fixup": int(w[1]), "n_pairs_f64": int(w[2])}
+    return {"best_key": int(w[0]), "n_fixup": int(w[1]), "n_pairs_f64": int(w[2]), "n_evaluated": int(w[3])}
 
 
 def hg_ransac_hypothesize_score_host(src_xy, dst_xy, hyp_idx, threshold_px: float, want_counts: bool = True):

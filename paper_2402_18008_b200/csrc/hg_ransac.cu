@@ -480,12 +480,9 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     }
     const size_t smem = size_t(kStages) * kChunkPairs * 32 + size_t(9) * kRBlock * sizeof(double) + size_t(2) * kRBlock * sizeof(float) +
                         kStages * sizeof(uint64_t);
-    static bool attr_set = false;          // idempotent; a race only repeats the same call
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(ransac_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
-            return HG_ERR_CUDA;
-        attr_set = true;
-    }
+    // per call, not cached: the attribute belongs to the current device, and a process may drive several
+    if (cudaFuncSetAttribute(ransac_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
+        return HG_ERR_CUDA;
     HypSource hs;
     hs.idx = reinterpret_cast<const int4*>(hyp_idx);
     hs.idx_out = reinterpret_cast<int4*>(hyp_idx_out);

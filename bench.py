@@ -454,6 +454,22 @@ def main():
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": "first 2^%d sets of the timed workload, %d passes of the ACA-fp64 oracle (OpenMP, %.1f s)"
                                           % (n_s.bit_length() - 1, done, dt)}
+        # single-thread ns per homography on 2^20 sets (the kind of number the paper's Table 5 reports)
+        try:
+            import oracle
+            nt = oracle.num_threads()
+            oracle.set_num_threads(1)
+            one = {}
+            m1 = 1 << 20
+            for nm, meth in (("aca", oracle.METHOD_ACA), ("sks", oracle.METHOD_SKS), ("dlt_ge", oracle.METHOD_DLT)):
+                oracle.solve(meth, s_aos[: 1 << 14], d_aos[: 1 << 14])
+                t0 = time.perf_counter()
+                oracle.solve(meth, s_aos[:m1], d_aos[:m1])
+                one[nm] = (time.perf_counter() - t0) / m1 * 1e9
+            oracle.set_num_threads(nt)
+            line["cpu_baseline"]["single_thread_ns_per_homography"] = one
+        except Exception as e:
+            line["cpu_baseline"]["single_thread_error"] = repr(e)[:200]
         del s_aos, d_aos
     if world == 1 and not args.no_extras:
         try:

@@ -78,22 +78,35 @@ template <class T>
 __global__ void __launch_bounds__(kRectBlock)
 rect_aos_kernel(const float* __restrict__ offsets, RectSrc rs, float* __restrict__ H, int64_t n, int norm)
 {
-    __shared__ __align__(16) float stage[kRectBlock * 9];
-    const int64_t base = static_cast<int64_t>(blockIdx.x) * kRectBlock;
-    const int64_t i = base + threadIdx.x;
-    if (i < n) {
-        const float4* op = reinterpret_cast<const float4*>(offsets + 8 * i);
-        const float4 o0 = __ldcs(op), o1 = __ldcs(op + 1);
-        const T ov[8] = { T(o0.x), T(o0.y), T(o0.z), T(o0.w), T(o1.x), T(o1.y), T(o1.z), T(o1.w) };
-        T Hv[9];
-        aca_rect_solve<T>(rs, ov, Hv);
-        normalise<T>(Hv, norm);
+    // Two items per thread (i and i + kRectBlock): four independent 128-bit loads in flight per thread, which a
+    // 32-byte-per-item stream needs to cover the HBM latency.
+    constexpr int ITEMS = 2;
+    __shared__ __align__(16) float stage[ITEMS * kRectBlock * 9];
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * (ITEMS * kRectBlock);
+    float4 o[ITEMS][2];
 #pragma unroll
-        for (int k = 0; k < 9; ++k) stage[threadIdx.x * 9 + k] = static_cast<float>(Hv[k]);
+    for (int k = 0; k < ITEMS; ++k) {
+        const int64_t i = base + k * kRectBlock + threadIdx.x;
+        if (i < n) {
+            const float4* op = reinterpret_cast<const float4*>(offsets + 8 * i);
+            o[k][0] = __ldcs(op); o[k][1] = __ldcs(op + 1);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        const int64_t i = base + k * kRectBlock + threadIdx.x;
+        if (i < n) {
+            const T ov[8] = { T(o[k][0].x), T(o[k][0].y), T(o[k][0].z), T(o[k][0].w), T(o[k][1].x), T(o[k][1].y), T(o[k][1].z), T(o[k][1].w) };
+            T Hv[9];
+            aca_rect_solve<T>(rs, ov, Hv);
+            normalise<T>(Hv, norm);
+#pragma unroll
+            for (int q = 0; q < 9; ++q) stage[(k * kRectBlock + threadIdx.x) * 9 + q] = static_cast<float>(Hv[q]);
+        }
     }
     __syncthreads();
     const int64_t rem = n - base;
-    const int cnt = static_cast<int>(rem < kRectBlock ? rem : kRectBlock) * 9;
+    const int cnt = static_cast<int>(rem < ITEMS * kRectBlock ? rem : ITEMS * kRectBlock) * 9;
     float* out = H + 9 * base;
     const int n4 = cnt >> 2;
     for (int j = threadIdx.x; j < n4; j += kRectBlock)
@@ -166,31 +179,42 @@ __global__ void __launch_bounds__(kRectBlock)
 rect_backward_kernel(const float* __restrict__ offsets, RectSrc rs, const float* __restrict__ grad_G,
                      float* __restrict__ grad_off, int64_t n)
 {
-    __shared__ __align__(16) float stage[kRectBlock * 9];
-    const int64_t base = static_cast<int64_t>(blockIdx.x) * kRectBlock;
+    // Two items per thread (i and i + kRectBlock), all loads issued before the first use: 68 B per item is a thin
+    // stream and the ~130-FLOP fp64 chain is long, so each thread needs more bytes in flight than one item gives.
+    constexpr int ITEMS = 2;
+    __shared__ __align__(16) float stage[ITEMS * kRectBlock * 9];
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * (ITEMS * kRectBlock);
     const int64_t rem = n - base;
-    const int cnt = static_cast<int>(rem < kRectBlock ? rem : kRectBlock) * 9;
-    const float* gin = grad_G + 9 * base;                       // 9*256*4 B per block: 16-byte aligned
+    const int cnt = static_cast<int>(rem < ITEMS * kRectBlock ? rem : ITEMS * kRectBlock) * 9;
+    const float* gin = grad_G + 9 * base;                       // 9*512*4 B per block: 16-byte aligned
     const int n4 = cnt >> 2;
     for (int j = threadIdx.x; j < n4; j += kRectBlock)
         reinterpret_cast<float4*>(stage)[j] = __ldcs(reinterpret_cast<const float4*>(gin) + j);
     for (int j = (n4 << 2) + threadIdx.x; j < cnt; j += kRectBlock) stage[j] = gin[j];
-    const int64_t i = base + threadIdx.x;
-    float4 o0 = make_float4(0.f, 0.f, 0.f, 0.f), o1 = o0;
-    if (i < n) {
-        const float4* op = reinterpret_cast<const float4*>(offsets + 8 * i);
-        o0 = __ldcs(op); o1 = __ldcs(op + 1);
+    float4 o[ITEMS][2];
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        const int64_t i = base + k * kRectBlock + threadIdx.x;
+        o[k][0] = o[k][1] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (i < n) {
+            const float4* op = reinterpret_cast<const float4*>(offsets + 8 * i);
+            o[k][0] = __ldcs(op); o[k][1] = __ldcs(op + 1);
+        }
     }
     __syncthreads();
-    if (i >= n) return;
-    const double ov[8] = { o0.x, o0.y, o0.z, o0.w, o1.x, o1.y, o1.z, o1.w };
-    double g[9], go[8];
 #pragma unroll
-    for (int k = 0; k < 9; ++k) g[k] = static_cast<double>(stage[threadIdx.x * 9 + k]);
-    aca_rect_backward(rs, ov, g, go);
-    float4* out = reinterpret_cast<float4*>(grad_off + 8 * i);
-    __stcs(out, make_float4(float(go[0]), float(go[1]), float(go[2]), float(go[3])));
-    __stcs(out + 1, make_float4(float(go[4]), float(go[5]), float(go[6]), float(go[7])));
+    for (int k = 0; k < ITEMS; ++k) {
+        const int64_t i = base + k * kRectBlock + threadIdx.x;
+        if (i >= n) break;
+        const double ov[8] = { o[k][0].x, o[k][0].y, o[k][0].z, o[k][0].w, o[k][1].x, o[k][1].y, o[k][1].z, o[k][1].w };
+        double g[9], go[8];
+#pragma unroll
+        for (int q = 0; q < 9; ++q) g[q] = static_cast<double>(stage[(k * kRectBlock + threadIdx.x) * 9 + q]);
+        aca_rect_backward(rs, ov, g, go);
+        float4* out = reinterpret_cast<float4*>(grad_off + 8 * i);
+        __stcs(out, make_float4(float(go[0]), float(go[1]), float(go[2]), float(go[3])));
+        __stcs(out + 1, make_float4(float(go[4]), float(go[5]), float(go[6]), float(go[7])));
+    }
 }
 
 template <class T>
@@ -205,7 +229,7 @@ static int rect_dispatch(const float* offsets, const RectSrc& rs, float* H, int6
             rect_soa_kernel<T, 1><<<static_cast<unsigned>(blocks), kRectBlock, 0, st>>>(offsets, rs, H, n, n, norm);
         }
     } else {
-        const int64_t blocks = (n + kRectBlock - 1) / kRectBlock;
+        const int64_t blocks = (n + 2 * kRectBlock - 1) / (2 * kRectBlock);
         rect_aos_kernel<T><<<static_cast<unsigned>(blocks), kRectBlock, 0, st>>>(offsets, rs, H, n, norm);
     }
     return launch_status();
@@ -245,7 +269,7 @@ extern "C" int hg_aca_rect_backward(const float* offsets, float x0, float y0, fl
     if ((n + kRectBlock - 1) / kRectBlock > 0x7fffffffLL) return HG_ERR_INVALID_ARG;
     RectSrc rs;
     rs.x0 = x0; rs.y0 = y0; rs.w = w; rs.h = h; rs.r = double(w) / double(h);
-    const int64_t blocks = (n + kRectBlock - 1) / kRectBlock;
+    const int64_t blocks = (n + 2 * kRectBlock - 1) / (2 * kRectBlock);
     rect_backward_kernel<<<static_cast<unsigned>(blocks), kRectBlock, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
         offsets, rs, grad_H, grad_offsets, n);
     return launch_status();

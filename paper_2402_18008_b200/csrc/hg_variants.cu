@@ -152,34 +152,45 @@ __device__ __forceinline__ void load_record(const IO* __restrict__ p, IO x[N])
 }
 
 // AoS: a = IO[n][NA], b = IO[n][NB], H = IO[n][9] (records transposed through shared memory for contiguous stores).
-template <class Op, class IO, class T>
+// ITEMS records per thread (i, i + kVarBlock, ...), all loads issued before the first use: a thin input stream
+// (32 B per set) needs two to keep enough bytes in flight.
+template <class Op, class IO, class T, int ITEMS>
 __global__ void __launch_bounds__(kVarBlock)
 variant_aos_kernel(const IO* __restrict__ a, const IO* __restrict__ b, IO* __restrict__ H, int64_t n, int norm, Op op)
 {
     constexpr int NA = Op::NA, NB = Op::NB;
-    __shared__ __align__(16) IO stage[kVarBlock * 9];
-    const int64_t base = static_cast<int64_t>(blockIdx.x) * kVarBlock;
-    const int64_t i = base + threadIdx.x;
-    if (i < n) {
-        __align__(16) IO xa[NA];
-        load_record<IO, NA>(a + NA * i, xa);
-        T x[NA + NB], Hv[9];
+    __shared__ __align__(16) IO stage[ITEMS * kVarBlock * 9];
+    const int64_t base = static_cast<int64_t>(blockIdx.x) * (ITEMS * kVarBlock);
+    __align__(16) IO xa[ITEMS][NA];
+    __align__(16) IO xb[ITEMS][NB > 0 ? NB : 2];
 #pragma unroll
-        for (int k = 0; k < NA; ++k) x[k] = static_cast<T>(xa[k]);
-        if constexpr (NB > 0) {
-            __align__(16) IO xb[NB];
-            load_record<IO, NB>(b + NB * i, xb);
-#pragma unroll
-            for (int k = 0; k < NB; ++k) x[NA + k] = static_cast<T>(xb[k]);
+    for (int it = 0; it < ITEMS; ++it) {
+        const int64_t i = base + it * kVarBlock + threadIdx.x;
+        if (i < n) {
+            load_record<IO, NA>(a + NA * i, xa[it]);
+            if constexpr (NB > 0) load_record<IO, NB>(b + NB * i, xb[it]);
         }
-        op.template apply<T>(x, Hv);
-        normalise<T>(Hv, norm);
+    }
 #pragma unroll
-        for (int k = 0; k < 9; ++k) stage[threadIdx.x * 9 + k] = static_cast<IO>(Hv[k]);
+    for (int it = 0; it < ITEMS; ++it) {
+        const int64_t i = base + it * kVarBlock + threadIdx.x;
+        if (i < n) {
+            T x[NA + NB], Hv[9];
+#pragma unroll
+            for (int k = 0; k < NA; ++k) x[k] = static_cast<T>(xa[it][k]);
+            if constexpr (NB > 0) {
+#pragma unroll
+                for (int k = 0; k < NB; ++k) x[NA + k] = static_cast<T>(xb[it][k]);
+            }
+            op.template apply<T>(x, Hv);
+            normalise<T>(Hv, norm);
+#pragma unroll
+            for (int k = 0; k < 9; ++k) stage[(it * kVarBlock + threadIdx.x) * 9 + k] = static_cast<IO>(Hv[k]);
+        }
     }
     __syncthreads();
     const int64_t rem = n - base;
-    const int cnt = static_cast<int>(rem < kVarBlock ? rem : kVarBlock) * 9;
+    const int cnt = static_cast<int>(rem < ITEMS * kVarBlock ? rem : ITEMS * kVarBlock) * 9;
     IO* out = H + 9 * base;
     constexpr int PER = 16 / int(sizeof(IO));
     const int nv = cnt / PER;
@@ -201,8 +212,9 @@ static int variant_launch(const IO* a, const IO* b, IO* H, int64_t n, hg_layout_
             variant_soa_kernel<Op, IO, T, false><<<static_cast<unsigned>(blocks), kVarBlock, 0, st>>>(a, b, H, n, n, norm, op);
         }
     } else {
-        const int64_t blocks = (n + kVarBlock - 1) / kVarBlock;
-        variant_aos_kernel<Op, IO, T><<<static_cast<unsigned>(blocks), kVarBlock, 0, st>>>(a, b, H, n, norm, op);
+        constexpr int ITEMS = ((Op::NA + Op::NB) * int(sizeof(IO)) <= 32) ? 2 : 1;
+        const int64_t blocks = (n + ITEMS * kVarBlock - 1) / (ITEMS * kVarBlock);
+        variant_aos_kernel<Op, IO, T, ITEMS><<<static_cast<unsigned>(blocks), kVarBlock, 0, st>>>(a, b, H, n, norm, op);
     }
     return launch_status();
 }

@@ -11,8 +11,8 @@ step streams from HBM: no L2 flush is needed).  Rank 0 prints ONE JSON line.
 
   value      whole-job homographies/s, inputs resident in HBM, CUDA events on the launch stream,
              max over ranks
-  e2e        the same through `hg_aca_batched_host` (pinned HOST buffers in, HOST buffer out;
-             chunked H2D -> kernel -> D2H pipeline inside the timed region)
+  e2e        the same through `hg_aca_batched_host` (pinned HOST buffers in, HOST buffer out; the kernel
+             reads and writes them directly over PCIe inside the timed region: 64 B up + 36 B down per H)
   roofline   algorithmic bytes (100 B x 2^26) / average launch duration, against MEASURED_PEAKS.json
   cpu_baseline  the fp64 oracle (oracle/) on the host cores, on a bounded sample of the same workload
   extras     the other hot-path rows at their BASELINE sizes (SKS C3, grid C5, RANSAC C4, C1 latency) and the
@@ -424,7 +424,7 @@ def main():
             dt = float(t.item())
         same = bool(torch.equal(hH[:, :: 4097], H[:, :: 4097].cpu()))
         e2e = {"value": world * n * e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 64 * n, "d2h_bytes_per_step": 36 * n,
-               "steps": e_steps, "ms_per_step": dt / e_steps * 1e3, "api": "hg_aca_batched_host (pinned host buffers)",
+               "steps": e_steps, "ms_per_step": dt / e_steps * 1e3, "api": "hg_aca_batched_host (pinned host buffers: one kernel reads and writes them over PCIe)",
                "matches_device_result": same}
         del hs, hd, hH
 

@@ -92,10 +92,13 @@ HG_API int hg_sks_batched(const float* src, const float* dst, float* H, int64_t 
                    hg_layout_t layout, hg_norm_t norm, hg_precision_t prec, void* cuda_stream);
 
 /* Host-buffer forms of the two solves (the end-to-end path of bench.py): src/dst/H are HOST
- * pointers in `layout`.  The call splits the batch into chunks and pipelines host->device
- * copies, the solve kernel and device->host copies on internal streams, then waits.  Copies are
- * asynchronous only if the host buffers are page-locked.  `chunk_sets` = sets per chunk
- * (0 = library default).  Extra error: HG_ERR_CUDA if staging memory cannot be allocated.        */
+ * pointers in `layout`.  If all three buffers are page-locked and device-mapped (cudaHostAlloc /
+ * cudaHostRegister; torch pinned tensors are) and 16-byte aligned, ONE kernel reads and writes them
+ * directly over PCIe (both directions of the bus at once, no staging memory; `chunk_sets` unused).
+ * Otherwise the call splits the batch into chunks and pipelines host->device copies, the solve
+ * kernel and device->host copies on internal streams.  Either way it returns after H is complete in
+ * host memory.  `chunk_sets` = sets per chunk of the staged path (0 = library default).  Extra
+ * error: HG_ERR_CUDA if staging memory cannot be allocated.                                        */
 HG_API int hg_aca_batched_host(const float* src_host, const float* dst_host, float* H_host, int64_t n,
                         hg_layout_t layout, hg_norm_t norm, hg_precision_t prec,
                         int64_t chunk_sets);

@@ -137,10 +137,20 @@ int solve_batched(int method, const float* src, const float* dst, float* H, int6
 }
 
 // ------------------------------------------------------------------------------------------
-// Host-buffer pipeline: chunked H2D -> solve -> D2H on kStreams streams (copy engines in both
-// directions overlap the kernel).  SoA chunks are strided in host memory (8 or 9 planes of
+// Host-buffer entry points.  Page-locked buffers: zero-copy (below).  Pageable buffers: chunked
+// H2D -> solve -> D2H on kStreams streams (copy engines in both directions overlap the kernel).  SoA chunks are strided in host memory (8 or 9 planes of
 // `n` floats): cudaMemcpy2DAsync moves them into chunk-local device planes.
 // ------------------------------------------------------------------------------------------
+// Device-visible alias of a page-locked host pointer, if it is one.
+static bool mapped_host_pointer(const void* host, void** dev)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, host) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (a.type != cudaMemoryTypeHost || a.devicePointer == nullptr) return false;
+    *dev = a.devicePointer;
+    return true;
+}
+
 static int solve_batched_host(int method, const float* src, const float* dst, float* H, int64_t n,
                               hg_layout_t layout, hg_norm_t norm, hg_precision_t prec, int64_t chunk)
 {
@@ -150,6 +160,26 @@ static int solve_batched_host(int method, const float* src, const float* dst, fl
     if (prec != HG_PREC_F64 && prec != HG_PREC_F32) return HG_ERR_INVALID_ARG;
     if (n == 0) return HG_OK;
     if (!src || !dst || !H) return HG_ERR_INVALID_ARG;
+    // Page-locked, device-mapped host buffers (cudaHostAlloc / cudaHostRegister, e.g. torch pinned tensors): the kernel
+    // reads and writes them directly over PCIe -- one launch, both directions of the bus busy at once, no staging
+    // memory.  Measured equal to the best of the staged pipeline (PCIe-bound) and steadier.  chunk_sets is ignored.
+    {
+        void *ds = nullptr, *dd = nullptr, *dh = nullptr;
+        if (mapped_host_pointer(src, &ds) && mapped_host_pointer(dst, &dd) && mapped_host_pointer(H, &dh) &&
+            aligned16(ds) && aligned16(dd) && aligned16(dh)) {
+            cudaStream_t zs = nullptr;
+            int rc = cuda_status(cudaStreamCreateWithFlags(&zs, cudaStreamNonBlocking));
+            if (rc == HG_OK)
+                rc = solve_batched(method, static_cast<const float*>(ds), static_cast<const float*>(dd), static_cast<float*>(dh),
+                                   n, n, layout, norm, prec, zs);
+            if (zs) {
+                const int r2 = cuda_status(cudaStreamSynchronize(zs));
+                if (rc == HG_OK) rc = r2;
+                cudaStreamDestroy(zs);
+            }
+            return rc;
+        }
+    }
     if (chunk == 0) chunk = int64_t(1) << 21;            // 2 Mi sets: 128 MiB in, 72 MiB out per chunk
     chunk = (chunk + 3) & ~int64_t(3);
     if (chunk > n) chunk = n;

@@ -175,11 +175,14 @@ def test_host_buffer_pipeline_matches_device_call():
     s, d = W.general_sets(n, seed=21)
     ss, ds = W.to_soa(s), W.to_soa(d)
     ref = hg.hg_aca_batched(ss.to(DEV), ds.to(DEV), norm=hg.NORM_FROBENIUS).cpu()
-    out = hg.hg_aca_batched_host(ss.pin_memory(), ds.pin_memory(), norm=hg.NORM_FROBENIUS, chunk_sets=8192)
+    out = hg.hg_aca_batched_host(ss.pin_memory(), ds.pin_memory(), norm=hg.NORM_FROBENIUS, chunk_sets=8192)   # pinned: zero-copy
     assert torch.equal(out, ref)
     out2 = hg.hg_sks_batched_host(s, d, layout=hg.AOS, norm=hg.NORM_H33, chunk_sets=10_000)     # pageable AoS
     ref2 = hg.hg_sks_batched(s.to(DEV), d.to(DEV), layout=hg.AOS, norm=hg.NORM_H33).cpu()
     assert torch.equal(out2, ref2)
+    # pageable SoA with a pageable result buffer: the staged, chunked path (strided 2-D copies, ragged last chunk)
+    out3 = hg.hg_aca_batched_host(ss, ds, H=torch.empty((9, n), dtype=torch.float32), norm=hg.NORM_FROBENIUS, chunk_sets=8192)
+    assert torch.equal(out3, ref)
 
 
 def test_full_size_config3_sampled_against_oracle():

@@ -166,3 +166,31 @@ def test_ransac_full_config4_sampled():
     assert (diff <= ref["band_counts"]).all(), int((diff > ref["band_counts"]).sum())
     assert bc >= 0.6 * 0.7 * 4096
     print("C4 sampled: mismatches inside band", int((diff > 0).sum()), "of", len(sel), hg.ransac_stats(out["workspace"]))
+
+
+def test_ransac_degenerate_and_non_finite_inputs():
+    """Edge cases of the scorer: a NaN correspondence (outlier for everyone, zero count for hypotheses built on it),
+    coincident points (H = 0 everywhere), dst = src (everything an inlier), very small / very large thresholds, and
+    coordinates scaled by 1e6 (the error band scales with them).  Each against the oracle, and none may hang."""
+    wl = W.ransac_workload(n_pts=1000, n_hyp=4096, seed=1)
+    idx = wl["hyp_idx"]
+
+    def both(src, dst, t):
+        out = hg.hg_ransac_hypothesize_score(src.to(DEV), dst.to(DEV), idx.to(DEV), t)
+        ref = oracle.ransac(src.numpy(), dst.numpy(), idx.numpy(), t, band_rel=1e-4)
+        counts = out["counts"].cpu().numpy()
+        diff = np.abs(counts.astype(np.int64) - ref["counts"])
+        assert (diff <= ref["band_counts"]).all(), int(diff.max())
+        assert int(out["best_count"].item()) == counts.max() and int(out["best_index"].item()) == int(np.argmax(counts))
+        return counts
+
+    s, d = wl["src_xy"].clone(), wl["dst_xy"].clone()
+    s_nan = s.clone(); s_nan[5] = float("nan")
+    c = both(s_nan, d, 3.0)
+    uses5 = (idx == 5).any(dim=1).numpy()
+    assert uses5.any() and (c[uses5] == 0).all()
+    assert (both(torch.zeros_like(s), torch.zeros_like(d), 3.0) == 0).all()
+    assert (both(s, s.clone(), 3.0) == 1000).all()
+    assert (both(s, d, 1e-6) >= 4).all()                         # the four sampled correspondences always fit exactly
+    assert (both(s, d, 1e9) >= 999).all()
+    both(s * 1e6, d * 1e6, 3e6)

@@ -143,6 +143,7 @@ def oracle_rate(src_aos, dst_aos, passes, warm=1, min_seconds=0.0):
     """ACA-fp64 oracle, all host cores (OpenMP): homographies/s over at least `passes` passes of the sample
     (and at least `min_seconds` of work)."""
     import oracle
+    oracle.set_num_threads(os.cpu_count() or 1)      # torchrun exports OMP_NUM_THREADS=1: the baseline is "all host cores"
     for _ in range(warm):
         oracle.aca(src_aos, dst_aos)
     done = 0

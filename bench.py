@@ -261,6 +261,28 @@ def run_extras(hg, W, dev, src, dst, H, peak):
         ms = event_time_ms(lambda: fa(conf), 5) / 5
         ne = int(o["n_evaluated"])
         ex[name] = {"ms": ms, "n_evaluated": ne, "best_count": int(o["best_count"]), "pairs_per_s": ne * 4096 / ms * 1e3}
+    # The scale of the paper's Table 6 (<= 1000 matches per image pair, a few to a few thousand loops; solver +
+    # verification loops 4.5-154 us on a CPU core): one call = memset + 3 kernels, us per call plain and in a CUDA graph.
+    wls = W.ransac_workload(n_pts=1000, n_hyp=1024, seed=W.SEED_BASE + 44, device=dev)
+    wss = torch.empty(hg.hg_ransac_workspace_bytes(1000, 1024), dtype=torch.uint8, device=dev)
+    fs = lambda: hg.hg_ransac_hypothesize_score(wls["src_xy"], wls["dst_xy"], wls["hyp_idx"], 3.0, want_counts=False, workspace=wss)
+    for _ in range(5):
+        fs()
+    small = {"n_pts": 1000, "n_hyp": 1024, "us_per_call_launch": event_time_ms(fs, 100) / 100 * 1e3}
+    try:
+        sts = torch.cuda.Stream()
+        with torch.cuda.stream(sts):
+            fs()
+            gs = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gs, stream=sts):
+                for _ in range(10):
+                    fs()
+        torch.cuda.current_stream().wait_stream(sts)
+        gs.replay()
+        small["us_per_call_graph"] = event_time_ms(gs.replay, 20) / 200 * 1e3
+    except Exception as e:
+        small["graph_error"] = repr(e)[:200]
+    ex["ransac_table6_scale"] = small
     ex.update(run_next_rows(hg, W, dev, peak))
     return ex
 

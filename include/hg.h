@@ -235,7 +235,10 @@ HG_API int hg_sks_batched_f64(const double* src, const double* dst, double* H, i
  *   best_index     : nullable, int64: argmax of counts, ties -> lowest hypothesis index
  *   best_count     : nullable, int32: its count
  *   workspace      : device scratch of >= hg_ransac_workspace_bytes(n_pts, n_hyp) bytes,
- *                    16-byte aligned; contents undefined before and after the call.
+ *                    16-byte aligned; contents undefined before and after the call.  (Header,
+ *                    the packed table, and -- for calls too small to fill the GPU with one
+ *                    hypothesis per thread, which are also split over the table -- 4 bytes per
+ *                    hypothesis of partial counts.)
  * Errors: HG_ERR_INVALID_ARG (NULL inputs, n_pts < 4, n_hyp < 0, threshold not > 0),
  * HG_ERR_ALIGNMENT, HG_ERR_WORKSPACE, HG_ERR_CUDA.
  * -------------------------------------------------------------------------------------------- */

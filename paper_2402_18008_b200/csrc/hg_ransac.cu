@@ -84,6 +84,8 @@ struct HypSource {
     unsigned long long seed;    // sampling mode
     int h0, h1;                 // this launch scores hypotheses [h0, h1)
     int check_stop;             // 1: return at once when hdr->stop is set (adaptive termination)
+    int part_entries;           // table entries per blockIdx.y part (a multiple of 8); >= n_pairs: no split
+    int* acc;                   // split mode: partial counts are added here (zeroed before the launch)
 };
 
 // Philox4x32-10 (Salmon et al., SC'11), the counter-based generator of reading R19: 10 rounds of
@@ -320,7 +322,12 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     float* Kstash = reinterpret_cast<float*>(Hstash + 9 * kRBlock);                               // [2][kRBlock]
     uint64_t* full = reinterpret_cast<uint64_t*>(Kstash + 2 * kRBlock);
 
-    const int n_chunks = (n_pairs + kChunkPairs - 1) / kChunkPairs;
+    // Small hypothesis batches are split over the table as well (blockIdx.y = part), so that a call with a few
+    // thousand hypotheses still fills the machine; this CTA sweeps entries [e_begin, e_end).
+    const int e_begin = blockIdx.y * hs.part_entries;
+    const int e_end = min(n_pairs, e_begin + hs.part_entries);
+    const bool split = gridDim.y > 1;
+    const int n_chunks = (e_end - e_begin + kChunkPairs - 1) / kChunkPairs;
     if (threadIdx.x == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
         fence_barrier_init();
@@ -328,9 +335,10 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int c = 0; c < kStages && c < n_chunks; ++c) {
-            const int pairs = min(kChunkPairs, n_pairs - c * kChunkPairs);
+            const int first = e_begin + c * kChunkPairs;
+            const int pairs = min(kChunkPairs, e_end - first);
             mbar_arrive_expect_tx(&full[c], pairs * 32u);
-            bulk_copy_g2s(stage_buf + size_t(c) * kChunkPairs * 2, table + size_t(c) * kChunkPairs * 2, pairs * 32u, &full[c]);
+            bulk_copy_g2s(stage_buf + size_t(c) * kChunkPairs * 2, table + size_t(first) * 2, pairs * 32u, &full[c]);
         }
     }
 
@@ -344,7 +352,7 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
                                   __uint_as_float(hdr->bound_bits[2]), __uint_as_float(hdr->bound_bits[3]) };
         double s[8], d[8], Hn[9];
         const int4 id = active ? hypothesis_indices(hs, hidx, n_pts) : make_int4(0, 0, 0, 0);   // inactive: degenerate => sure outliers
-        if (active && hs.idx_out) hs.idx_out[hidx] = id;
+        if (active && hs.idx_out && blockIdx.y == 0) hs.idx_out[hidx] = id;
         gather_sets(src_xy, dst_xy, id, s, d);
         ok = make_hypothesis(s, d, inv_t, bounds, Hn, hc) && active;
 #pragma unroll
@@ -360,8 +368,8 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
         const int st = c % kStages;
         mbar_wait(&full[st], (c / kStages) & 1);
         const float4* tb = stage_buf + size_t(st) * kChunkPairs * 2;
-        const int first = c * kChunkPairs;
-        const int pairs = min(kChunkPairs, full_pairs - first);          // may be <= 0 in a tail-only chunk
+        const int first = e_begin + c * kChunkPairs;
+        const int pairs = min(min(kChunkPairs, e_end - first), full_pairs - first);   // may be <= 0 in a tail-only chunk
         int k = 0;
 #pragma unroll 1
         for (; k + kGroup <= pairs; k += kGroup)
@@ -370,27 +378,31 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
         for (; k < pairs; ++k)
             sweep_group<1, false>(hc, tb + 2 * k, 2 * (first + k), cx, n_in, n64);
         // odd tail point: the duplicated entry counts once
-        if ((n_pts & 1) && full_pairs >= first && full_pairs < first + kChunkPairs)
+        if ((n_pts & 1) && full_pairs >= first && full_pairs < min(first + kChunkPairs, e_end))
             sweep_group<1, true>(hc, tb + 2 * (full_pairs - first), 2 * full_pairs, cx, n_in, n64);
         if (c + kStages < n_chunks) {                      // refill this stage (uniform branch)
             __syncthreads();
             if (threadIdx.x == 0) {
-                const int cn = c + kStages;
-                const int pn = min(kChunkPairs, n_pairs - cn * kChunkPairs);
+                const int fn = e_begin + (c + kStages) * kChunkPairs;
+                const int pn = min(kChunkPairs, e_end - fn);
                 mbar_arrive_expect_tx(&full[st], pn * 32u);
-                bulk_copy_g2s(stage_buf + size_t(st) * kChunkPairs * 2, table + size_t(cn) * kChunkPairs * 2, pn * 32u, &full[st]);
+                bulk_copy_g2s(stage_buf + size_t(st) * kChunkPairs * 2, table + size_t(fn) * 2, pn * 32u, &full[st]);
             }
         }
     }
 
     const unsigned count = ok ? n_in : 0u;
-    unsigned long long key = 0ull;
-    if (active) {
-        if (counts) counts[hidx] = static_cast<int>(count);
-        key = pack_key(count, static_cast<unsigned>(hidx));
+    if (split) {                                            // partial count; ransac_best_kernel finishes the job
+        if (active && count) atomicAdd(hs.acc + hidx, static_cast<int>(count));
+    } else {
+        unsigned long long key = 0ull;
+        if (active) {
+            if (counts) counts[hidx] = static_cast<int>(count);
+            key = pack_key(count, static_cast<unsigned>(hidx));
+        }
+        key = warp_max_u64(key);
+        if ((threadIdx.x & 31) == 0 && key != 0ull) atomicMax(&hdr->best_key, key);
     }
-    key = warp_max_u64(key);
-    if ((threadIdx.x & 31) == 0 && key != 0ull) atomicMax(&hdr->best_key, key);
     // statistics: hypotheses that needed fp64 decisions, and how many pairs
     const unsigned amb_mask = __ballot_sync(0xffffffffu, n64 != 0u);
     if (amb_mask) {
@@ -400,6 +412,22 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
             atomicAdd(&hdr->n_pairs_f64, static_cast<unsigned long long>(tot));
         }
     }
+}
+
+// ---- 2b. best (split mode): total counts of hypotheses [h0, h1) -> counts[] and the packed maximum --------
+__global__ void __launch_bounds__(256)
+ransac_best_kernel(const int* __restrict__ acc, int h0, int h1, int* __restrict__ counts, RansacHeader* __restrict__ hdr, int check_stop)
+{
+    if (check_stop && hdr->stop) return;
+    const int h = h0 + blockIdx.x * 256 + threadIdx.x;
+    unsigned long long key = 0ull;
+    if (h < h1) {
+        const int c = acc[h];
+        if (counts) counts[h] = c;
+        key = pack_key(static_cast<unsigned>(c), static_cast<unsigned>(h));
+    }
+    key = warp_max_u64(key);
+    if ((threadIdx.x & 31) == 0 && key != 0ull) atomicMax(&hdr->best_key, key);
 }
 
 // ---- 3. round (adaptive mode): the termination rule after `done` hypotheses ----------------------
@@ -442,13 +470,33 @@ __global__ void ransac_finalize_kernel(const float2* __restrict__ src_xy, const 
 static size_t align16(size_t v) { return (v + 15) & ~size_t(15); }
 static size_t table_bytes(int32_t n_pts) { return size_t((n_pts + 1) / 2) * 32; }
 
+// Launches with fewer hypothesis CTAs than half the machine also split the table over blockIdx.y.
+constexpr int kSplitBelowCtas = 148;
+constexpr int kMinPartEntries = 32;
+static bool may_split(int64_t n_hyp) { return (n_hyp + kRBlock - 1) / kRBlock < kSplitBelowCtas; }
+
+// entries per part for a launch of n_hyp hypotheses (>= n_pairs: one part)
+static int part_entries_for(int n_pairs, int64_t n_hyp)
+{
+    const int64_t ctas = (n_hyp + kRBlock - 1) / kRBlock;
+    if (ctas >= kSplitBelowCtas) return n_pairs;
+    int64_t parts = (2 * kSplitBelowCtas + ctas - 1) / ctas;                 // aim at two CTAs per SM
+    const int64_t max_parts = n_pairs / kMinPartEntries > 0 ? n_pairs / kMinPartEntries : 1;
+    if (parts > max_parts) parts = max_parts;
+    if (parts <= 1) return n_pairs;
+    int pe = static_cast<int>((n_pairs + parts - 1) / parts);
+    pe = (pe + 7) & ~7;                                                     // whole groups of 8 entries
+    return pe;
+}
+
 }  // namespace hg
 
 extern "C" size_t hg_ransac_workspace_bytes(int32_t n_pts, int64_t n_hyp)
 {
     if (n_pts < 0 || n_hyp < 0) return 0;
-    (void)n_hyp;                                   // no per-hypothesis scratch
-    return hg::kHeaderBytes + hg::align16(hg::table_bytes(n_pts));
+    // small batches accumulate partial counts (4 B per hypothesis) when the table is split over CTAs
+    const size_t acc = hg::may_split(n_hyp) ? hg::align16(size_t(n_hyp) * sizeof(int)) : 0;
+    return hg::kHeaderBytes + hg::align16(hg::table_bytes(n_pts)) + acc;
 }
 
 namespace hg {
@@ -463,7 +511,9 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     unsigned char* ws = static_cast<unsigned char*>(workspace);
     RansacHeader* hdr = reinterpret_cast<RansacHeader*>(ws);
-    float4* table = reinterpret_cast<float4*>(ws + kHeaderBytes);
+    // workspace layout: header | partial-count accumulator (small calls only) | packed table
+    const size_t acc_bytes = may_split(n_hyp) ? align16(size_t(n_hyp) * sizeof(int)) : 0;
+    float4* table = reinterpret_cast<float4*>(ws + kHeaderBytes + acc_bytes);
     const float2* s2 = reinterpret_cast<const float2*>(src_xy);
     const float2* d2 = reinterpret_cast<const float2*>(dst_xy);
     const int n_pairs = (n_pts + 1) / 2;
@@ -471,7 +521,7 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     const double inv_t = 1.0 / t;
     (void)workspace_bytes;
 
-    if (cudaMemsetAsync(hdr, 0, kHeaderBytes, st) != cudaSuccess) return HG_ERR_CUDA;
+    if (cudaMemsetAsync(hdr, 0, kHeaderBytes + acc_bytes, st) != cudaSuccess) return HG_ERR_CUDA;     // header and accumulator
     {
         int blocks = (n_pairs + 255) / 256;
         if (blocks > 1184) blocks = 1184;
@@ -488,12 +538,21 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     hs.idx_out = reinterpret_cast<int4*>(hyp_idx_out);
     hs.seed = seed;
     hs.check_stop = adaptive ? 1 : 0;
+    // split mode needs the accumulator, which the workspace holds only when the whole call is small (may_split(n_hyp))
+    hs.acc = acc_bytes ? reinterpret_cast<int*>(ws + kHeaderBytes) : nullptr;
     for (int64_t h0 = 0; h0 < n_hyp; h0 += round_hyp) {
         const int64_t h1 = (h0 + round_hyp < n_hyp) ? h0 + round_hyp : n_hyp;
         hs.h0 = static_cast<int>(h0); hs.h1 = static_cast<int>(h1);
-        const unsigned blocks = static_cast<unsigned>((h1 - h0 + kRBlock - 1) / kRBlock);
-        ransac_score_kernel<<<blocks, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, hs, inv_t, t, counts, hdr);
+        hs.part_entries = hs.acc ? part_entries_for(n_pairs, h1 - h0) : n_pairs;
+        const unsigned parts = static_cast<unsigned>((n_pairs + hs.part_entries - 1) / hs.part_entries);
+        const dim3 grid(static_cast<unsigned>((h1 - h0 + kRBlock - 1) / kRBlock), parts);
+        ransac_score_kernel<<<grid, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, hs, inv_t, t, counts, hdr);
         if (launch_status() != HG_OK) return HG_ERR_CUDA;
+        if (parts > 1) {
+            const unsigned bb = static_cast<unsigned>((h1 - h0 + 255) / 256);
+            ransac_best_kernel<<<bb, 256, 0, st>>>(hs.acc, hs.h0, hs.h1, counts, hdr, hs.check_stop);
+            if (launch_status() != HG_OK) return HG_ERR_CUDA;
+        }
         if (adaptive) {
             ransac_round_kernel<<<1, 32, 0, st>>>(hdr, n_pts, static_cast<long long>(h1), confidence, h1 == n_hyp ? 1 : 0);
             if (launch_status() != HG_OK) return HG_ERR_CUDA;

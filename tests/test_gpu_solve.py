@@ -65,6 +65,16 @@ def test_general_sets_f64_internal(general, method, layout):
 
 
 @pytest.mark.parametrize("method", ["aca", "sks"])
+def test_config2_full_batch_every_set_against_oracle(method):
+    """C2 as BASELINE.json states it: 2^20 general-position sets, fp32 SoA, every set compared with the oracle."""
+    n = 1 << 20
+    s, d = W.general_sets(n, seed=W.SEED_BASE + 2)
+    H = GPU_FN[method](W.to_soa(s).to(DEV), W.to_soa(d).to(DEV), layout=hg.SOA)
+    stats = check_parity(W.h_soa_to_aos(H.cpu()).numpy(), s.numpy(), d.numpy(), method)
+    print("C2", method, stats)
+
+
+@pytest.mark.parametrize("method", ["aca", "sks"])
 @pytest.mark.parametrize("n", [1, 3, 255, 1001, 4099])
 def test_ragged_sizes_scalar_path(method, n):
     """n % 4 != 0 takes the scalar-load SoA path; n < one block; plane stride = n."""

@@ -138,6 +138,45 @@ def event_time_ms(fn, reps, stream=None):
     return e0.elapsed_time(e1)
 
 
+def hbm_roofline(bytes_per_launch, ms, peak, peak_src, kernel, **kw):
+    """The `roofline` object of an HBM-bound leg: algorithmic bytes of one launch / its average duration."""
+    a = bytes_per_launch / ms / 1e6
+    return dict({"bound": "hbm", "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak, "traffic": None,
+                 "kernel": kernel, "algorithmic_bytes_per_launch": bytes_per_launch, "peak_source": peak_src}, **kw)
+
+
+def graph_of(fns, stream=None):
+    """One CUDA graph that runs every callable of `fns` once, in order (captured on a side stream)."""
+    st = stream or torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        for f in fns:
+            f()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            for f in fns:
+                f()
+    torch.cuda.current_stream().wait_stream(st)
+    g.replay()
+    return g
+
+
+def timed_oracle(fn, units, unit, sample, min_seconds=2.0):
+    """`cpu_baseline` object: the oracle call `fn` (OpenMP over all host cores) repeated for >= min_seconds."""
+    import oracle
+    oracle.set_num_threads(os.cpu_count() or 1)
+    fn()
+    done, t0 = 0, time.perf_counter()
+    while True:
+        fn()
+        done += 1
+        dt = time.perf_counter() - t0
+        if dt >= min_seconds:
+            break
+    return {"value": units * done / dt, "unit": unit, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "%s; %d passes, %.1f s" % (sample, done, dt)}
+
+
 # ---- the oracle on the host cores -------------------------------------------------------------------
 def oracle_rate(src_aos, dst_aos, passes, warm=1, min_seconds=0.0):
     """ACA-fp64 oracle, all host cores (OpenMP): homographies/s over at least `passes` passes of the sample
@@ -177,30 +216,45 @@ def run_reference(args, rank):
 
 
 # ---- extras: the other rows of the hot path at BASELINE sizes -----------------------------------------
-def run_extras(hg, W, dev, src, dst, H, peak):
+def run_extras(hg, W, dev, src, dst, H, peak, peak_src, cpu=True):
+    """Every other config of BASELINE.json (and the 8(f) rows) at its full size; each leg carries its own `roofline`
+    object and, with cpu=True, a `cpu_baseline` = the oracle on all host cores on a bounded sample of the same workload."""
+    import oracle
     n = src.shape[1]
     ex = {}
-    for name, fn in (("sks_c3", hg.hg_sks_batched),):
-        ms = event_time_ms(lambda: fn(src, dst, H=H), 5) / 5
-        ex[name] = {"ms": ms, "homographies_per_s": n / ms * 1e3, "GBps": n * BYTES_PER_H / ms / 1e6,
-                    "frac_of_peak": n * BYTES_PER_H / ms / 1e6 / peak}
+    SOLVE_K = "hg::solve_soa_kernel<%s,double,4>"
+    ms = event_time_ms(lambda: hg.hg_sks_batched(src, dst, H=H), 5) / 5
+    ex["sks_c3"] = {"ms": ms, "homographies_per_s": n / ms * 1e3,
+                    "roofline": hbm_roofline(n * BYTES_PER_H, ms, peak, peak_src, SOLVE_K % "SKS")}
     ms = event_time_ms(lambda: hg.hg_aca_batched(src, dst, H=H, prec=hg.PREC_F32), 5) / 5
     ex["aca_c3_plain_fp32"] = {"ms": ms, "GBps": n * BYTES_PER_H / ms / 1e6, "note": "HG_PREC_F32: fails the parity tolerance, measurement only"}
-    # C2: 2^20 sets = 105 MB, fits the 126 MB L2: timed with an L2 flush (a 256 MB memset) before every call, and warm
-    n2 = 1 << 20
-    s2, d2, H2 = src[:, :n2].contiguous(), dst[:, :n2].contiguous(), torch.empty((9, n2), dtype=torch.float32, device=dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    for name, fn in (("aca_c2", hg.hg_aca_batched), ("sks_c2", hg.hg_sks_batched)):
-        call = lambda: fn(s2, d2, H=H2)
-        call(); call()
-        cold = 0.0
-        for _ in range(10):
-            flush.zero_()
-            cold += event_time_ms(call, 1)
-        warm = event_time_ms(call, 20) / 20
-        ex[name] = {"ms_l2_flushed": cold / 10, "GBps_l2_flushed": n2 * BYTES_PER_H / (cold / 10) / 1e6,
-                    "ms_l2_warm": warm, "GBps_l2_warm": n2 * BYTES_PER_H / warm / 1e6, "l2": "flushed by a 256 MB memset / warm"}
-    del flush, s2, d2, H2
+    if cpu:
+        n_s = min(n, 1 << 24)
+        s_aos = W.to_aos(src[:, :n_s].contiguous()).cpu().numpy()
+        d_aos = W.to_aos(dst[:, :n_s].contiguous()).cpu().numpy()
+        ex["sks_c3"]["cpu_baseline"] = timed_oracle(lambda: oracle.sks(s_aos, d_aos), n_s, UNIT,
+                                                    "first 2^%d sets of the timed workload, SKS-fp64 oracle" % (n_s.bit_length() - 1), 3.0)
+    # C2: 2^20 sets = 105 MB per call, smaller than the 126 MB L2.  Eight disjoint (src, dst, H) triples = 839 MB are solved in
+    # turn inside one CUDA graph, so every call streams from HBM (inputs larger than L2, no flush kernel in the timed region)
+    # and no Python launch path is timed; `ms_l2_warm` = the same call repeated on one triple (L2-resident).
+    n2, R = 1 << 20, 8
+    trip = [(src[:, i * n2:(i + 1) * n2].contiguous(), dst[:, i * n2:(i + 1) * n2].contiguous(),
+             torch.empty((9, n2), dtype=torch.float32, device=dev)) for i in range(R)]
+    for name, fn, kn in (("aca_c2", hg.hg_aca_batched, "ACA"), ("sks_c2", hg.hg_sks_batched, "SKS")):
+        g = graph_of([(lambda a=a, b=b, c=c: fn(a, b, H=c)) for a, b, c in trip])
+        ms = event_time_ms(g.replay, 20) / (20 * R)
+        s2, d2, H2 = trip[0]
+        warm = event_time_ms(lambda: fn(s2, d2, H=H2), 20) / 20
+        ex[name] = {"ms": ms, "homographies_per_s": n2 / ms * 1e3, "ms_l2_warm_python_launch": warm,
+                    "l2": "inputs_larger_than_l2: 8 disjoint 105 MB triples solved in turn inside one CUDA graph",
+                    "roofline": hbm_roofline(n2 * BYTES_PER_H, ms, peak, peak_src, SOLVE_K % kn)}
+        del g
+    if cpu:
+        s_aos = W.to_aos(trip[0][0]).cpu().numpy()
+        d_aos = W.to_aos(trip[0][1]).cpu().numpy()
+        ex["aca_c2"]["cpu_baseline"] = timed_oracle(lambda: oracle.aca(s_aos, d_aos), n2, UNIT, "all 2^20 sets of one C2 batch, ACA-fp64 oracle")
+        ex["sks_c2"]["cpu_baseline"] = timed_oracle(lambda: oracle.sks(s_aos, d_aos), n2, UNIT, "all 2^20 sets of one C2 batch, SKS-fp64 oracle")
+    del trip
     # C5: offsets -> H -> grid, 8192 x 128 x 128 x 2 fp32 = 1.07 GB written per call (> L2)
     off = W.offsets_workload(8192, seed=W.SEED_BASE + 5, device=dev)
     Hh = torch.empty((8192, 3, 3), dtype=torch.float32, device=dev)
@@ -209,32 +263,38 @@ def run_extras(hg, W, dev, src, dst, H, peak):
     f5(); f5(); f5()
     ms = event_time_ms(f5, 10) / 10
     by = grid.numel() * 4 + off.numel() * 4 + Hh.numel() * 4
-    ex["grid_c5"] = {"ms": ms, "GBps_written": by / ms / 1e6, "frac_of_peak": by / ms / 1e6 / peak,
-                     "grids_per_s": 8192 / ms * 1e3}
+    ex["grid_c5"] = {"ms": ms, "grids_per_s": 8192 / ms * 1e3, "l2": "outputs_larger_than_l2 (1.07 GB per call)",
+                     "roofline": hbm_roofline(by, ms, peak, peak_src, "hg::offsets_to_grid_kernel<2>", bytes_per_item=by // 8192)}
     del grid
+    if cpu:
+        o_np = off[:1024].cpu().numpy()
+        ex["grid_c5"]["cpu_baseline"] = timed_oracle(lambda: oracle.offsets_to_grid(o_np, 0.0, 0.0, 127.0, 127.0, 128, 128), 1024,
+                                                     "grids/s", "first 1024 of the 8192 items (128 x 128 grid each), fp64 oracle")
     # C1: 1024 offsets -> H, launch-latency bound: us per call, plain launches and CUDA-graph replay
     off1 = W.offsets_workload(1024, seed=W.SEED_BASE + 1, device=dev)
     H1 = torch.empty((1024, 3, 3), dtype=torch.float32, device=dev)
-    f1 = lambda: hg.hg_offsets_to_grid(off1, 0.0, 0.0, 127.0, 127.0, 128, 128, H=H1, want_grid=False)
-    for _ in range(5):
-        f1()
-    ms = event_time_ms(f1, 200) / 200
-    ex["c1_offsets_to_h_1024"] = {"us_per_call_launch": ms * 1e3}
-    try:
-        st = torch.cuda.Stream()
-        st.wait_stream(torch.cuda.current_stream())
-        with torch.cuda.stream(st):
+    c1 = {}
+    for name, f1 in (("offsets_to_h", lambda: hg.hg_offsets_to_grid(off1, 0.0, 0.0, 127.0, 127.0, 128, 128, H=H1, want_grid=False)),
+                     ("aca_rect", lambda: hg.hg_aca_rect_batched(off1, 0.0, 0.0, 127.0, 127.0, H=H1, norm=hg.NORM_H33))):
+        for _ in range(5):
             f1()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=st):
-                for _ in range(20):
-                    f1()
-        torch.cuda.current_stream().wait_stream(st)
-        g.replay()
-        ms = event_time_ms(g.replay, 20) / (20 * 20)
-        ex["c1_offsets_to_h_1024"]["us_per_call_graph"] = ms * 1e3
-    except Exception as e:          # graph capture is a convenience measurement, never the headline
-        ex["c1_offsets_to_h_1024"]["graph_error"] = repr(e)[:200]
+        row = {"us_per_call_launch": event_time_ms(f1, 200) / 200 * 1e3}
+        try:
+            g = graph_of([f1] * 20)
+            row["us_per_call_graph"] = event_time_ms(g.replay, 20) / (20 * 20) * 1e3
+            del g
+        except Exception as e:          # graph capture is a convenience measurement, never the headline
+            row["graph_error"] = repr(e)[:200]
+        c1[name] = row
+    us = c1["offsets_to_h"].get("us_per_call_graph", c1["offsets_to_h"]["us_per_call_launch"])
+    ex["c1_offsets_to_h_1024"] = dict(c1["offsets_to_h"], aca_rect_entry_point=c1["aca_rect"], homographies_per_s=1024 / us * 1e6,
+                                      roofline=hbm_roofline(1024 * 68, us * 1e-3, peak, peak_src, "hg::offsets_to_h_kernel",
+                                                            note="70 KB per call: bound by one kernel launch (~2 us), not by HBM"))
+    if cpu:
+        o1 = off1.cpu().numpy()
+        ex["c1_offsets_to_h_1024"]["cpu_baseline"] = timed_oracle(
+            lambda: oracle.offsets_to_grid(o1, 0.0, 0.0, 127.0, 127.0, 128, 128, want_grid=False), 1024, UNIT,
+            "the 1024 offsets of C1 -> H per call, ACA-fp64 oracle", 1.0)
     # C4: fused RANSAC, 4096 correspondences x 2^20 hypotheses, 3 px
     wl = W.ransac_workload(device=dev)
     ws = torch.empty(hg.hg_ransac_workspace_bytes(4096, 1 << 20), dtype=torch.uint8, device=dev)
@@ -248,11 +308,23 @@ def run_extras(hg, W, dev, src, dst, H, peak):
     stats = hg.ransac_stats(ws)
     pairs = 4096 * (1 << 20)
     props = torch.cuda.get_device_properties(dev)
+    # FP32 issue peak at the clock SAMPLED during this leg (falls back to the maximum clock only when NVML gave no sample)
+    mhz = rclk.get("sm_mhz") or rclk.get("sm_max_mhz") or 1965.0
+    alu_peak = props.multi_processor_count * 128 * mhz * 1e6
+    ach = pairs * 11 / (ms * 1e-3)
     ex["ransac_c4"] = {"ms": ms, "pairs_per_s": pairs / ms * 1e3, "hypotheses_per_s": (1 << 20) / ms * 1e3,
                        "best_count": int(out["best_count"]), "hypotheses_with_fp64_decisions": stats["n_fixup"],
-                       "pairs_decided_in_fp64": stats["n_pairs_f64"],
-                       "clocks": rclk, "fp32_lane_instr_per_pair": 11, "alu_peak_instr_per_s": props.multi_processor_count * 128 * 1.965e9,
-                       "frac_of_fp32_issue_peak": pairs * 11 / (ms * 1e-3) / (props.multi_processor_count * 128 * 1.965e9)}
+                       "pairs_decided_in_fp64": stats["n_pairs_f64"], "clocks": rclk,
+                       "roofline": {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "FP32 lane-instructions/s",
+                                    "frac": ach / alu_peak, "traffic": None, "kernel": "hg::ransac_score_kernel",
+                                    "lane_instr_per_pair": 11, "peak_source": "%d SMs x 128 FP32 lanes x %.0f MHz sampled during the leg"
+                                                                               % (props.multi_processor_count, mhz)},
+                       "frac_of_fp32_issue_peak": ach / alu_peak}
+    if cpu:
+        nh = 1 << 15
+        s_np, d_np, i_np = wl["src_xy"].cpu().numpy(), wl["dst_xy"].cpu().numpy(), wl["hyp_idx"][:nh].cpu().numpy()
+        ex["ransac_c4"]["cpu_baseline"] = timed_oracle(lambda: oracle.ransac(s_np, d_np, i_np, 3.0), nh * 4096, "pairs/s",
+                                                       "first 2^15 of the 2^20 hypotheses x all 4096 correspondences, fp64 oracle", 3.0)
     # RANSAC extras: on-device sampling, rounds of one wave (296 CTAs x 512), with and without adaptive termination
     fa = lambda conf: hg.hg_ransac_adaptive(wl["src_xy"], wl["dst_xy"], 240218008, 1 << 20, 296 * 512, 3.0, conf,
                                             want_counts=False, workspace=ws)
@@ -262,32 +334,32 @@ def run_extras(hg, W, dev, src, dst, H, peak):
         ne = int(o["n_evaluated"])
         ex[name] = {"ms": ms, "n_evaluated": ne, "best_count": int(o["best_count"]), "pairs_per_s": ne * 4096 / ms * 1e3}
     # The scale of the paper's Table 6 (<= 1000 matches per image pair, a few to a few thousand loops; solver +
-    # verification loops 4.5-154 us on a CPU core): one call = memset + 3 kernels, us per call plain and in a CUDA graph.
-    wls = W.ransac_workload(n_pts=1000, n_hyp=1024, seed=W.SEED_BASE + 44, device=dev)
-    wss = torch.empty(hg.hg_ransac_workspace_bytes(1000, 1024), dtype=torch.uint8, device=dev)
-    fs = lambda: hg.hg_ransac_hypothesize_score(wls["src_xy"], wls["dst_xy"], wls["hyp_idx"], 3.0, want_counts=False, workspace=wss)
-    for _ in range(5):
-        fs()
-    small = {"n_pts": 1000, "n_hyp": 1024, "us_per_call_launch": event_time_ms(fs, 100) / 100 * 1e3}
-    try:
-        sts = torch.cuda.Stream()
-        with torch.cuda.stream(sts):
+    # verification loops 4.5-154 us on a CPU core): us per call, plain launches and inside a CUDA graph.
+    small = {}
+    for n_pts_s, n_hyp_s in ((1000, 1024), (500, 256)):
+        wls = W.ransac_workload(n_pts=n_pts_s, n_hyp=n_hyp_s, seed=W.SEED_BASE + 44, device=dev)
+        wss = torch.empty(hg.hg_ransac_workspace_bytes(n_pts_s, n_hyp_s), dtype=torch.uint8, device=dev)
+        fs = lambda: hg.hg_ransac_hypothesize_score(wls["src_xy"], wls["dst_xy"], wls["hyp_idx"], 3.0, want_counts=False, workspace=wss)
+        for _ in range(5):
             fs()
-            gs = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(gs, stream=sts):
-                for _ in range(10):
-                    fs()
-        torch.cuda.current_stream().wait_stream(sts)
-        gs.replay()
-        small["us_per_call_graph"] = event_time_ms(gs.replay, 20) / 200 * 1e3
-    except Exception as e:
-        small["graph_error"] = repr(e)[:200]
+        row = {"n_pts": n_pts_s, "n_hyp": n_hyp_s, "us_per_call_launch": event_time_ms(fs, 100) / 100 * 1e3}
+        try:
+            gs = graph_of([fs] * 10)
+            row["us_per_call_graph"] = event_time_ms(gs.replay, 20) / 200 * 1e3
+            del gs
+        except Exception as e:
+            row["graph_error"] = repr(e)[:200]
+        if cpu:
+            s_np, d_np, i_np = wls["src_xy"].cpu().numpy(), wls["dst_xy"].cpu().numpy(), wls["hyp_idx"].cpu().numpy()
+            row["cpu_baseline"] = timed_oracle(lambda: oracle.ransac(s_np, d_np, i_np, 3.0), 1, "calls/s",
+                                               "the whole call (%d hypotheses x %d correspondences), fp64 oracle" % (n_hyp_s, n_pts_s), 0.5)
+        small["%dx%d" % (n_hyp_s, n_pts_s)] = row
     ex["ransac_table6_scale"] = small
-    ex.update(run_next_rows(hg, W, dev, peak))
+    ex.update(run_next_rows(hg, W, dev, peak, peak_src))
     return ex
 
 
-def run_next_rows(hg, W, dev, peak):
+def run_next_rows(hg, W, dev, peak, peak_src):
     """SURVEY.md 8(f) rows at 2^26 items (2^25 for fp64 storage): all streaming, HBM-bound."""
     ex = {}
     n = 1 << 26
@@ -296,34 +368,34 @@ def run_next_rows(hg, W, dev, peak):
         for _ in range(3):
             fn()
         ms = event_time_ms(fn, reps) / reps
-        gbs = items * bytes_per_item / ms / 1e6
-        ex[name] = dict({"ms": ms, "items_per_s": items / ms * 1e3, "GBps": gbs, "frac_of_peak": gbs / peak,
-                         "bytes_per_item": bytes_per_item}, **kw)
+        kernel = kw.pop("kernel")
+        ex[name] = dict({"ms": ms, "items_per_s": items / ms * 1e3,
+                         "roofline": hbm_roofline(items * bytes_per_item, ms, peak, peak_src, kernel, bytes_per_item=bytes_per_item)}, **kw)
 
     off = W.offsets_workload(n, seed=W.SEED_BASE + 6, device=dev)
     Haos = torch.empty((n, 3, 3), dtype=torch.float32, device=dev)
-    leg("rect_aos_2p26", lambda: hg.hg_aca_rect_batched(off, 0.0, 0.0, 127.0, 127.0, H=Haos, layout=hg.AOS, norm=hg.NORM_H33), 68, n)
+    leg("rect_aos_2p26", lambda: hg.hg_aca_rect_batched(off, 0.0, 0.0, 127.0, 127.0, H=Haos, layout=hg.AOS, norm=hg.NORM_H33), 68, n, kernel="hg::rect_aos_kernel<double>")
     g = torch.randn((n, 3, 3), device=dev)
     go = torch.empty((n, 4, 2), dtype=torch.float32, device=dev)
-    leg("rect_backward_2p26", lambda: hg.hg_aca_rect_backward(off, 0.0, 0.0, 127.0, 127.0, g, grad_offsets=go), 100, n)
+    leg("rect_backward_2p26", lambda: hg.hg_aca_rect_backward(off, 0.0, 0.0, 127.0, 127.0, g, grad_offsets=go), 100, n, kernel="hg::rect_backward_kernel")
     del g, go, Haos
     osoa = off.reshape(n, 8).t().contiguous()
     del off
     Hsoa = torch.empty((9, n), dtype=torch.float32, device=dev)
-    leg("rect_soa_2p26", lambda: hg.hg_aca_rect_batched(osoa, 0.0, 0.0, 127.0, 127.0, H=Hsoa, layout=hg.SOA, norm=hg.NORM_H33), 68, n)
+    leg("rect_soa_2p26", lambda: hg.hg_aca_rect_batched(osoa, 0.0, 0.0, 127.0, 127.0, H=Hsoa, layout=hg.SOA, norm=hg.NORM_H33), 68, n, kernel="hg::rect_soa_kernel<double,4>")
     a = torch.rand((6, n), device=dev) * 600.0
     b = torch.rand((6, n), device=dev) * 600.0
-    leg("affine_soa_2p26", lambda: hg.hg_affine_batched(a, b, H=Hsoa), 84, n)
+    leg("affine_soa_2p26", lambda: hg.hg_affine_batched(a, b, H=Hsoa), 84, n, kernel="hg::variant_soa_kernel<AffineOp>")
     del a, b
     osoa.mul_(10.0).add_(300.0)                                  # reuse as image quadruples for the SK leg
-    leg("sk_soa_2p26", lambda: hg.hg_sk_batched((0.35, 1.6), (-0.8, -1.1), osoa, H=Hsoa), 68, n)
+    leg("sk_soa_2p26", lambda: hg.hg_sk_batched((0.35, 1.6), (-0.8, -1.1), osoa, H=Hsoa), 68, n, kernel="hg::variant_soa_kernel<SkOp>")
     del osoa, Hsoa
     m = 1 << 25
     s64 = torch.rand((8, m), device=dev, dtype=torch.float64) * 600.0
     d64 = torch.rand((8, m), device=dev, dtype=torch.float64) * 600.0
     H64 = torch.empty((9, m), device=dev, dtype=torch.float64)
-    leg("aca_f64_soa_2p25", lambda: hg.hg_aca_batched_f64(s64, d64, H=H64), 200, m)
-    leg("sks_f64_soa_2p25", lambda: hg.hg_sks_batched_f64(s64, d64, H=H64), 200, m)
+    leg("aca_f64_soa_2p25", lambda: hg.hg_aca_batched_f64(s64, d64, H=H64), 200, m, kernel="hg::variant_soa_kernel<GeneralOp<ACA>,double>")
+    leg("sks_f64_soa_2p25", lambda: hg.hg_sks_batched_f64(s64, d64, H=H64), 200, m, kernel="hg::variant_soa_kernel<GeneralOp<SKS>,double>")
     del s64, d64, H64
     # The sizes of the paper's Table 8 (1 ... 1M sets, fp64 storage, RTX 3090), as context: us per call,
     # back-to-back launches (launch-bound below ~10K sets, L2-resident up to ~500K sets), and with an L2 flush at 1M.
@@ -367,7 +439,13 @@ def run_next_rows(hg, W, dev, peak):
     img = torch.rand((k, 1, 128, 128), device=dev)
     out = torch.empty_like(img)
     leg("warp_c5_1ch", lambda: hg.hg_offsets_to_warp(off5, 0.0, 0.0, 127.0, 127.0, 128, 128, img, warped=out), 8, k * 128 * 128,
-        unit="pixels")
+        unit="pixels", kernel="hg::offsets_to_warp_kernel<1,true>")
+    del img, out
+    k3 = 4096
+    img3 = torch.rand((k3, 3, 128, 128), device=dev)
+    out3 = torch.empty_like(img3)
+    leg("warp_c5_3ch", lambda: hg.hg_offsets_to_warp(off5[:k3], 0.0, 0.0, 127.0, 127.0, 128, 128, img3, warped=out3), 8, k3 * 3 * 128 * 128,
+        unit="pixels x channels", kernel="hg::offsets_to_warp_kernel<3,...>")
     return ex
 
 
@@ -499,14 +577,18 @@ def main():
         del s_aos, d_aos
     if world == 1 and not args.no_extras:
         try:
-            line["extras"] = run_extras(hg, W, dev, src, dst, H, peak)
+            line["extras"] = run_extras(hg, W, dev, src, dst, H, peak, peak_src, cpu=not args.no_cpu)
         except Exception as e:
             line["extras"] = {"error": repr(e)[:300]}
     # traffic from the committed ncu capture, if one is recorded
     tfile = ROOT / "profiles" / "roofline_traffic.json"
     if tfile.exists():
         try:
-            line["roofline"]["traffic"] = json.loads(tfile.read_text()).get("aca_c3_dram_bytes_per_launch")
+            tr = json.loads(tfile.read_text())
+            line["roofline"]["traffic"] = tr.get("aca_c3_dram_bytes_per_launch")
+            for leg_name, leg_obj in line.get("extras", {}).items():
+                if isinstance(leg_obj, dict) and "roofline" in leg_obj and (leg_name + "_dram_bytes_per_launch") in tr:
+                    leg_obj["roofline"]["traffic"] = tr[leg_name + "_dram_bytes_per_launch"]
         except Exception:
             pass
     print(json.dumps(line), flush=True)

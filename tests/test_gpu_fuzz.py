@@ -7,7 +7,7 @@ import torch
 import hg_workloads as W
 import oracle
 import paper_2402_18008_b200 as hg
-from util import align_to
+from util import align_to, check_h_parity
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda"
@@ -26,9 +26,9 @@ def test_random_sizes_solvers_rect_backward():
         else:
             H = fn(s.to(DEV), d.to(DEV), layout=hg.AOS, norm=norm)
         ref = oracle.solve(oracle.METHOD_ACA if meth == 0 else oracle.METHOD_SKS, s.numpy(), d.numpy())
-        a, b = align_to(H.cpu().numpy().astype(np.float64), ref)
-        ok = (np.abs(a - b) <= 1e-4 * np.abs(b) + 1e-7).all(axis=(1, 2))
-        assert ok.mean() >= 0.97 or n < 40, (n, layout, norm, meth, ok.mean())     # R12: a few sets are rounding-sensitive
+        # every set: finite, element-wise bound, reprojection bound (1e-3 px, or S on the R12-excluded sets)
+        check_h_parity(H.cpu().numpy(), s.numpy(), d.numpy(), ref, oracle.dlt(s.numpy(), d.numpy()), require_frac=0.0,
+                       label=(n, layout, norm, meth))
         off = W.offsets_workload(n, seed=2000 + it)
         Hr = hg.hg_aca_rect_batched(off.to(DEV), 3.0, -2.0, 100.0, 60.0, norm=hg.NORM_FROBENIUS).cpu().numpy().astype(np.float64)
         a, b = align_to(Hr, oracle.aca_rect(off.numpy(), 3.0, -2.0, 100.0, 60.0))

@@ -77,19 +77,24 @@ def test_grid_config1_h_only_matches_oracle_and_general_solver():
     assert np.abs(a2 - b2).max() <= 2e-7
 
 
-def test_grid_full_config5_sampled():
-    """C5 at BASELINE size: 8192 x 128 x 128 x 2; a sample of items compared with the oracle and
-    the corner property checked on every item."""
+def test_grid_full_config5_every_item():
+    """C5 at BASELINE size: 8192 x 128 x 128 x 2 in the launch configuration bench.py times; EVERY pixel of EVERY item
+    compared with the oracle (in slabs of 512 items), plus the corner property and every H."""
     n = 8192
     off = W.offsets_workload(n, seed=W.SEED_BASE + 5)
     H, g = hg.hg_offsets_to_grid(off.to(DEV), 0.0, 0.0, 127.0, 127.0, 128, 128)
-    sel = np.arange(0, n, 127)
-    _, g_ref = oracle.offsets_to_grid(off.numpy()[sel], 0.0, 0.0, 127.0, 127.0, 128, 128)
-    assert np.abs(g[torch.from_numpy(sel).to(DEV)].cpu().numpy() - g_ref).max() <= GRID_TOL
+    worst = 0.0
+    for b0 in range(0, n, 512):
+        H_ref, g_ref = oracle.offsets_to_grid(off.numpy()[b0:b0 + 512], 0.0, 0.0, 127.0, 127.0, 128, 128)
+        worst = max(worst, float(np.abs(g[b0:b0 + 512].cpu().numpy() - g_ref).max()))
+        Hg, Hr = align_to(H[b0:b0 + 512].cpu().numpy().astype(np.float64), H_ref)
+        assert (np.abs(Hg - Hr) <= 1e-4 * np.abs(Hr) + 1e-7).all()
+    assert worst <= GRID_TOL, worst
     corners = W.patch_corners().to(DEV)
     got = torch.stack([g[:, 0, 0], g[:, 0, 127], g[:, 127, 127], g[:, 127, 0]], dim=1)
     assert (got - (corners[None] + off.to(DEV))).abs().max().item() <= GRID_TOL
     assert torch.isfinite(g).all()
+    print("C5 every item: max |grid - oracle| =", worst, "px")
 
 
 # ---- RANSAC ------------------------------------------------------------------------------------
@@ -151,21 +156,17 @@ def test_ransac_host_entry_point_and_no_counts():
     assert nc["counts"] is None and nc["best_index"].item() == dev["best_index"].item()
 
 
-def test_ransac_full_config4_sampled():
-    """C4 at BASELINE size (4096 correspondences, 2^20 hypotheses, t = 3 px), in the launch
-    configuration bench.py times; the oracle scores a strided sample of 8192 hypotheses plus the
-    GPU's best hypothesis."""
+def test_ransac_full_config4_every_hypothesis():
+    """C4 at BASELINE size (4096 correspondences, 2^20 hypotheses, t = 3 px), in the launch configuration bench.py
+    times; the oracle scores ALL 2^20 hypotheses (4.29e9 pairs, OpenMP) and every count, the best index, the best count
+    and the best H are compared."""
     wl = W.ransac_workload(n_pts=4096, n_hyp=1 << 20, seed=W.SEED_BASE + 4)
     out = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV), 3.0)
-    counts = out["counts"].cpu().numpy()
-    bi, bc = int(out["best_index"].item()), int(out["best_count"].item())
-    assert bc == counts.max() and bi == int(np.argmax(counts))
-    sel = np.unique(np.concatenate([np.arange(0, 1 << 20, 128), [bi, (1 << 20) - 1]]))
-    ref = oracle.ransac(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy()[sel], 3.0, band_rel=1e-4)
-    diff = np.abs(counts[sel].astype(np.int64) - ref["counts"])
-    assert (diff <= ref["band_counts"]).all(), int((diff > ref["band_counts"]).sum())
-    assert bc >= 0.6 * 0.7 * 4096
-    print("C4 sampled: mismatches inside band", int((diff > 0).sum()), "of", len(sel), hg.ransac_stats(out["workspace"]))
+    ref = oracle.ransac(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy(), 3.0, band_rel=1e-4)
+    diff = check_ransac(wl, 3.0, out, ref)
+    assert int(out["best_count"].item()) >= 0.6 * 0.7 * 4096
+    print("C4 every hypothesis: counts differing (all inside the band)", int((diff > 0).sum()), "of", 1 << 20,
+          "hypotheses with in-band pairs", int((ref["band_counts"] > 0).sum()), hg.ransac_stats(out["workspace"]))
 
 
 def test_ransac_degenerate_and_non_finite_inputs():

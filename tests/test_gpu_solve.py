@@ -2,8 +2,9 @@
 
 Comparison form and tolerances (BASELINE.json north_star, reading R12): both H are
 scaled to unit Frobenius norm and sign-aligned; a sample is *well-conditioned* when it passes the
-area filter of the generator and its own fp32-rounding sensitivity S is <= 1e-3 px; on those,
-4-point reprojection error <= 1e-3 px and |dH_ij| <= 1e-4 |H_ij| + 1e-7.
+area filter of the generator and its own fp32-rounding sensitivity S is <= 1e-3 px.  Asserted on EVERY set:
+finite H and |dH_ij| <= 1e-4 |H_ij| + 1e-7; 4-point reprojection error <= 1e-3 px on the well-conditioned sets and
+<= S + 1e-6 px on the others (tests/util.py::check_h_parity; the all-sample statistics are printed).
 """
 import numpy as np
 import pytest
@@ -12,33 +13,20 @@ import torch
 import hg_workloads as W
 import oracle
 import paper_2402_18008_b200 as hg
-from util import align_to, project, rounding_sensitivity
+from util import align_to, check_h_parity, project
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda"
 
-REL_TOL, ABS_FLOOR, REPROJ_TOL, S_MAX = 1e-4, 1e-7, 1e-3, 1e-3
 ORACLE = {"aca": oracle.METHOD_ACA, "sks": oracle.METHOD_SKS}
 GPU_FN = {"aca": hg.hg_aca_batched, "sks": hg.hg_sks_batched}
 
 
 def check_parity(H_gpu, src, dst, method, require_frac=0.98):
-    """H_gpu [n,3,3] (any scale), src/dst float32 numpy [n,4,2].  Returns the statistics dict."""
-    H_dlt = oracle.dlt(src, dst)
-    H_ref = oracle.solve(ORACLE[method], src, dst)
-    Hg, Hr = align_to(H_gpu.astype(np.float64), H_ref)
-    S = rounding_sensitivity(H_dlt, src)
-    well = S <= S_MAX
-    assert well.mean() >= require_frac, well.mean()
-    dH = np.abs(Hg - Hr)
-    tol = REL_TOL * np.abs(Hr) + ABS_FLOOR
-    elem_ok = (dH <= tol).all(axis=(1, 2))
-    reproj = np.abs(project(H_gpu.astype(np.float64), src) - dst.astype(np.float64)).max(axis=(1, 2))
-    assert np.isfinite(H_gpu[well]).all()
-    assert elem_ok[well].all(), (method, "elementwise", int((~elem_ok[well]).sum()), float((dH / tol)[well].max()))
-    assert (reproj[well] <= REPROJ_TOL).all(), (method, "reproj", float(reproj[well].max()))
-    return {"well_frac": float(well.mean()), "max_reproj_well": float(reproj[well].max()),
-            "max_rel": float((dH / tol)[well].max())}
+    """H_gpu [n,3,3] (any scale), src/dst float32 numpy [n,4,2].  Every set is checked (util.check_h_parity);
+    returns the all-sample statistics."""
+    return check_h_parity(H_gpu, src, dst, oracle.solve(ORACLE[method], src, dst), oracle.dlt(src, dst),
+                          require_frac=require_frac, label=method)
 
 
 @pytest.fixture(scope="module")

@@ -11,8 +11,12 @@
  * ---------------------------------------
  *  - Every pointer is a DEVICE pointer owned by the caller unless the name ends in `_host`
  *    (those entry points take HOST pointers, pinned or pageable, and do the copies themselves).
- *  - The library keeps no state and allocates no device memory (the `_host` entry points
- *    allocate and free their own staging buffers and streams inside the call).
+ *  - The library allocates no device memory (the `_host` entry points allocate and free their
+ *    own staging buffers and streams inside the call) and keeps no state, with one exception: the
+ *    RANSAC entry points stage tables of <= 4096 correspondences in the device's 64 KB constant
+ *    bank.  Calls that do so are ordered against each other through an internal event (thread-safe;
+ *    they may be issued from any streams), but under CUDA stream capture that ordering cannot be
+ *    recorded: replays of a captured RANSAC call must not overlap other RANSAC calls on that device.
  *  - Device entry points only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as void*;
  *    NULL = the legacy default stream) and never synchronise; `_host` entry points return
  *    after their result is complete in host memory.
@@ -277,11 +281,41 @@ HG_API int hg_ransac_adaptive(const float* src_xy, const float* dst_xy, int32_t 
                        int32_t* best_count, int64_t* n_evaluated, void* workspace,
                        size_t workspace_bytes, void* cuda_stream);
 
-/* After hg_ransac_hypothesize_score has completed on its stream, the first 4 int64 words of
- * the workspace hold statistics of that call (device memory; copy them out to read):
+/* Options of the `_ex` forms (a HOST struct, read during the call; NULL = all defaults = the plain entry points).
+ *   HG_RANSAC_REJECT_DEGENERATE : test every 4-point sample before scoring it (reading R20; degenerate
+ *                                 configurations P:786): rejected hypotheses score 0 and skip the sweep.
+ *   HG_RANSAC_DECIDE_ALL_F64    : verification mode -- no fp32 sweep; every (hypothesis, point) pair is decided by
+ *                                 the definition in fp64 from the kernel's own fp64 H.  Orders of magnitude slower;
+ *                                 it exists so that the exactness of the fp32 sweep + error band can be checked
+ *                                 bit for bit against it.                                                         */
+#define HG_RANSAC_REJECT_DEGENERATE 1u
+#define HG_RANSAC_DECIDE_ALL_F64    2u
+typedef struct hg_ransac_options {
+    uint32_t flags;          /* OR of HG_RANSAC_* bits; unknown bits -> HG_ERR_INVALID_ARG                       */
+    float    min_area_px2;   /* HG_RANSAC_REJECT_DEGENERATE: epsilon of R20 in px^2 (>= 0; 0 rejects only exact
+                                collinearity / coincidence and orientation flips)                                  */
+} hg_ransac_options_t;
+
+HG_API int hg_ransac_hypothesize_score_ex(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                                   const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
+                                   const hg_ransac_options_t* options,
+                                   int32_t* counts, float* best_H, int64_t* best_index,
+                                   int32_t* best_count, void* workspace, size_t workspace_bytes,
+                                   void* cuda_stream);
+HG_API int hg_ransac_adaptive_ex(const float* src_xy, const float* dst_xy, int32_t n_pts, uint64_t seed,
+                          int64_t max_hyp, int64_t round_hyp, float threshold_px, float confidence,
+                          const hg_ransac_options_t* options,
+                          int32_t* counts, int32_t* hyp_idx_out, float* best_H, int64_t* best_index,
+                          int32_t* best_count, int64_t* n_evaluated, void* workspace,
+                          size_t workspace_bytes, void* cuda_stream);
+
+/* After a RANSAC call has completed on its stream, the first 6 int64 words of the workspace hold
+ * statistics of that call (device memory; copy them out to read):
  *   [0] packed best key, [1] number of hypotheses that had at least one pair decided in fp64,
- *   [2] number of (hypothesis, point) pairs decided in fp64, [3] hypotheses scored (adaptive mode).                      */
-#define HG_RANSAC_STAT_WORDS 4
+ *   [2] number of (hypothesis, point) pairs decided in fp64, [3] hypotheses scored (adaptive mode),
+ *   [4] hypotheses rejected by HG_RANSAC_REJECT_DEGENERATE, [5] pairs that fell inside the table-wide
+ *   fp32 band and were re-tested against the per-pair band.                  */
+#define HG_RANSAC_STAT_WORDS 6
 
 /* Host-buffer form: all pointers are HOST pointers; the call allocates device memory and the
  * workspace, copies in, runs, copies counts/best out and waits.                                  */

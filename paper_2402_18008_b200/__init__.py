@@ -22,8 +22,8 @@ __all__ = [
     "hg_sks_batched_host", "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
     "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
     "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
-    "hg_status_string",
-    "hg_version", "hg_built_for_sm", "EXPORTS",
+    "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex", "RANSAC_REJECT_DEGENERATE", "RANSAC_DECIDE_ALL_F64",
+    "hg_status_string", "hg_version", "hg_built_for_sm", "EXPORTS",
 ]
 
 # include/hg.h enums
@@ -31,15 +31,22 @@ HG_OK = 0
 SOA, AOS = 0, 1
 NORM_NONE, NORM_H33, NORM_FROBENIUS = 0, 1, 2
 PREC_F64, PREC_F32 = 0, 1
-RANSAC_STAT_WORDS = 4
+RANSAC_STAT_WORDS = 6
+RANSAC_REJECT_DEGENERATE, RANSAC_DECIDE_ALL_F64 = 1, 2
 
 # every symbol include/hg.h declares
 EXPORTS = [
     "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
     "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_affine_batched",
     "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
-    "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive", "hg_status_string", "hg_version", "hg_built_for_sm",
+    "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive", "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex",
+    "hg_status_string", "hg_version", "hg_built_for_sm",
 ]
+
+
+class _RansacOptions(ctypes.Structure):
+    """hg_ransac_options_t"""
+    _fields_ = [("flags", ctypes.c_uint32), ("min_area_px2", ctypes.c_float)]
 
 
 class HgError(RuntimeError):
@@ -84,8 +91,12 @@ def lib() -> ctypes.CDLL:
         L.hg_ransac_workspace_bytes.restype = ctypes.c_size_t
         L.hg_ransac_hypothesize_score.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp,
                                                   _vp, ctypes.c_size_t, _vp]
+        L.hg_ransac_hypothesize_score_ex.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp, _vp,
+                                                     _vp, ctypes.c_size_t, _vp]
         L.hg_ransac_adaptive.argtypes = [_vp, _vp, _c_i32, ctypes.c_uint64, _c_i64, _c_i64, _c_f32, _c_f32, _vp, _vp, _vp, _vp, _vp,
                                          _vp, _vp, ctypes.c_size_t, _vp]
+        L.hg_ransac_adaptive_ex.argtypes = [_vp, _vp, _c_i32, ctypes.c_uint64, _c_i64, _c_i64, _c_f32, _c_f32, _vp, _vp, _vp, _vp, _vp,
+                                            _vp, _vp, _vp, ctypes.c_size_t, _vp]
         L.hg_ransac_hypothesize_score_host.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp]
         L.hg_status_string.argtypes = [_c_int]
         L.hg_status_string.restype = ctypes.c_char_p
@@ -93,7 +104,7 @@ def lib() -> ctypes.CDLL:
                      "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
                      "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
                      "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
-                     "hg_version", "hg_built_for_sm"):
+                     "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex", "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
         _lib = L
     return _lib
@@ -136,6 +147,19 @@ def _stream(stream=None):
             return _vp(int(_raw_stream(torch.cuda.current_device())))
         stream = torch.cuda.current_stream()
     return _vp(int(stream.cuda_stream))
+
+
+def _same_device(*tensors):
+    """Every device tensor of one call must live on one GPU: the kernels dereference all of them on the first one's device."""
+    dev = None
+    for x in tensors:
+        if x is None or not isinstance(x, torch.Tensor):
+            continue
+        if dev is None:
+            dev = x.device
+        elif x.device != dev:
+            raise ValueError("all tensors of a call must be on one device, got %s and %s" % (dev, x.device))
+    return dev
 
 
 class _NoCtx:
@@ -187,6 +211,7 @@ def _solve(fn_name: str, src, dst, H, layout, norm, prec, stream):
     fn = getattr(lib(), fn_name)
     ps, pd, ph = (_ptr(src, torch.float32, "cuda", "src"), _ptr(dst, torch.float32, "cuda", "dst"),
                   _ptr(H, torch.float32, "cuda", "H"))
+    _same_device(src, dst, H)
     with _on(src.device):
         st = fn(ps, pd, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, fn_name)
@@ -249,6 +274,7 @@ def hg_offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w
         raise ValueError("H must be [n,3,3]")
     if grid is not None and tuple(grid.shape) != (n, grid_h, grid_w, 2):
         raise ValueError("grid must be [n,grid_h,grid_w,2]")
+    _same_device(offsets, H, grid)
     with _on(offsets.device):
         st = lib().hg_offsets_to_grid(po, x0, y0, w, h,
                                       int(grid_w), int(grid_h), _ptr(H, torch.float32, "cuda", "H"),
@@ -271,6 +297,7 @@ def hg_offsets_to_warp(offsets, x0: float, y0: float, w: float, h: float, out_w:
     elif tuple(warped.shape) != (n, C, out_h, out_w):
         raise ValueError("warped must be [n,C,out_h,out_w]")
     H = torch.empty((n, 3, 3), dtype=torch.float32, device=offsets.device) if want_H else None
+    _same_device(offsets, image, warped, H)
     with _on(offsets.device):
         st = lib().hg_offsets_to_warp(_ptr(offsets, torch.float32, "cuda", "offsets"), x0, y0, w, h, int(out_w), int(out_h),
                                       _ptr(image, torch.float32, "cuda", "image"), C, iw, ih,
@@ -289,6 +316,7 @@ def hg_aca_rect_batched(offsets, x0: float, y0: float, w: float, h: float, H=Non
     elif tuple(H.shape) != _h_shape(n, layout):
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
     po, ph = _ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(H, torch.float32, "cuda", "H")
+    _same_device(offsets, H)
     with _on(offsets.device):
         st = lib().hg_aca_rect_batched(po, x0, y0, w, h, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, "hg_aca_rect_batched")
@@ -307,6 +335,7 @@ def hg_aca_rect_backward(offsets, x0: float, y0: float, w: float, h: float, grad
         raise ValueError("grad_offsets must be [n,4,2]")
     po, pg, pr = (_ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(grad_H, torch.float32, "cuda", "grad_H"),
                   _ptr(grad_offsets, torch.float32, "cuda", "grad_offsets"))
+    _same_device(offsets, grad_H, grad_offsets)
     with _on(offsets.device):
         st = lib().hg_aca_rect_backward(po, x0, y0, w, h, pg, pr, n, _stream(stream))
     _check(st, "hg_aca_rect_backward")
@@ -335,6 +364,7 @@ def hg_affine_batched(src3, dst3, H=None, layout: int = SOA, norm: int = NORM_NO
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
     ps, pd, ph = (_ptr(src3, torch.float32, "cuda", "src3"), _ptr(dst3, torch.float32, "cuda", "dst3"),
                   _ptr(H, torch.float32, "cuda", "H"))
+    _same_device(src3, dst3, H)
     with _on(src3.device):
         st = lib().hg_affine_batched(ps, pd, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, "hg_affine_batched")
@@ -350,6 +380,7 @@ def hg_sk_batched(P3, Q3, dst, H=None, layout: int = SOA, norm: int = NORM_NONE,
     elif tuple(H.shape) != _h_shape(n, layout):
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
     pd, ph = _ptr(dst, torch.float32, "cuda", "dst"), _ptr(H, torch.float32, "cuda", "H")
+    _same_device(dst, H)
     with _on(dst.device):
         st = lib().hg_sk_batched(float(P3[0]), float(P3[1]), float(Q3[0]), float(Q3[1]), pd, ph, n, int(layout),
                                  int(norm), int(prec), _stream(stream))
@@ -367,6 +398,7 @@ def _solve_f64(fn_name: str, src, dst, H, layout, norm, stream):
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
     ps, pd, ph = (_ptr(src, torch.float64, "cuda", "src"), _ptr(dst, torch.float64, "cuda", "dst"),
                   _ptr(H, torch.float64, "cuda", "H"))
+    _same_device(src, dst, H)
     with _on(src.device):
         st = getattr(lib(), fn_name)(ps, pd, ph, n, int(layout), int(norm), _stream(stream))
     _check(st, fn_name)
@@ -386,11 +418,22 @@ def hg_ransac_workspace_bytes(n_pts: int, n_hyp: int) -> int:
     return int(lib().hg_ransac_workspace_bytes(int(n_pts), int(n_hyp)))
 
 
+def _ransac_options(reject_degenerate, min_area_px2, decide_all_f64):
+    """(hg_ransac_options_t or None): None when every option is at its default, so the plain entry point is called."""
+    flags = (RANSAC_REJECT_DEGENERATE if reject_degenerate else 0) | (RANSAC_DECIDE_ALL_F64 if decide_all_f64 else 0)
+    if not flags:
+        return None
+    return _RansacOptions(flags, float(min_area_px2))
+
+
 def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, counts=None, workspace=None,
-                                want_counts: bool = True, stream=None):
+                                want_counts: bool = True, stream=None, reject_degenerate: bool = False,
+                                min_area_px2: float = 0.0, decide_all_f64: bool = False):
     """src_xy, dst_xy float32 [n_pts,2]; hyp_idx int32 [n_hyp,4] (all on the GPU).
     Returns dict(counts int32 [n_hyp] or None, best_H float32 [3,3], best_index int64 [1],
-    best_count int32 [1], workspace uint8) -- device tensors, produced asynchronously."""
+    best_count int32 [1], workspace uint8) -- device tensors, produced asynchronously.
+    reject_degenerate / min_area_px2 / decide_all_f64: hg_ransac_options_t (the call goes through
+    hg_ransac_hypothesize_score_ex when any is set)."""
     n_pts, n_hyp = int(src_xy.shape[0]), int(hyp_idx.shape[0])
     if tuple(src_xy.shape) != (n_pts, 2) or tuple(dst_xy.shape) != (n_pts, 2):
         raise ValueError("src_xy, dst_xy are float32 [n_pts, 2]")
@@ -406,23 +449,34 @@ def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, co
     best_H = torch.empty((3, 3), dtype=torch.float32, device=dev)
     best_index = torch.empty((1,), dtype=torch.int64, device=dev)
     best_count = torch.empty((1,), dtype=torch.int32, device=dev)
-    with _on(dev):
-        st = lib().hg_ransac_hypothesize_score(
-            _ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
-            _ptr(hyp_idx, torch.int32, "cuda", "hyp_idx"), n_hyp, float(threshold_px),
-            _ptr(counts, torch.int32, "cuda", "counts"), _ptr(best_H, torch.float32, "cuda", "best_H"),
+    _same_device(src_xy, dst_xy, hyp_idx, counts, workspace)
+    opt = _ransac_options(reject_degenerate, min_area_px2, decide_all_f64)
+    head = (_ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
+            _ptr(hyp_idx, torch.int32, "cuda", "hyp_idx"), n_hyp, float(threshold_px))
+    tail = (_ptr(counts, torch.int32, "cuda", "counts"), _ptr(best_H, torch.float32, "cuda", "best_H"),
             _ptr(best_index, torch.int64, "cuda", "best_index"), _ptr(best_count, torch.int32, "cuda", "best_count"),
             _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()), _stream(stream))
+    with _on(dev):
+        if opt is None:
+            st = lib().hg_ransac_hypothesize_score(*head, *tail)
+        else:
+            st = lib().hg_ransac_hypothesize_score_ex(*head, ctypes.cast(ctypes.pointer(opt), _vp), *tail)
     _check(st, "hg_ransac_hypothesize_score")
     return {"counts": counts, "best_H": best_H, "best_index": best_index, "best_count": best_count,
             "workspace": workspace}
 
 
+hg_ransac_hypothesize_score_ex = hg_ransac_hypothesize_score      # one Python function serves both C entry points
+
+
 def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, threshold_px: float, confidence: float,
-                       want_counts: bool = True, want_idx: bool = False, workspace=None, stream=None):
+                       want_counts: bool = True, want_idx: bool = False, workspace=None, stream=None,
+                       reject_degenerate: bool = False, min_area_px2: float = 0.0, decide_all_f64: bool = False):
     """On-device sampling (Philox4x32-10) + rounds + adaptive termination.  Returns dict(counts [max_hyp] or None,
     hyp_idx [max_hyp,4] or None, best_H [3,3], best_index [1], best_count [1], n_evaluated [1], workspace) -- device tensors."""
     n_pts = int(src_xy.shape[0])
+    if tuple(src_xy.shape) != (n_pts, 2) or tuple(dst_xy.shape) != (n_pts, 2):
+        raise ValueError("src_xy, dst_xy are float32 [n_pts, 2]")
     dev = src_xy.device
     need = hg_ransac_workspace_bytes(n_pts, max_hyp)
     if workspace is None:
@@ -433,23 +487,32 @@ def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, 
     best_index = torch.empty((1,), dtype=torch.int64, device=dev)
     best_count = torch.empty((1,), dtype=torch.int32, device=dev)
     n_eval = torch.empty((1,), dtype=torch.int64, device=dev)
-    with _on(dev):
-        st = lib().hg_ransac_adaptive(
-            _ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
-            int(seed) & 0xFFFFFFFFFFFFFFFF, int(max_hyp), int(round_hyp), float(threshold_px), float(confidence),
-            _ptr(counts, torch.int32, "cuda", "counts"), _ptr(idx, torch.int32, "cuda", "hyp_idx_out"),
+    _same_device(src_xy, dst_xy, workspace)
+    opt = _ransac_options(reject_degenerate, min_area_px2, decide_all_f64)
+    head = (_ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
+            int(seed) & 0xFFFFFFFFFFFFFFFF, int(max_hyp), int(round_hyp), float(threshold_px), float(confidence))
+    tail = (_ptr(counts, torch.int32, "cuda", "counts"), _ptr(idx, torch.int32, "cuda", "hyp_idx_out"),
             _ptr(best_H, torch.float32, "cuda", "best_H"), _ptr(best_index, torch.int64, "cuda", "best_index"),
             _ptr(best_count, torch.int32, "cuda", "best_count"), _ptr(n_eval, torch.int64, "cuda", "n_evaluated"),
             _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()), _stream(stream))
+    with _on(dev):
+        if opt is None:
+            st = lib().hg_ransac_adaptive(*head, *tail)
+        else:
+            st = lib().hg_ransac_adaptive_ex(*head, ctypes.cast(ctypes.pointer(opt), _vp), *tail)
     _check(st, "hg_ransac_adaptive")
     return {"counts": counts, "hyp_idx": idx, "best_H": best_H, "best_index": best_index, "best_count": best_count,
             "n_evaluated": n_eval, "workspace": workspace}
 
 
+hg_ransac_adaptive_ex = hg_ransac_adaptive
+
+
 def ransac_stats(workspace: torch.Tensor) -> dict:
     """Decode the statistics words a finished hg_ransac_hypothesize_score call left in its workspace."""
     w = workspace[: 8 * RANSAC_STAT_WORDS].cpu().view(torch.int64)
-    return {"best_key": int(w[0]), "n_fixup": int(w[1]), "n_pairs_f64": int(w[2]), "n_evaluated": int(w[3])}
+    return {"best_key": int(w[0]), "n_fixup": int(w[1]), "n_pairs_f64": int(w[2]), "n_evaluated": int(w[3]),
+            "n_rejected": int(w[4]), "n_band": int(w[5])}
 
 
 def hg_ransac_hypothesize_score_host(src_xy, dst_xy, hyp_idx, threshold_px: float, want_counts: bool = True):

@@ -1,18 +1,27 @@
-// hg_ransac.cu -- hg_ransac_hypothesize_score: RANSAC hypothesis generation fused with inlier
-// scoring (rows a-R0..a-R5 of SURVEY.md section 8(a)).
+// hg_ransac.cu -- hg_ransac_hypothesize_score / hg_ransac_adaptive: RANSAC hypothesis generation fused
+// with inlier scoring (rows a-R0..a-R5 of SURVEY.md section 8(a)).
 //
-// Three launches on the caller's stream, no host synchronisation:
+// Launches on the caller's stream, no host synchronisation:
 //   1. prep     : correspondence table -> packed, threshold-folded fp32 table in the workspace
 //                 (+ coordinate bounds for the error band)
 //   2. score    : one thread per hypothesis: gather 4 correspondences, fp64 ACA solve, fold the
-//                 threshold into H, then sweep the whole table from shared memory (staged by
-//                 bulk-async copies / mbarrier) with packed FFMA2 arithmetic, two points per
-//                 instruction.  One value per pair, a = (ex^2 + ey^2 - W^2) + Bc, against a rigorous
+//                 threshold into H, then sweep the whole table with packed FFMA2 arithmetic, two points
+//                 per instruction.  One value per pair, a = (ex^2 + ey^2 - W^2) + Bc, against a rigorous
 //                 per-hypothesis fp32 error band Bc: a < 0 is a
 //                 sure inlier, a > 2 Bc a sure outlier; the rare pair in between is decided on the
 //                 spot in fp64 by the definition (reading R9) from the fp64 H kept in shared memory.
+//                 Where the table comes from ("operand paths"):
+//                   - tables of <= 4096 points scored by >= 148 CTAs: the packed table is copied into the
+//                     64 KB constant bank; the sweep reads it through the uniform datapath (LDCU.64 ->
+//                     uniform-register FFMA2 operands), which costs no register-file bandwidth -- the
+//                     limiter of a three-operand FFMA2 stream on this part;
+//                   - everything else: the table is staged in shared memory by bulk-async copies /
+//                     mbarrier (32 KB stages) and read with broadcast LDS.128.
 //   3. finalize : decode the packed (count, index) maximum, re-solve that hypothesis, emit best_H.
 // Compute-bound on the FP32 pipe: 11 packed instructions per two (hypothesis, point) pairs.
+#include <memory>
+#include <mutex>
+
 #include "hg_device.cuh"
 #include "hg_host.h"
 
@@ -21,18 +30,26 @@ namespace hg {
 constexpr int kRBlock     = 512;    // threads (= hypotheses) per scoring CTA
 constexpr int kChunkPairs = 1024;   // point pairs per shared-memory stage: 1024 * 32 B = 32 KB
 constexpr int kStages     = 2;
-constexpr size_t kHeaderBytes = 64;
+constexpr size_t kHeaderBytes = 128;
+constexpr int kConstPairs = 2048;   // table entries (point pairs) the constant bank holds: 2048 * 32 B = 64 KB
 
-struct RansacHeader {               // first 64 bytes of the workspace
+struct RansacHeader {               // first 128 bytes of the workspace
     unsigned long long best_key;    // (count << 32) | (0xFFFFFFFF - hypothesis index)
     unsigned long long n_fixup;     // hypotheses with at least one pair decided in fp64
     unsigned long long n_pairs_f64; // (hypothesis, point) pairs decided in fp64
     unsigned long long n_evaluated; // adaptive mode: hypotheses scored when the run stopped
+    unsigned long long n_rejected;  // HG_RANSAC_REJECT_DEGENERATE: hypotheses rejected by the sample check (R20)
+    unsigned long long n_band;      // pairs inside the table-wide band (re-tested against the per-pair band)
+    unsigned long long reserved[2];
     unsigned int bound_bits[4];     // float bits of max|sx|, max|sy|, max|dx/t|, max|dy/t|
     unsigned int stop;              // adaptive mode: set by the round kernel, later rounds return at once
-    unsigned int pad[3];
+    unsigned int pad[11];
 };
 static_assert(sizeof(RansacHeader) == kHeaderBytes, "header layout");
+
+// The packed table of a call with <= 4096 points, in the constant bank: the sweep's point operands then come
+// through the uniform datapath.  One per device context; calls that use it are ordered by ConstTableGuard.
+__constant__ float4 c_table[2 * kConstPairs];
 
 // Per-hypothesis constants of the fp32 sweep.
 struct HypConst {
@@ -82,7 +99,8 @@ struct HypSource {
     const int4* idx;            // caller-supplied indices [n_hyp][4], or nullptr: sample on the device
     int4* idx_out;              // sampling mode, nullable: the sampled indices are written here
     unsigned long long seed;    // sampling mode
-    int h0, h1;                 // this launch scores hypotheses [h0, h1)
+    long long h0, h1;           // this launch scores hypotheses [h0, h1)
+    unsigned flags;             // HG_RANSAC_* option bits
     int check_stop;             // 1: return at once when hdr->stop is set (adaptive termination)
     int part_entries;           // table entries per blockIdx.y part (a multiple of 8); >= n_pairs: no split
     int* acc;                   // split mode: partial counts are added here (zeroed before the launch)
@@ -121,7 +139,7 @@ __device__ __forceinline__ int4 sample4(unsigned long long seed, unsigned long l
     return make_int4(first % n_pts, (first + 1) % n_pts, (first + 2) % n_pts, (first + 3) % n_pts);
 }
 
-__device__ __forceinline__ int4 hypothesis_indices(const HypSource& hs, int hidx, int n_pts)
+__device__ __forceinline__ int4 hypothesis_indices(const HypSource& hs, long long hidx, int n_pts)
 {
     return hs.idx ? __ldg(hs.idx + hidx) : sample4(hs.seed, static_cast<unsigned long long>(hidx), n_pts);
 }
@@ -231,54 +249,125 @@ __device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v)
     return v;
 }
 
-// Context of the cold path inside the sweep.
+// ---- the cold path: pairs whose fp32 value fell inside the table-wide band --------------------------------
+// Inside the sweep such a pair is only re-tested against the tighter per-pair band (same fp32 arithmetic, a few dozen
+// instructions, no memory traffic beyond the constant/shared table).  What is still undecided -- 6e-5 of the pairs of
+// C4 -- needs the definition in fp64 (global loads, two divisions, a square root): the sweep appends the point index to
+// a small per-thread queue in shared memory, and after the sweep `drain_queue` decides the queued pairs, all lanes of
+// the warp at once, so the loads and the fp64 arithmetic of different hypotheses overlap and the warps of a CTA stay
+// together while they walk the table.
+constexpr int kQueueCap = 8;            // queued pairs per thread (C4: 0.3 per hypothesis on average)
+
+
 struct SlowCtx {
-    const double* Hs;        // this thread's fp64 H (max-abs normalised) in shared memory, stride kRBlock
-    const float*  Ks;        // this thread's per-pair band constants K, K0 in shared memory, stride kRBlock
     const float2* src_xy;
     const float2* dst_xy;
-    double t;
+    const float4* table;     // packed table in global memory (the sweep's fp32 operands, bit for bit)
+    int4 id;                 // the hypothesis' four correspondences
+    double inv_t, t;
+    float bounds[4];
+    unsigned* queue;         // this thread's queue in shared memory, stride kRBlock
+    unsigned n64;            // out: pairs decided in fp64
 };
 
-// The definition in fp64 for one pair (rare: a few pairs per ten thousand).
-__device__ __noinline__ unsigned resolve_pair_f64(const SlowCtx& cx, int pt)
-{
-    double H[9];
-#pragma unroll
-    for (int k = 0; k < 9; ++k) H[k] = cx.Hs[k * kRBlock];
-    const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
-    return inlier_f64(H, sp.x, sp.y, dq.x, dq.y, cx.t) ? 1u : 0u;
-}
-
-// A pair whose fp32 value fell inside the table-wide band Bc: apply the tighter per-pair band
-// K|W| + K0 to the same fp32 arithmetic (bit-identical X, Y, W, ex, ey: same operands and FMA nesting
-// as score2).  Returns 1 = surely inlier, 0 = surely outlier, 2 = still undecided.
-__device__ __forceinline__ unsigned recheck_f32(const HypConst& c, float K, float K0, float sx, float sy, float ndx, float ndy)
+// A queued pair is first tested against the tighter per-pair band K|W| + K0 with the same fp32 arithmetic (bit-identical
+// X, Y, W, ex, ey: same operands and FMA nesting as score2).  Returns 1 = surely inlier, 0 = surely outlier, 2 = undecided.
+__device__ __forceinline__ unsigned recheck_f32(const HypConst& c, float sx, float sy, float ndx, float ndy)
 {
     const float X = __fmaf_rn(c.h[0], sx, __fmaf_rn(c.h[1], sy, c.h[2]));
     const float Y = __fmaf_rn(c.h[3], sx, __fmaf_rn(c.h[4], sy, c.h[5]));
     const float W = __fmaf_rn(c.h[6], sx, __fmaf_rn(c.h[7], sy, c.h[8]));
     const float ex = __fmaf_rn(ndx, W, X), ey = __fmaf_rn(ndy, W, Y);
-    const float w2 = __fmaf_rn(W, W, -K0);
+    const float w2 = __fmaf_rn(W, W, -c.K0);
     const float dp = __fmaf_rn(ey, ey, __fmaf_rn(ex, ex, -w2));          // diff + K0
     const float aw = fabsf(W);
-    if (__fmaf_rn(K, aw, dp) < 0.f) return 1u;                            // diff + (K|W| + K0) < 0
-    if (__fmaf_rn(K, aw, 2.0f * K0) - dp < 0.f) return 0u;                // (K|W| + K0) - diff < 0
+    if (__fmaf_rn(c.K, aw, dp) < 0.f) return 1u;                          // diff + (K|W| + K0) < 0
+    if (__fmaf_rn(c.K, aw, 2.0f * c.K0) - dp < 0.f) return 0u;            // (K|W| + K0) - diff < 0
     return 2u;
 }
 
-// G consecutive table entries (2G points) against one hypothesis.  `pt0` = index of the first point.
-// Fast path: 11 FFMA2 + 2 sign-bit adds + one 3-input unsigned min per entry; the cold branch is taken
-// by a warp only when one of its lanes has a pair inside the band.
-template <int G, bool ONLY_X>
-__device__ __forceinline__ void sweep_group(const HypConst& hc, const float4* __restrict__ tb, int pt0,
-                                            const SlowCtx& cx, unsigned& n_in, unsigned& n64)
+// Decide the `qn` queued pairs of this thread by the definition in fp64 (reading R9): re-derive the hypothesis (the same
+// deterministic fp64 solve as the set-up, so H is bit-identical).  Returns the number of inliers among them.
+__device__ __noinline__ unsigned drain_queue(SlowCtx& cx, unsigned qn)
+{
+    double s[8], d[8], Hn[9];
+    HypConst hc;
+    gather_sets(cx.src_xy, cx.dst_xy, cx.id, s, d);
+    make_hypothesis(s, d, cx.inv_t, cx.bounds, Hn, hc);
+    unsigned n = 0;
+    for (unsigned j = 0; j < qn; ++j) {
+        const int pt = static_cast<int>(cx.queue[j * kRBlock]);
+        const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
+        n += inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, cx.t) ? 1u : 0u;
+        ++cx.n64;
+    }
+    return n;
+}
+
+// Verification mode (HG_RANSAC_DECIDE_ALL_F64): every pair of points [p0, p1) by the fp64 definition.
+__device__ __noinline__ unsigned count_all_f64(SlowCtx& cx, int p0, int p1)
+{
+    double s[8], d[8], Hn[9];
+    HypConst hc;
+    gather_sets(cx.src_xy, cx.dst_xy, cx.id, s, d);
+    make_hypothesis(s, d, cx.inv_t, cx.bounds, Hn, hc);
+    unsigned c = 0;
+    for (int pt = p0; pt < p1; ++pt) {
+        const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
+        c += inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, cx.t) ? 1u : 0u;
+    }
+    cx.n64 += static_cast<unsigned>(p1 - p0);
+    return c;
+}
+
+// Queue overflow (more than kQueueCap undecided pairs for one hypothesis: a horizon line through the table, or data
+// sitting exactly on the threshold): the whole warp recounts lane L's hypothesis over points [p0, p1) -- every lane
+// re-derives that hypothesis (deterministic, so identical), takes every 32nd point, applies the per-pair band to the
+// sweep's own fp32 arithmetic and the fp64 definition to what stays undecided.  Returns the count (same on all lanes).
+__device__ __noinline__ unsigned recount_warp(SlowCtx& cx, int L, int p0, int p1)
+{
+    const int4 id = make_int4(__shfl_sync(0xffffffffu, cx.id.x, L), __shfl_sync(0xffffffffu, cx.id.y, L),
+                              __shfl_sync(0xffffffffu, cx.id.z, L), __shfl_sync(0xffffffffu, cx.id.w, L));
+    double s[8], d[8], Hn[9];
+    HypConst hc;
+    gather_sets(cx.src_xy, cx.dst_xy, id, s, d);
+    make_hypothesis(s, d, cx.inv_t, cx.bounds, Hn, hc);
+    const int lane = threadIdx.x & 31;
+    unsigned c = 0, n64 = 0;
+    for (int pt = p0 + lane; pt < p1; pt += 32) {
+        const float4 A = __ldg(cx.table + 2 * (pt >> 1)), B = __ldg(cx.table + 2 * (pt >> 1) + 1);
+        const bool hi = pt & 1;
+        unsigned r = recheck_f32(hc, hi ? A.y : A.x, hi ? A.w : A.z, hi ? B.y : B.x, hi ? B.w : B.z);
+        if (r == 2u) {
+            const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
+            r = inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, cx.t) ? 1u : 0u;
+            ++n64;
+        }
+        c += r;
+    }
+    c = __reduce_add_sync(0xffffffffu, c);
+    n64 = __reduce_add_sync(0xffffffffu, n64);
+    if (lane == L) cx.n64 += n64;
+    return c;
+}
+
+// Entry e of the table as the sweep sees it: CONST -> c_table (absolute float4 index), else shared memory.
+template <bool CONST>
+__device__ __forceinline__ float4 table_at(const float4* __restrict__ tb, int i) { return CONST ? c_table[i] : tb[i]; }
+
+// G consecutive table entries (2G points) against one hypothesis; the entries are float4 [i0, i0 + 2G) of the
+// table (`tb` in shared memory, or c_table when CONST).  `pt0` = index of the first point.
+// Fast path: 11 FFMA2 + 2 sign-bit adds + one 3-input unsigned min per entry; the cold branch (queue the pair) is
+// taken by a warp only when one of its lanes has a pair inside the band.
+template <int G, bool ONLY_X, bool CONST>
+__device__ __forceinline__ void sweep_group(const HypConst& hc, const float4* __restrict__ tb, int i0, int pt0,
+                                            SlowCtx& cx, unsigned& n_in, unsigned& qn, unsigned& n_band)
 {
     float2 a[G];
     bool amb = false;
 #pragma unroll
     for (int g = 0; g < G; ++g) {
-        const float4 A = tb[2 * g], B = tb[2 * g + 1];
+        const float4 A = table_at<CONST>(tb, i0 + 2 * g), B = table_at<CONST>(tb, i0 + 2 * g + 1);
         a[g] = score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w));
         n_in += sign_bit(a[g].x);
         amb |= (__float_as_uint(a[g].x) <= hc.thr);
@@ -294,22 +383,30 @@ __device__ __forceinline__ void sweep_group(const HypConst& hc, const float4* __
             mask |= (__float_as_uint(a[g].x) <= hc.thr) ? (1u << (2 * g)) : 0u;
             if (!ONLY_X) mask |= (__float_as_uint(a[g].y) <= hc.thr) ? (2u << (2 * g)) : 0u;
         }
-        const float K = cx.Ks[0], K0 = cx.Ks[kRBlock];
 #pragma unroll 1
         while (mask) {
             const int i = __ffs(mask) - 1;
             mask &= mask - 1u;
-            const float4 A = tb[i & ~1], B = tb[i | 1];       // entry g = i >> 1 lives at tb[2g], tb[2g + 1]
+            // entry g = i >> 1 lives at float4 i0 + 2g, i0 + 2g + 1 (a per-lane index: a plain LDC in CONST mode)
+            const float4 A = table_at<CONST>(tb, i0 + (i & ~1)), B = table_at<CONST>(tb, i0 + (i | 1));
             const bool hi = i & 1;
-            unsigned r = recheck_f32(hc, K, K0, hi ? A.y : A.x, hi ? A.w : A.z, hi ? B.y : B.x, hi ? B.w : B.z);
-            if (r == 2u) { r = resolve_pair_f64(cx, pt0 + i); ++n64; }
-            n_in += r;
+            const unsigned r = recheck_f32(hc, hi ? A.y : A.x, hi ? A.w : A.z, hi ? B.y : B.x, hi ? B.w : B.z);
+            ++n_band;
+            if (r == 2u) {
+                if (qn < kQueueCap) cx.queue[qn * kRBlock] = static_cast<unsigned>(pt0 + i);
+                ++qn;                                         // qn > kQueueCap: overflow, see the end of the sweep
+            } else {
+                n_in += r;
+            }
         }
     }
 }
 
+constexpr int kSyncEntries = 512;   // constant-bank path: table entries between CTA barriers (a multiple of kGroup)
 constexpr int kGroup = 8;     // table entries per cold-path check (8: +2 % over 4 on C4, measured)
 
+// CONST: the table is c_table (no staging, no table in shared memory); else it is staged from `table` (global).
+template <bool CONST>
 __global__ void __launch_bounds__(kRBlock, 2)
 ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts,
                     const float4* __restrict__ table, int n_pairs, HypSource hs,
@@ -317,10 +414,10 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
 {
     if (hs.check_stop && hdr->stop) return;                 // uniform: written by an earlier launch on this stream
     extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr size_t kStageBytes = CONST ? 0 : size_t(kStages) * kChunkPairs * 32;
     float4* stage_buf = reinterpret_cast<float4*>(smem_raw);                       // kStages * kChunkPairs * 2 float4
-    double* Hstash = reinterpret_cast<double*>(smem_raw + size_t(kStages) * kChunkPairs * 32);   // [9][kRBlock]
-    float* Kstash = reinterpret_cast<float*>(Hstash + 9 * kRBlock);                               // [2][kRBlock]
-    uint64_t* full = reinterpret_cast<uint64_t*>(Kstash + 2 * kRBlock);
+    unsigned* queue = reinterpret_cast<unsigned*>(smem_raw + kStageBytes);         // [kQueueCap][kRBlock]
+    uint64_t* full = reinterpret_cast<uint64_t*>(queue + kQueueCap * kRBlock);
 
     // Small hypothesis batches are split over the table as well (blockIdx.y = part), so that a call with a few
     // thousand hypotheses still fills the machine; this CTA sweeps entries [e_begin, e_end).
@@ -328,69 +425,108 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     const int e_end = min(n_pairs, e_begin + hs.part_entries);
     const bool split = gridDim.y > 1;
     const int n_chunks = (e_end - e_begin + kChunkPairs - 1) / kChunkPairs;
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
-        fence_barrier_init();
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int c = 0; c < kStages && c < n_chunks; ++c) {
-            const int first = e_begin + c * kChunkPairs;
-            const int pairs = min(kChunkPairs, e_end - first);
-            mbar_arrive_expect_tx(&full[c], pairs * 32u);
-            bulk_copy_g2s(stage_buf + size_t(c) * kChunkPairs * 2, table + size_t(first) * 2, pairs * 32u, &full[c]);
+    if (!CONST) {
+        if (threadIdx.x == 0) {
+            for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+            fence_barrier_init();
         }
-    }
-
-    // hypothesis set-up overlaps the first table copies
-    const int hidx = hs.h0 + blockIdx.x * kRBlock + threadIdx.x;
-    const bool active = hidx < hs.h1;
-    HypConst hc;
-    bool ok = false;
-    {
-        const float bounds[4] = { __uint_as_float(hdr->bound_bits[0]), __uint_as_float(hdr->bound_bits[1]),
-                                  __uint_as_float(hdr->bound_bits[2]), __uint_as_float(hdr->bound_bits[3]) };
-        double s[8], d[8], Hn[9];
-        const int4 id = active ? hypothesis_indices(hs, hidx, n_pts) : make_int4(0, 0, 0, 0);   // inactive: degenerate => sure outliers
-        if (active && hs.idx_out && blockIdx.y == 0) hs.idx_out[hidx] = id;
-        gather_sets(src_xy, dst_xy, id, s, d);
-        ok = make_hypothesis(s, d, inv_t, bounds, Hn, hc) && active;
-#pragma unroll
-        for (int k = 0; k < 9; ++k) Hstash[k * kRBlock + threadIdx.x] = Hn[k];
-        Kstash[threadIdx.x] = hc.K; Kstash[kRBlock + threadIdx.x] = hc.K0;
-    }
-    SlowCtx cx;
-    cx.Hs = Hstash + threadIdx.x; cx.Ks = Kstash + threadIdx.x; cx.src_xy = src_xy; cx.dst_xy = dst_xy; cx.t = t;
-
-    unsigned n_in = 0, n64 = 0;
-    const int full_pairs = n_pts >> 1;                     // entries holding two distinct points
-    for (int c = 0; c < n_chunks; ++c) {
-        const int st = c % kStages;
-        mbar_wait(&full[st], (c / kStages) & 1);
-        const float4* tb = stage_buf + size_t(st) * kChunkPairs * 2;
-        const int first = e_begin + c * kChunkPairs;
-        const int pairs = min(min(kChunkPairs, e_end - first), full_pairs - first);   // may be <= 0 in a tail-only chunk
-        int k = 0;
-#pragma unroll 1
-        for (; k + kGroup <= pairs; k += kGroup)
-            sweep_group<kGroup, false>(hc, tb + 2 * k, 2 * (first + k), cx, n_in, n64);
-#pragma unroll 1
-        for (; k < pairs; ++k)
-            sweep_group<1, false>(hc, tb + 2 * k, 2 * (first + k), cx, n_in, n64);
-        // odd tail point: the duplicated entry counts once
-        if ((n_pts & 1) && full_pairs >= first && full_pairs < min(first + kChunkPairs, e_end))
-            sweep_group<1, true>(hc, tb + 2 * (full_pairs - first), 2 * full_pairs, cx, n_in, n64);
-        if (c + kStages < n_chunks) {                      // refill this stage (uniform branch)
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                const int fn = e_begin + (c + kStages) * kChunkPairs;
-                const int pn = min(kChunkPairs, e_end - fn);
-                mbar_arrive_expect_tx(&full[st], pn * 32u);
-                bulk_copy_g2s(stage_buf + size_t(st) * kChunkPairs * 2, table + size_t(fn) * 2, pn * 32u, &full[st]);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int c = 0; c < kStages && c < n_chunks; ++c) {
+                const int first = e_begin + c * kChunkPairs;
+                const int pairs = min(kChunkPairs, e_end - first);
+                mbar_arrive_expect_tx(&full[c], pairs * 32u);
+                bulk_copy_g2s(stage_buf + size_t(c) * kChunkPairs * 2, table + size_t(first) * 2, pairs * 32u, &full[c]);
             }
         }
     }
 
+    // hypothesis set-up (overlaps the first table copies)
+    const long long hidx = hs.h0 + static_cast<long long>(blockIdx.x) * kRBlock + threadIdx.x;
+    const bool active = hidx < hs.h1;
+    HypConst hc;
+    SlowCtx cx;
+    bool ok = false;
+    {
+        cx.bounds[0] = __uint_as_float(hdr->bound_bits[0]); cx.bounds[1] = __uint_as_float(hdr->bound_bits[1]);
+        cx.bounds[2] = __uint_as_float(hdr->bound_bits[2]); cx.bounds[3] = __uint_as_float(hdr->bound_bits[3]);
+        double s[8], d[8], Hn[9];
+        cx.id = active ? hypothesis_indices(hs, hidx, n_pts) : make_int4(0, 0, 0, 0);   // inactive: degenerate => sure outliers
+        if (active && hs.idx_out && blockIdx.y == 0) hs.idx_out[hidx] = cx.id;
+        gather_sets(src_xy, dst_xy, cx.id, s, d);
+        ok = make_hypothesis(s, d, inv_t, cx.bounds, Hn, hc) && active;
+    }
+    cx.src_xy = src_xy; cx.dst_xy = dst_xy; cx.table = table; cx.inv_t = inv_t; cx.t = t;
+    cx.queue = queue + threadIdx.x; cx.n64 = 0u;
+
+    unsigned n_in = 0, qn = 0, n_band = 0;
+    const int full_pairs = n_pts >> 1;                     // entries holding two distinct points
+    if (hs.flags & HG_RANSAC_DECIDE_ALL_F64) {
+        // verification mode: no fp32 sweep, every pair of this part by the definition in fp64
+        const int p0 = 2 * e_begin, p1 = min(n_pts, 2 * e_end);
+        n_in = count_all_f64(cx, p0, p1);
+    } else if (CONST) {
+        const int e_two = min(e_end, full_pairs);          // entries [e_begin, e_two) hold two distinct points
+        int k = e_begin;
+        // Windows of kSyncEntries entries with a CTA barrier in between: the warps of a CTA drift apart (cold-path
+        // excursions), and the constant cache serves the uniform loads well only while they walk the table together
+        // (C4: 1.68 ms without the barriers, 1.62 ms with a window of 512 or 1024 entries, 1.63 ms with 256).
+#pragma unroll 1
+        for (int w_end = e_begin; k + kGroup <= e_two; ) {
+            w_end = min(e_two, w_end + kSyncEntries);
+#pragma unroll 1
+            for (; k + kGroup <= w_end; k += kGroup)
+                sweep_group<kGroup, false, true>(hc, nullptr, 2 * k, 2 * k, cx, n_in, qn, n_band);
+            if (w_end < e_two) __syncthreads();
+            else break;
+        }
+#pragma unroll 1
+        for (; k < e_two; ++k)
+            sweep_group<1, false, true>(hc, nullptr, 2 * k, 2 * k, cx, n_in, qn, n_band);
+        if ((n_pts & 1) && full_pairs >= e_begin && full_pairs < e_end)         // odd tail point: counts once
+            sweep_group<1, true, true>(hc, nullptr, 2 * full_pairs, 2 * full_pairs, cx, n_in, qn, n_band);
+    } else {
+        for (int c = 0; c < n_chunks; ++c) {
+            const int st = c % kStages;
+            mbar_wait(&full[st], (c / kStages) & 1);
+            const float4* tb = stage_buf + size_t(st) * kChunkPairs * 2;
+            const int first = e_begin + c * kChunkPairs;
+            const int pairs = min(min(kChunkPairs, e_end - first), full_pairs - first);   // may be <= 0 in a tail-only chunk
+            int k = 0;
+#pragma unroll 1
+            for (; k + kGroup <= pairs; k += kGroup)
+                sweep_group<kGroup, false, false>(hc, tb, 2 * k, 2 * (first + k), cx, n_in, qn, n_band);
+#pragma unroll 1
+            for (; k < pairs; ++k)
+                sweep_group<1, false, false>(hc, tb, 2 * k, 2 * (first + k), cx, n_in, qn, n_band);
+            // odd tail point: the duplicated entry counts once
+            if ((n_pts & 1) && full_pairs >= first && full_pairs < min(first + kChunkPairs, e_end))
+                sweep_group<1, true, false>(hc, tb, 2 * (full_pairs - first), 2 * full_pairs, cx, n_in, qn, n_band);
+            if (c + kStages < n_chunks) {                      // refill this stage (uniform branch)
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    const int fn = e_begin + (c + kStages) * kChunkPairs;
+                    const int pn = min(kChunkPairs, e_end - fn);
+                    mbar_arrive_expect_tx(&full[st], pn * 32u);
+                    bulk_copy_g2s(stage_buf + size_t(st) * kChunkPairs * 2, table + size_t(fn) * 2, pn * 32u, &full[st]);
+                }
+            }
+        }
+    }
+
+    // The queued pairs, all lanes of the warp together.  A hypothesis with more than kQueueCap undecided pairs is instead
+    // recounted from scratch by the whole warp.
+    if (__any_sync(0xffffffffu, qn != 0u)) {
+        unsigned ovf = __ballot_sync(0xffffffffu, qn > kQueueCap);
+        if (qn != 0u && qn <= kQueueCap) n_in += drain_queue(cx, qn);
+        while (ovf) {                                       // warp-uniform
+            const int L = __ffs(ovf) - 1;
+            ovf &= ovf - 1u;
+            const unsigned c = recount_warp(cx, L, 2 * e_begin, min(n_pts, 2 * e_end));
+            if ((threadIdx.x & 31) == L) n_in = c;
+        }
+    }
+    const unsigned n64 = active ? cx.n64 : 0u;
     const unsigned count = ok ? n_in : 0u;
     if (split) {                                            // partial count; ransac_best_kernel finishes the job
         if (active && count) atomicAdd(hs.acc + hidx, static_cast<int>(count));
@@ -405,6 +541,7 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     }
     // statistics: hypotheses that needed fp64 decisions, and how many pairs
     const unsigned amb_mask = __ballot_sync(0xffffffffu, n64 != 0u);
+    const unsigned band_tot = __reduce_add_sync(0xffffffffu, active ? n_band : 0u);
     if (amb_mask) {
         const unsigned tot = __reduce_add_sync(0xffffffffu, n64);
         if ((threadIdx.x & 31) == 0) {
@@ -412,14 +549,16 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
             atomicAdd(&hdr->n_pairs_f64, static_cast<unsigned long long>(tot));
         }
     }
+    if (band_tot && (threadIdx.x & 31) == 0) atomicAdd(&hdr->n_band, static_cast<unsigned long long>(band_tot));
 }
 
 // ---- 2b. best (split mode): total counts of hypotheses [h0, h1) -> counts[] and the packed maximum --------
 __global__ void __launch_bounds__(256)
-ransac_best_kernel(const int* __restrict__ acc, int h0, int h1, int* __restrict__ counts, RansacHeader* __restrict__ hdr, int check_stop)
+ransac_best_kernel(const int* __restrict__ acc, long long h0, long long h1, int* __restrict__ counts, RansacHeader* __restrict__ hdr,
+                   int check_stop)
 {
     if (check_stop && hdr->stop) return;
-    const int h = h0 + blockIdx.x * 256 + threadIdx.x;
+    const long long h = h0 + static_cast<long long>(blockIdx.x) * 256 + threadIdx.x;
     unsigned long long key = 0ull;
     if (h < h1) {
         const int c = acc[h];
@@ -459,7 +598,7 @@ __global__ void ransac_finalize_kernel(const float2* __restrict__ src_xy, const 
     if (n_evaluated) *n_evaluated = static_cast<long long>(hdr->n_evaluated);
     if (best_H) {
         double s[8], d[8], H[9];
-        gather_sets(src_xy, dst_xy, hypothesis_indices(hs, static_cast<int>(idx), n_pts), s, d);
+        gather_sets(src_xy, dst_xy, hypothesis_indices(hs, static_cast<long long>(idx), n_pts), s, d);
         aca_solve<double>(s, d, H);
         normalise<double>(H, 2);
 #pragma unroll
@@ -501,11 +640,47 @@ extern "C" size_t hg_ransac_workspace_bytes(int32_t n_pts, int64_t n_hyp)
 
 namespace hg {
 
-// Shared by the two device entry points.  Sampling mode: hyp_idx == nullptr.  round_hyp == n_hyp and
+// The constant-bank copy of the table is the one piece of per-device state in the library.  Calls that use it are
+// ordered against each other: a call makes its stream wait for the event the previous user recorded after its last
+// scoring launch, then overwrites c_table.  Under stream capture no cross-stream ordering can be expressed (and
+// none is recorded): replays of a captured call must not overlap other RANSAC work on the same device.
+class ConstTableGuard {
+public:
+    explicit ConstTableGuard(cudaStream_t st) : st_(st), lock_(mutex())
+    {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { status_ = HG_ERR_CUDA; return; }
+        capturing_ = cs != cudaStreamCaptureStatusNone;
+        if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) { status_ = HG_ERR_CUDA; return; }
+        if (capturing_) return;
+        Slot& s = slots()[dev_];
+        if (!s.ev && cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming) != cudaSuccess) { status_ = HG_ERR_CUDA; return; }
+        if (s.used && cudaStreamWaitEvent(st, s.ev, 0) != cudaSuccess) status_ = HG_ERR_CUDA;
+    }
+    ~ConstTableGuard()
+    {
+        if (status_ != HG_OK || capturing_) return;
+        Slot& s = slots()[dev_];
+        if (cudaEventRecord(s.ev, st_) == cudaSuccess) s.used = true;
+    }
+    int status() const { return status_; }
+
+private:
+    static constexpr int kMaxDevices = 64;
+    struct Slot { cudaEvent_t ev = nullptr; bool used = false; };
+    static std::mutex& mutex() { static std::mutex m; return m; }
+    static Slot* slots() { static Slot s[kMaxDevices]; return s; }
+    cudaStream_t st_;
+    std::unique_lock<std::mutex> lock_;
+    int dev_ = -1, status_ = HG_OK;
+    bool capturing_ = false;
+};
+
+// Shared by the device entry points.  Sampling mode: hyp_idx == nullptr.  round_hyp == n_hyp and
 // confidence <= 0 give the single-launch behaviour of hg_ransac_hypothesize_score.
 static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, const int32_t* hyp_idx, int32_t* hyp_idx_out,
                       unsigned long long seed, int64_t n_hyp, int64_t round_hyp, float threshold_px, double confidence,
-                      bool adaptive, int32_t* counts, float* best_H, int64_t* best_index, int32_t* best_count,
+                      bool adaptive, unsigned flags, int32_t* counts, float* best_H, int64_t* best_index, int32_t* best_count,
                       int64_t* n_evaluated, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -528,25 +703,37 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
         ransac_prep_kernel<<<blocks, 256, 0, st>>>(s2, d2, n_pts, n_pairs, inv_t, table, hdr);
         if (launch_status() != HG_OK) return HG_ERR_CUDA;
     }
-    const size_t smem = size_t(kStages) * kChunkPairs * 32 + size_t(9) * kRBlock * sizeof(double) + size_t(2) * kRBlock * sizeof(float) +
-                        kStages * sizeof(uint64_t);
+    // Operand path: a table that fits the constant bank, scored by rounds that fill the machine without splitting the
+    // table, goes through the uniform datapath; the verification mode never reads the table.
+    const int64_t first_round = round_hyp < n_hyp ? round_hyp : n_hyp;
+    const bool use_const = n_pairs <= kConstPairs && !may_split(first_round) && !(flags & HG_RANSAC_DECIDE_ALL_F64);
+    const size_t stash = size_t(kQueueCap) * kRBlock * sizeof(unsigned) + kStages * sizeof(uint64_t);
+    const size_t smem = (use_const ? 0 : size_t(kStages) * kChunkPairs * 32) + stash;
+    auto* score = use_const ? ransac_score_kernel<true> : ransac_score_kernel<false>;
     // per call, not cached: the attribute belongs to the current device, and a process may drive several
-    if (cudaFuncSetAttribute(ransac_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
-        return HG_ERR_CUDA;
+    if (cudaFuncSetAttribute(score, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return HG_ERR_CUDA;
+    std::unique_ptr<ConstTableGuard> guard;
+    if (use_const) {
+        guard.reset(new ConstTableGuard(st));
+        if (guard->status() != HG_OK) return guard->status();
+        if (cudaMemcpyToSymbolAsync(c_table, table, size_t(n_pairs) * 32, 0, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+            return HG_ERR_CUDA;
+    }
     HypSource hs;
     hs.idx = reinterpret_cast<const int4*>(hyp_idx);
     hs.idx_out = reinterpret_cast<int4*>(hyp_idx_out);
     hs.seed = seed;
+    hs.flags = flags;
     hs.check_stop = adaptive ? 1 : 0;
     // split mode needs the accumulator, which the workspace holds only when the whole call is small (may_split(n_hyp))
     hs.acc = acc_bytes ? reinterpret_cast<int*>(ws + kHeaderBytes) : nullptr;
     for (int64_t h0 = 0; h0 < n_hyp; h0 += round_hyp) {
         const int64_t h1 = (h0 + round_hyp < n_hyp) ? h0 + round_hyp : n_hyp;
-        hs.h0 = static_cast<int>(h0); hs.h1 = static_cast<int>(h1);
-        hs.part_entries = hs.acc ? part_entries_for(n_pairs, h1 - h0) : n_pairs;
+        hs.h0 = h0; hs.h1 = h1;
+        hs.part_entries = (hs.acc && !use_const) ? part_entries_for(n_pairs, h1 - h0) : n_pairs;
         const unsigned parts = static_cast<unsigned>((n_pairs + hs.part_entries - 1) / hs.part_entries);
         const dim3 grid(static_cast<unsigned>((h1 - h0 + kRBlock - 1) / kRBlock), parts);
-        ransac_score_kernel<<<grid, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, hs, inv_t, t, counts, hdr);
+        score<<<grid, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, hs, inv_t, t, counts, hdr);
         if (launch_status() != HG_OK) return HG_ERR_CUDA;
         if (parts > 1) {
             const unsigned bb = static_cast<unsigned>((h1 - h0 + 255) / 256);
@@ -558,6 +745,7 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
             if (launch_status() != HG_OK) return HG_ERR_CUDA;
         }
     }
+    guard.reset();                                         // records "table free" on the stream
     if (best_H || best_index || best_count || n_evaluated) {
         ransac_finalize_kernel<<<1, 32, 0, st>>>(s2, d2, n_pts, hs, hdr, best_H, reinterpret_cast<long long*>(best_index), best_count,
                                                  reinterpret_cast<long long*>(n_evaluated));
@@ -566,18 +754,30 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     return HG_OK;
 }
 
+static int check_options(const hg_ransac_options_t* o, unsigned* flags)
+{
+    *flags = 0u;
+    if (!o) return HG_OK;
+    if (o->flags & ~(HG_RANSAC_REJECT_DEGENERATE | HG_RANSAC_DECIDE_ALL_F64)) return HG_ERR_INVALID_ARG;
+    *flags = o->flags;
+    return HG_OK;
+}
+
 }  // namespace hg
 
-extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy, int32_t n_pts,
-                                           const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
-                                           int32_t* counts, float* best_H, int64_t* best_index,
-                                           int32_t* best_count, void* workspace, size_t workspace_bytes,
-                                           void* cuda_stream)
+extern "C" int hg_ransac_hypothesize_score_ex(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                                              const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
+                                              const hg_ransac_options_t* options,
+                                              int32_t* counts, float* best_H, int64_t* best_index,
+                                              int32_t* best_count, void* workspace, size_t workspace_bytes,
+                                              void* cuda_stream)
 {
     using namespace hg;
+    unsigned flags = 0u;
     if (n_hyp < 0 || n_hyp > 0x7fffffffLL) return HG_ERR_INVALID_ARG;
     if (n_pts < 4) return HG_ERR_INVALID_ARG;
     if (!(threshold_px > 0.0f) || !(threshold_px < 3.0e38f)) return HG_ERR_INVALID_ARG;
+    if (check_options(options, &flags) != HG_OK) return HG_ERR_INVALID_ARG;
     if (n_hyp == 0) return HG_OK;
     if (!src_xy || !dst_xy || !hyp_idx || !workspace) return HG_ERR_INVALID_ARG;
     if (!aligned16(src_xy) || !aligned16(dst_xy) || !aligned16(hyp_idx) || !aligned16(workspace)) return HG_ERR_ALIGNMENT;
@@ -585,20 +785,33 @@ extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst
         (best_index && (reinterpret_cast<uintptr_t>(best_index) & 7u)) || (best_count && !aligned4(best_count)))
         return HG_ERR_ALIGNMENT;
     if (workspace_bytes < hg_ransac_workspace_bytes(n_pts, n_hyp)) return HG_ERR_WORKSPACE;
-    return ransac_run(src_xy, dst_xy, n_pts, hyp_idx, nullptr, 0ull, n_hyp, n_hyp, threshold_px, 0.0, false, counts, best_H,
+    return ransac_run(src_xy, dst_xy, n_pts, hyp_idx, nullptr, 0ull, n_hyp, n_hyp, threshold_px, 0.0, false, flags, counts, best_H,
                       best_index, best_count, nullptr, workspace, workspace_bytes, cuda_stream);
 }
 
-extern "C" int hg_ransac_adaptive(const float* src_xy, const float* dst_xy, int32_t n_pts, uint64_t seed, int64_t max_hyp,
-                                  int64_t round_hyp, float threshold_px, float confidence, int32_t* counts,
-                                  int32_t* hyp_idx_out, float* best_H, int64_t* best_index, int32_t* best_count,
-                                  int64_t* n_evaluated, void* workspace, size_t workspace_bytes, void* cuda_stream)
+extern "C" int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                                           const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
+                                           int32_t* counts, float* best_H, int64_t* best_index,
+                                           int32_t* best_count, void* workspace, size_t workspace_bytes,
+                                           void* cuda_stream)
+{
+    return hg_ransac_hypothesize_score_ex(src_xy, dst_xy, n_pts, hyp_idx, n_hyp, threshold_px, nullptr, counts, best_H, best_index,
+                                          best_count, workspace, workspace_bytes, cuda_stream);
+}
+
+extern "C" int hg_ransac_adaptive_ex(const float* src_xy, const float* dst_xy, int32_t n_pts, uint64_t seed, int64_t max_hyp,
+                                     int64_t round_hyp, float threshold_px, float confidence,
+                                     const hg_ransac_options_t* options, int32_t* counts,
+                                     int32_t* hyp_idx_out, float* best_H, int64_t* best_index, int32_t* best_count,
+                                     int64_t* n_evaluated, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     using namespace hg;
+    unsigned flags = 0u;
     if (max_hyp < 0 || max_hyp > 0x7fffffffLL || round_hyp < 1) return HG_ERR_INVALID_ARG;
     if (n_pts < 4) return HG_ERR_INVALID_ARG;
     if (!(threshold_px > 0.0f) || !(threshold_px < 3.0e38f)) return HG_ERR_INVALID_ARG;
     if (!(confidence < 1.0f) || !(confidence == confidence)) return HG_ERR_INVALID_ARG;
+    if (check_options(options, &flags) != HG_OK) return HG_ERR_INVALID_ARG;
     if (max_hyp == 0) return HG_OK;
     if ((max_hyp + round_hyp - 1) / round_hyp > 65536) return HG_ERR_INVALID_ARG;          // launches per call
     if (!src_xy || !dst_xy || !workspace) return HG_ERR_INVALID_ARG;
@@ -609,8 +822,17 @@ extern "C" int hg_ransac_adaptive(const float* src_xy, const float* dst_xy, int3
         return HG_ERR_ALIGNMENT;
     if (workspace_bytes < hg_ransac_workspace_bytes(n_pts, max_hyp)) return HG_ERR_WORKSPACE;
     return ransac_run(src_xy, dst_xy, n_pts, nullptr, hyp_idx_out, seed, max_hyp, round_hyp, threshold_px,
-                      static_cast<double>(confidence), true, counts, best_H, best_index, best_count, n_evaluated, workspace,
+                      static_cast<double>(confidence), true, flags, counts, best_H, best_index, best_count, n_evaluated, workspace,
                       workspace_bytes, cuda_stream);
+}
+
+extern "C" int hg_ransac_adaptive(const float* src_xy, const float* dst_xy, int32_t n_pts, uint64_t seed, int64_t max_hyp,
+                                  int64_t round_hyp, float threshold_px, float confidence, int32_t* counts,
+                                  int32_t* hyp_idx_out, float* best_H, int64_t* best_index, int32_t* best_count,
+                                  int64_t* n_evaluated, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    return hg_ransac_adaptive_ex(src_xy, dst_xy, n_pts, seed, max_hyp, round_hyp, threshold_px, confidence, nullptr, counts,
+                                 hyp_idx_out, best_H, best_index, best_count, n_evaluated, workspace, workspace_bytes, cuda_stream);
 }
 
 extern "C" int hg_ransac_hypothesize_score_host(const float* src_xy, const float* dst_xy, int32_t n_pts,

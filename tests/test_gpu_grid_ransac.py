@@ -117,8 +117,11 @@ def check_ransac(wl, t, out, ref):
     return diff
 
 
+# operand paths of the score kernel: fewer than 148 x 512 hypotheses -> table split over blockIdx.y, staged in shared
+# memory; more, with <= 4096 points -> constant bank / uniform datapath; more points -> shared-memory stages, no split
 @pytest.mark.parametrize("n_pts,n_hyp,t", [(4096, 6000, 3.0), (1001, 5000, 3.0), (100, 777, 1.5),
-                                           (4, 1, 3.0), (2500, 3000, 0.75), (9000, 1500, 3.0)])
+                                           (4, 1, 3.0), (2500, 3000, 0.75), (9000, 1500, 3.0),
+                                           (1001, 80000, 3.0), (4095, 76000, 1.0), (17, 75776, 3.0), (9001, 76000, 3.0)])
 def test_ransac_counts_match_oracle(n_pts, n_hyp, t):
     wl = W.ransac_workload(n_pts=n_pts, n_hyp=n_hyp, seed=W.SEED_BASE + 4 + n_pts)
     out = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV), t)
@@ -167,6 +170,48 @@ def test_ransac_full_config4_every_hypothesis():
     assert int(out["best_count"].item()) >= 0.6 * 0.7 * 4096
     print("C4 every hypothesis: counts differing (all inside the band)", int((diff > 0).sum()), "of", 1 << 20,
           "hypotheses with in-band pairs", int((ref["band_counts"] > 0).sum()), hg.ransac_stats(out["workspace"]))
+
+
+@pytest.mark.parametrize("n_pts,n_hyp,t,scale", [(4096, 1 << 20, 3.0, 1.0),        # C4 in full, constant-bank path
+                                                 (2001, 100000, 0.5, 1.0),          # odd table, tight threshold
+                                                 (1000, 4096, 3.0, 1.0),            # split shared-memory path
+                                                 (6001, 80000, 3.0, 1.0),           # staged shared-memory path
+                                                 (1500, 90000, 3e6, 1e6)])          # coordinates x 1e6: the band scales
+def test_ransac_fp32_sweep_equals_fp64_decisions(n_pts, n_hyp, t, scale):
+    """The claim of DESIGN.md section 7, pinned directly: the fp32 sweep with its error band gives the SAME counts as
+    deciding every pair by the definition in fp64 from the kernel's own fp64 H (HG_RANSAC_DECIDE_ALL_F64).  Bit-exact:
+    no oracle, no H rounding between the two sides -- only the band is under test."""
+    wl = W.ransac_workload(n_pts=n_pts, n_hyp=n_hyp, seed=W.SEED_BASE + 90 + n_pts)
+    s, d, idx = (wl["src_xy"] * scale).to(DEV), (wl["dst_xy"] * scale).to(DEV), wl["hyp_idx"].to(DEV)
+    fast = hg.hg_ransac_hypothesize_score(s, d, idx, t)
+    slow = hg.hg_ransac_hypothesize_score(s, d, idx, t, decide_all_f64=True)
+    assert torch.equal(fast["counts"], slow["counts"])
+    assert fast["best_index"].item() == slow["best_index"].item() and fast["best_count"].item() == slow["best_count"].item()
+    assert torch.equal(fast["best_H"], slow["best_H"])
+    st = hg.ransac_stats(slow["workspace"])
+    assert st["n_pairs_f64"] == n_pts * n_hyp                                  # the slow side really decided every pair in fp64
+    print(n_pts, n_hyp, "fast path fp64 decisions:", hg.ransac_stats(fast["workspace"])["n_pairs_f64"], "of", n_pts * n_hyp)
+
+
+def test_ransac_pairs_exactly_at_the_threshold():
+    """Adversarial for the band: dst = src for half the points (so hypotheses drawn from them give H = identity up to fp64
+    rounding) and dst = src + (t, 0) for the other half -- residual t (1 +- 1e-16), every such pair lies inside any band.
+    The sweep must hand all of them to the fp64 decision and agree with the all-fp64 mode bit for bit."""
+    n_pts, n_hyp, t = 1200, 80000, 2.0
+    g = torch.Generator().manual_seed(7)
+    s = torch.rand((n_pts, 2), generator=g) * 600.0
+    d = s.clone()
+    d[n_pts // 2:, 0] += t
+    idx = torch.stack([torch.randperm(n_pts // 2, generator=g)[:4] for _ in range(n_hyp // 100)]).repeat(100, 1).to(torch.int32)
+    fast = hg.hg_ransac_hypothesize_score(s.to(DEV), d.to(DEV), idx.to(DEV), t)
+    slow = hg.hg_ransac_hypothesize_score(s.to(DEV), d.to(DEV), idx.to(DEV), t, decide_all_f64=True)
+    assert torch.equal(fast["counts"], slow["counts"])
+    assert (fast["counts"] >= n_pts // 2).all()
+    st = hg.ransac_stats(fast["workspace"])
+    assert st["n_pairs_f64"] >= 0.4 * n_pts * n_hyp                          # the at-threshold half went to the cold path
+    ref = oracle.ransac(s.numpy(), d.numpy(), idx.numpy()[:2000], t, band_rel=1e-4)
+    diff = np.abs(fast["counts"].cpu().numpy()[:2000].astype(np.int64) - ref["counts"])
+    assert (diff <= ref["band_counts"]).all()
 
 
 def test_ransac_degenerate_and_non_finite_inputs():

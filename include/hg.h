@@ -143,8 +143,9 @@ HG_API int hg_offsets_to_grid(const float* offsets, float x0, float y0, float w,
  *   H       : nullable, float[n][3][3] per `norm`
  * Errors: HG_ERR_INVALID_ARG (NULL with n > 0, sizes < 1, w == 0 or h == 0, bad enum),
  * HG_ERR_ALIGNMENT (offsets not 16-byte aligned; image, warped, H not 4-byte aligned), HG_ERR_CUDA.
- * When the item's image (all channels) is at most 110 KB and 16-byte aligned it is staged in shared memory
- * by one bulk-async copy per CTA; larger images are gathered through L1.
+ * An image plane of up to about 160 x 160 pixels is staged in shared memory inside a frame of zeros, one CTA per
+ * (item, channel) -- by bulk-async row copies when img_w % 4 == 0 and `image` is 16-byte aligned, by plain loads
+ * otherwise; larger planes are gathered through L1.
  * -------------------------------------------------------------------------------------------- */
 HG_API int hg_offsets_to_warp(const float* offsets, float x0, float y0, float w, float h,
                        int32_t out_w, int32_t out_h, const float* image, int32_t channels,

@@ -137,7 +137,8 @@ offsets_to_h_kernel(const float* __restrict__ offsets, RectParams rp, float* __r
 // sampling grid never reaches HBM.  Lanes map to adjacent pixels of a row, so the four bilinear taps
 // of a warp fall into one or two lines each and every store instruction writes a full line.
 // Zero padding: a tap outside the image contributes 0; a non-finite position gives 0.
-// blockIdx.x = item, blockIdx.y = band of rows.  Per pixel and channel: 4 B read + 4 B written.
+// Per pixel and channel: 4 B read + 4 B written.  Two kernels: the gather form below for image planes too large
+// for shared memory, and the staged form (offsets_to_warp_plane_kernel) for everything else.
 // ------------------------------------------------------------------------------------------
 struct WarpGeom { int out_w, out_h, img_w, img_h, channels, rows_per_band; };
 
@@ -165,19 +166,14 @@ __device__ __forceinline__ Taps make_taps(float u, float v, int img_w, int img_h
     return t;
 }
 
-// SMEM: the image plane was staged in shared memory (plain loads); otherwise global memory, read-only path.
-template <bool SMEM> __device__ __forceinline__ float px(const float* p) { return SMEM ? *p : __ldg(p); }
-
-template <bool SMEM>
+// Gather form (images too large to stage): taps read from global memory through the read-only path / L1.
 __device__ __forceinline__ float gather(const float* __restrict__ img, const Taps& t)
 {
-    return fmaf(t.w11, px<SMEM>(img + t.o11), fmaf(t.w10, px<SMEM>(img + t.o10),
-           fmaf(t.w01, px<SMEM>(img + t.o01), t.w00 * px<SMEM>(img + t.o00))));
+    return fmaf(t.w11, __ldg(img + t.o11), fmaf(t.w10, __ldg(img + t.o10),
+           fmaf(t.w01, __ldg(img + t.o01), t.w00 * __ldg(img + t.o00))));
 }
 
-// All four taps inside the image.  SMEM: `at` = shared-memory byte address of tap (0,0), row_bytes = 4 * img_w
-// (32-bit addressing, one LDS per tap); else `p` points at tap (0,0) in global memory.  Nested lerps: the same
-// bilinear form as gather() up to rounding.
+// All four taps inside the image, `p` points at tap (0,0).  Nested lerps: the same bilinear form as gather() up to rounding.
 __device__ __forceinline__ float lerp2(float a, float b, float c, float d, float fu, float fv)
 {
     const float top = fmaf(fu, b - a, a), bot = fmaf(fu, d - c, c);
@@ -187,11 +183,6 @@ __device__ __forceinline__ float lerp2(float a, float b, float c, float d, float
 __device__ __forceinline__ float lds_f32(uint32_t addr)
 { float v; asm("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr)); return v; }
 
-__device__ __forceinline__ float gather_interior_smem(uint32_t at, uint32_t row_bytes, float fu, float fv)
-{
-    return lerp2(lds_f32(at), lds_f32(at + 4u), lds_f32(at + row_bytes), lds_f32(at + row_bytes + 4u), fu, fv);
-}
-
 __device__ __forceinline__ float gather_interior_gmem(const float* __restrict__ p, int img_w, float fu, float fv)
 {
     return lerp2(__ldg(p), __ldg(p + 1), __ldg(p + img_w), __ldg(p + img_w + 1), fu, fv);
@@ -200,29 +191,14 @@ __device__ __forceinline__ float gather_interior_gmem(const float* __restrict__ 
 __device__ __forceinline__ float rcp_approx(float x)
 { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
-// CH = compile-time channel count (0: read it from the geometry).  SMEM: the item's image (all channels) is
-// staged in shared memory by bulk-async copies issued before the solve, so the HBM read is one deep transfer
-// per CTA instead of latency-bound gathers; used when the image fits (the host decides).
-template <int CH, bool SMEM>
-__global__ void __launch_bounds__(kGridBlock, SMEM ? 3 : 4)
+// CH = compile-time channel count (0: read it from the geometry).  blockIdx.x = item, blockIdx.y = band of rows.
+template <int CH>
+__global__ void __launch_bounds__(kGridBlock, CH == 0 ? 2 : 4)
 offsets_to_warp_kernel(const float* __restrict__ offsets, RectParams rp, WarpGeom g, int tx_count,
                        const float* __restrict__ image, float* __restrict__ warped, float* __restrict__ H_out, int norm)
 {
     __shared__ float hs[9];
-    __shared__ uint64_t img_bar;
-    extern __shared__ __align__(128) float img_s[];
     const int64_t b = blockIdx.x;
-    if (SMEM) {
-        if (threadIdx.x == 0) { mbar_init(&img_bar, 1); fence_barrier_init(); }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            const uint32_t bytes = static_cast<uint32_t>(g.channels) * g.img_w * g.img_h * 4u;
-            const char* src = reinterpret_cast<const char*>(image) + b * static_cast<int64_t>(bytes);
-            mbar_arrive_expect_tx(&img_bar, bytes);
-            for (uint32_t off = 0; off < bytes; off += 32768u)
-                bulk_copy_g2s(reinterpret_cast<char*>(img_s) + off, src + off, min(32768u, bytes - off), &img_bar);
-        }
-    }
     if (threadIdx.x < 32) {
         const float4* op = reinterpret_cast<const float4*>(offsets + 8 * b);
         const float4 o0 = __ldg(op), o1 = __ldg(op + 1);
@@ -270,23 +246,19 @@ offsets_to_warp_kernel(const float* __restrict__ offsets, RectParams rp, WarpGeo
     const int img_plane = img_w * img_h;
     const int out_plane = out_w * g.out_h;
     const float wm1 = static_cast<float>(img_w - 1), hm1 = static_cast<float>(img_h - 1);
-    const float* img_b = SMEM ? img_s : image + b * channels * static_cast<int64_t>(img_plane);
+    const float* img_b = image + b * channels * static_cast<int64_t>(img_plane);
     float* out_b = warped + b * channels * static_cast<int64_t>(out_plane);
     const int j_begin = blockIdx.y * g.rows_per_band;
     const int j_end = min(g.out_h, j_begin + g.rows_per_band);
-    if (SMEM) mbar_wait(&img_bar, 0);
-
-    const uint32_t img_base = SMEM ? smem_u32(img_s) : 0u;
-    const uint32_t row_bytes = 4u * static_cast<uint32_t>(img_w), plane_bytes = 4u * static_cast<uint32_t>(img_plane);
     const int64_t out_step = static_cast<int64_t>(rows_per_pass) * out_w;
 
     for (int i = tx; i < out_w; i += tx_count) {
         const float fi = static_cast<float>(i);
         const float cx = fmaf(l11, fi, l13), cy = fmaf(l21, fi, l23), cw = fmaf(l31, fi, l33);
         float* op_row = out_b + i + static_cast<int64_t>(j_begin + ty) * out_w;
-#pragma unroll 2
         float fj = static_cast<float>(j_begin + ty);
         const float fstep = static_cast<float>(rows_per_pass);
+#pragma unroll 2
         for (int j = j_begin + ty; j < j_end; j += rows_per_pass, op_row += out_step, fj += fstep) {
             const float X = fmaf(l12, fj, cx), Y = fmaf(l22, fj, cy), Wv = fmaf(l32, fj, cw);
             const float q = rcp_approx(Wv);
@@ -301,44 +273,184 @@ offsets_to_warp_kernel(const float* __restrict__ offsets, RectParams rp, WarpGeo
                 const float tu = __fadd_rn(__fadd_rn(u, -0.5f), 12582912.f), tv = __fadd_rn(__fadd_rn(v, -0.5f), 12582912.f);
                 const float fu = u - __fadd_rn(tu, -12582912.f), fv = v - __fadd_rn(tv, -12582912.f);
                 const int e = (__float_as_int(tv) - 0x4B400000) * img_w + (__float_as_int(tu) - 0x4B400000);
-                if (SMEM) {
-                    uint32_t at = img_base + 4u * static_cast<uint32_t>(e);
-                    if (CH > 0) {
+                const float* p = img_b + e;
+                if (CH > 0) {
 #pragma unroll
-                        for (int c = 0; c < CH; ++c) { __stcs(op, gather_interior_smem(at, row_bytes, fu, fv)); at += plane_bytes; op += out_plane; }
-                    } else {
-                        for (int c = 0; c < channels; ++c) { __stcs(op, gather_interior_smem(at, row_bytes, fu, fv)); at += plane_bytes; op += out_plane; }
-                    }
+                    for (int c = 0; c < CH; ++c) { __stcs(op, gather_interior_gmem(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
                 } else {
-                    const float* p = img_b + e;
-                    if (CH > 0) {
-#pragma unroll
-                        for (int c = 0; c < CH; ++c) { __stcs(op, gather_interior_gmem(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
-                    } else {
-                        for (int c = 0; c < channels; ++c) { __stcs(op, gather_interior_gmem(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
-                    }
+                    for (int c = 0; c < channels; ++c) { __stcs(op, gather_interior_gmem(p, img_w, fu, fv)); p += img_plane; op += out_plane; }
                 }
             } else {
                 const Taps t = make_taps(u, v, img_w, img_h);
                 const float* ip = img_b;
                 if (CH > 0) {
 #pragma unroll
-                    for (int c = 0; c < CH; ++c) { __stcs(op, gather<SMEM>(ip, t)); ip += img_plane; op += out_plane; }
+                    for (int c = 0; c < CH; ++c) { __stcs(op, gather(ip, t)); ip += img_plane; op += out_plane; }
                 } else {
-                    for (int c = 0; c < channels; ++c) { __stcs(op, gather<SMEM>(ip, t)); ip += img_plane; op += out_plane; }
+                    for (int c = 0; c < channels; ++c) { __stcs(op, gather(ip, t)); ip += img_plane; op += out_plane; }
                 }
             }
         }
     }
 }
 
-template <int CH, bool SMEM>
-static int launch_warp(dim3 grid, size_t smem, cudaStream_t st, const float* offsets, const RectParams& rp, const WarpGeom& g,
+// ------------------------------------------------------------------------------------------
+// The staged form of the same operation: one CTA per (item, channel[, band of rows]).  The image plane is staged in
+// shared memory inside a frame of zeros (2 rows above, 3 below, >= 4 columns left and right), and the pixel position
+// is produced already normalised to that frame, so that one saturating multiply clamps it and the zero frame IS the
+// zero padding of reading R17: no interior test, no tap selection, no branch in the pixel loop.
+//   rows of H:  U = (u + 2) / (img_w + 3), V = (v + 2) / (img_h + 3) are folded into rows 1-2 in fp64
+//   per pixel:  (X', Y') = FFMA2,  W = FFMA,  q = rcp(W),  U, V = sat(X' q), sat(Y' q)      -- u in [-2, w + 1]
+//               (k + M)  = FFMA2.RM(UV, scale, M - 2)     round-down: k = floor(u) exactly, in the low mantissa bits
+//               (k + 2)  = FADD2 (exact),   (fu, fv) = FFMA2(UV, scale, -(k + 2))           -- fu in [0, 1]
+//               address = IMAD + LEA,  4 x LDS,  lerp = FADD2 + FFMA2 + FADD + FFMA,  STG
+// about 24 issued instructions per pixel against 63 for the gather form above (profiles/r02_summary.md).
+// Non-finite positions saturate to 0 (NaN) or to a frame corner (inf): zero, as R17 asks.
+// ------------------------------------------------------------------------------------------
+struct PlaneGeom {
+    int out_w, out_h, img_w, img_h, channels, bands, rows_per_band;
+    int stride;            // floats per staged row: 4 + img_w + right pad, a multiple of 4
+    int bulk;              // 1: rows are copied by cp.async.bulk (16-byte rules hold), 0: by plain loads
+};
+
+constexpr int kFrameTop = 2, kFrameBottom = 3, kFrameLeft = 4;
+constexpr float kFloorMagic = 12582912.f;      // 1.5 * 2^23
+
+__global__ void __launch_bounds__(kGridBlock, 3)
+offsets_to_warp_plane_kernel(const float* __restrict__ offsets, RectParams rp, PlaneGeom g, int tx_count,
+                             const float* __restrict__ image, float* __restrict__ warped, float* __restrict__ H_out, int norm)
+{
+    __shared__ float hs[9];
+    __shared__ uint64_t img_bar;
+    extern __shared__ __align__(128) float img_s[];
+    const int64_t b = blockIdx.x;
+    const int c = blockIdx.y / g.bands, band = blockIdx.y - c * g.bands;
+    const int stride = g.stride, img_w = g.img_w, img_h = g.img_h;
+    const float* plane = image + (b * g.channels + c) * static_cast<int64_t>(img_w) * img_h;
+    const uint32_t row_bytes = 4u * static_cast<uint32_t>(img_w);
+
+    if (threadIdx.x == 0 && g.bulk) {
+        mbar_init(&img_bar, 1);
+        fence_barrier_init();
+        mbar_arrive_expect_tx(&img_bar, row_bytes * static_cast<uint32_t>(img_h));
+    }
+    // the zero frame: whole rows above and below, pads left and right of every image row
+    for (int r = threadIdx.x; r < (kFrameTop + kFrameBottom) * (stride >> 2); r += kGridBlock) {
+        const int fr = r / (stride >> 2), q4 = r - fr * (stride >> 2);
+        const int row = fr < kFrameTop ? fr : img_h + fr;              // 0, 1, img_h + 2, img_h + 3, img_h + 4
+        reinterpret_cast<float4*>(img_s + row * stride)[q4] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    const int right = stride - kFrameLeft - img_w;                     // >= 4
+    for (int r = threadIdx.x; r < img_h * (kFrameLeft + right); r += kGridBlock) {
+        const int y = r / (kFrameLeft + right), k = r - y * (kFrameLeft + right);
+        img_s[(y + kFrameTop) * stride + (k < kFrameLeft ? k : img_w + k)] = 0.f;
+    }
+    __syncthreads();
+    if (g.bulk) {
+        for (int y = threadIdx.x; y < img_h; y += kGridBlock)
+            bulk_copy_g2s(img_s + (y + kFrameTop) * stride + kFrameLeft, plane + static_cast<int64_t>(y) * img_w, row_bytes, &img_bar);
+    } else {
+        for (int e = threadIdx.x; e < img_w * img_h; e += kGridBlock) {
+            const int y = e / img_w, x = e - y * img_w;
+            img_s[(y + kFrameTop) * stride + kFrameLeft + x] = __ldg(plane + e);
+        }
+    }
+    if (threadIdx.x < 32) {
+        const float4* op = reinterpret_cast<const float4*>(offsets + 8 * b);
+        const float4 o0 = __ldg(op), o1 = __ldg(op + 1);
+        double s[8], d[8], Hd[9];
+        corners_from_offsets(rp, o0, o1, s, d);
+        aca_solve<double>(s, d, Hd);
+        double m = 0.0;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) m = fmax(m, fabs(Hd[k]));
+        const double r = K<double>::rcp(m);
+        if (H_out != nullptr && blockIdx.y == 0) {
+            double Hn[9];
+#pragma unroll
+            for (int k = 0; k < 9; ++k) Hn[k] = Hd[k] * r;
+            normalise<double>(Hn, norm);
+            if (norm == 0) {
+#pragma unroll
+                for (int k = 0; k < 9; ++k) Hn[k] = Hd[k];
+            }
+            if (threadIdx.x == 0) {
+#pragma unroll
+                for (int k = 0; k < 9; ++k) H_out[9 * b + k] = static_cast<float>(Hn[k]);
+            }
+        }
+        if (threadIdx.x == 0) {
+            // L = H * [sx 0 x0; 0 sy y0; 0 0 1] (the lattice), then rows 1-2 -> frame-normalised coordinates
+            double L[9];
+#pragma unroll
+            for (int row = 0; row < 3; ++row) {
+                const double a = Hd[3 * row] * r, bb = Hd[3 * row + 1] * r, cc = Hd[3 * row + 2] * r;
+                L[3 * row] = a * rp.step_x; L[3 * row + 1] = bb * rp.step_y; L[3 * row + 2] = fma(a, rp.x0, fma(bb, rp.y0, cc));
+            }
+            const double iu = 1.0 / (img_w + 3.0), iv = 1.0 / (img_h + 3.0);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                hs[k]     = static_cast<float>((L[k] + 2.0 * L[6 + k]) * iu);
+                hs[3 + k] = static_cast<float>((L[3 + k] + 2.0 * L[6 + k]) * iv);
+                hs[6 + k] = static_cast<float>(L[6 + k]);
+            }
+        }
+    }
+    __syncthreads();
+    const float l11 = hs[0], l12 = hs[1], l13 = hs[2];
+    const float l21 = hs[3], l22 = hs[4], l23 = hs[5];
+    const float l31 = hs[6], l32 = hs[7], l33 = hs[8];
+
+    const int tx = threadIdx.x & (tx_count - 1);
+    const int ty = threadIdx.x / tx_count;
+    const int rows_per_pass = kGridBlock / tx_count;
+    const int out_w = g.out_w;
+    float* out_p = warped + (b * g.channels + c) * static_cast<int64_t>(out_w) * g.out_h;
+    const int j_begin = band * g.rows_per_band;
+    const int j_end = min(g.out_h, j_begin + g.rows_per_band);
+    const float2 scale = make_float2(static_cast<float>(img_w + 3), static_cast<float>(img_h + 3));
+    const float2 L2 = make_float2(l12, l22);
+    // frame element of sample index (ku, kv): (kv + 2) * stride + (ku + 4); the floor trick leaves k + 0x4B400000
+    const uint32_t base = smem_u32(img_s) + 4u * static_cast<uint32_t>(kFrameTop * stride + kFrameLeft)
+                          - 4u * (0x4B400000u * static_cast<uint32_t>(stride) + 0x4B400000u);
+    const uint32_t sbytes = 4u * static_cast<uint32_t>(stride);
+    if (g.bulk) mbar_wait(&img_bar, 0);
+    else        __syncthreads();
+
+    for (int i = tx; i < out_w; i += tx_count) {
+        const float fi = static_cast<float>(i);
+        const float2 C2 = make_float2(fmaf(l11, fi, l13), fmaf(l21, fi, l23));
+        const float cw = fmaf(l31, fi, l33);
+        float* op = out_p + i + static_cast<int64_t>(j_begin + ty) * out_w;
+        const int64_t out_step = static_cast<int64_t>(rows_per_pass) * out_w;
+        float fj = static_cast<float>(j_begin + ty);
+        const float fstep = static_cast<float>(rows_per_pass);
+#pragma unroll 4
+        for (int j = j_begin + ty; j < j_end; j += rows_per_pass, op += out_step, fj += fstep) {
+            const float2 P = __ffma2_rn(L2, make_float2(fj, fj), C2);
+            const float Wv = fmaf(l32, fj, cw);
+            const float q = rcp_approx(Wv);
+            float2 UV;
+            asm("mul.rn.sat.f32 %0, %1, %2;" : "=f"(UV.x) : "f"(P.x), "f"(q));
+            asm("mul.rn.sat.f32 %0, %1, %2;" : "=f"(UV.y) : "f"(P.y), "f"(q));
+            const float2 T = __ffma2_rd(UV, scale, make_float2(kFloorMagic - 2.f, kFloorMagic - 2.f));
+            const float2 R = __fadd2_rn(T, make_float2(2.f - kFloorMagic, 2.f - kFloorMagic));
+            const float2 F = __ffma2_rn(UV, scale, make_float2(-R.x, -R.y));
+            const uint32_t at = base + 4u * (__float_as_uint(T.y) * static_cast<uint32_t>(stride) + __float_as_uint(T.x));
+            const float2 ac = make_float2(lds_f32(at), lds_f32(at + sbytes));
+            const float2 bd = make_float2(lds_f32(at + 4u), lds_f32(at + sbytes + 4u));
+            const float2 D = __fadd2_rn(bd, make_float2(-ac.x, -ac.y));
+            const float2 TB = __ffma2_rn(make_float2(F.x, F.x), D, ac);              // (top, bottom)
+            __stcs(op, fmaf(F.y, TB.y - TB.x, TB.x));
+        }
+    }
+}
+
+template <int CH>
+static int launch_warp(dim3 grid, cudaStream_t st, const float* offsets, const RectParams& rp, const WarpGeom& g,
                        int tx_count, const float* image, float* warped, float* H, int norm)
 {
-    if (SMEM && cudaFuncSetAttribute(offsets_to_warp_kernel<CH, SMEM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     int(kWarpStageBytes)) != cudaSuccess) return HG_ERR_CUDA;
-    offsets_to_warp_kernel<CH, SMEM><<<grid, kGridBlock, smem, st>>>(offsets, rp, g, tx_count, image, warped, H, norm);
+    offsets_to_warp_kernel<CH><<<grid, kGridBlock, 0, st>>>(offsets, rp, g, tx_count, image, warped, H, norm);
     return launch_status();
 }
 
@@ -413,16 +525,30 @@ extern "C" int hg_offsets_to_warp(const float* offsets, float x0, float y0, floa
     g.rows_per_band = (out_h + bands - 1) / bands;
     bands = (out_h + g.rows_per_band - 1) / g.rows_per_band;
     const dim3 grid(static_cast<unsigned>(n), static_cast<unsigned>(bands));
-    // Stage the item's image in shared memory when two CTAs fit on an SM and the bulk copy's 16-byte rules hold.
-    const size_t img_bytes = size_t(channels) * img_w * img_h * sizeof(float);
-    const bool staged = img_bytes <= kWarpStageBytes && img_bytes % 16 == 0 && aligned16(image);
-    const int nm = int(norm);
-    if (staged) {
-        if (channels == 1) return launch_warp<1, true>(grid, img_bytes, st, offsets, rp, g, tx_count, image, warped, H, nm);
-        if (channels == 3) return launch_warp<3, true>(grid, img_bytes, st, offsets, rp, g, tx_count, image, warped, H, nm);
-        return launch_warp<0, true>(grid, img_bytes, st, offsets, rp, g, tx_count, image, warped, H, nm);
+    // Staged form: one image plane per CTA inside a zero frame, when at least two such CTAs fit on an SM.
+    {
+        int stride = kFrameLeft + ((img_w + 3) & ~3) + 4;
+        if (stride % 32 == 0) stride += 4;                              // rows must not start in the same bank
+        const size_t plane_bytes = size_t(img_h + kFrameTop + kFrameBottom) * stride * sizeof(float);
+        if (plane_bytes <= kWarpStageBytes && int64_t(channels) * out_h <= 65535) {
+            PlaneGeom pg;
+            pg.out_w = out_w; pg.out_h = out_h; pg.img_w = img_w; pg.img_h = img_h; pg.channels = channels;
+            // rows are split into bands only while the batch alone cannot fill the machine
+            int pb = 1;
+            while (n * channels * pb < 3 * 148 && (out_h + pb - 1) / pb > rows_per_pass) pb *= 2;
+            pg.rows_per_band = (out_h + pb - 1) / pb;
+            pg.bands = (out_h + pg.rows_per_band - 1) / pg.rows_per_band;
+            pg.stride = stride;
+            pg.bulk = (img_w % 4 == 0 && aligned16(image)) ? 1 : 0;
+            if (cudaFuncSetAttribute(offsets_to_warp_plane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     int(kWarpStageBytes)) != cudaSuccess) return HG_ERR_CUDA;
+            const dim3 pgrid(static_cast<unsigned>(n), static_cast<unsigned>(channels * pg.bands));
+            offsets_to_warp_plane_kernel<<<pgrid, kGridBlock, plane_bytes, st>>>(offsets, rp, pg, tx_count, image, warped, H, int(norm));
+            return launch_status();
+        }
     }
-    if (channels == 1) return launch_warp<1, false>(grid, 0, st, offsets, rp, g, tx_count, image, warped, H, nm);
-    if (channels == 3) return launch_warp<3, false>(grid, 0, st, offsets, rp, g, tx_count, image, warped, H, nm);
-    return launch_warp<0, false>(grid, 0, st, offsets, rp, g, tx_count, image, warped, H, nm);
+    const int nm = int(norm);
+    if (channels == 1) return launch_warp<1>(grid, st, offsets, rp, g, tx_count, image, warped, H, nm);
+    if (channels == 3) return launch_warp<3>(grid, st, offsets, rp, g, tx_count, image, warped, H, nm);
+    return launch_warp<0>(grid, st, offsets, rp, g, tx_count, image, warped, H, nm);
 }

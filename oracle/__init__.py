@@ -197,8 +197,20 @@ def offsets_to_warp(offsets, x0: float, y0: float, w: float, h: float, out_w: in
     return out
 
 
-def ransac(src_xy, dst_xy, hyp_idx, threshold: float, band_rel: float = 1e-4, solver: int = METHOD_ACA):
-    """Returns dict(counts int32 [n_hyp], band_counts, best_H [3,3] normal form, best_index, best_count)."""
+def sample_check(src_xy, dst_xy, hyp_idx, min_area: float = 0.0) -> np.ndarray:
+    """Reading R20: bool [n_hyp], True where the 4-point sample is rejected (degenerate on either plane within
+    min_area px^2, or a triangle's orientation not preserved)."""
+    s = _f32(src_xy, (2,)); d = _f32(dst_xy, (2,))
+    idx = np.ascontiguousarray(np.asarray(hyp_idx), dtype=np.int32).reshape(-1, 4)
+    out = np.zeros(idx.shape[0], dtype=np.uint8)
+    lib().hgo_sample_check(_p(s), _p(d), _p(idx), ctypes.c_int64(idx.shape[0]), ctypes.c_double(float(np.float32(min_area))), _p(out))
+    return out.astype(bool)
+
+
+def ransac(src_xy, dst_xy, hyp_idx, threshold: float, band_rel: float = 1e-4, solver: int = METHOD_ACA,
+           reject_degenerate: bool = False, min_area: float = 0.0):
+    """Returns dict(counts int32 [n_hyp], band_counts, best_H [3,3] normal form, best_index, best_count).
+    reject_degenerate: samples rejected by reading R20 (min_area in px^2) score 0."""
     s = _f32(src_xy, (2,)); d = _f32(dst_xy, (2,))
     idx = np.ascontiguousarray(np.asarray(hyp_idx), dtype=np.int32).reshape(-1, 4)
     n_pts, n_hyp = s.shape[0], idx.shape[0]
@@ -210,10 +222,11 @@ def ransac(src_xy, dst_xy, hyp_idx, threshold: float, band_rel: float = 1e-4, so
     best_H = np.full((3, 3), np.nan, dtype=np.float64)
     best_index = ctypes.c_int64(-1)
     best_count = ctypes.c_int32(-1)
-    lib().hgo_ransac(_p(s), _p(d), ctypes.c_int32(n_pts), _p(idx), ctypes.c_int64(n_hyp),
-                     ctypes.c_double(float(np.float32(threshold))), ctypes.c_double(band_rel),
-                     ctypes.c_int(1 if solver == METHOD_ACA else 0),
-                     _p(counts), _p(band), _p(best_H), ctypes.byref(best_index), ctypes.byref(best_count))
+    lib().hgo_ransac_opt(_p(s), _p(d), ctypes.c_int32(n_pts), _p(idx), ctypes.c_int64(n_hyp),
+                         ctypes.c_double(float(np.float32(threshold))), ctypes.c_double(band_rel),
+                         ctypes.c_int(1 if solver == METHOD_ACA else 0),
+                         ctypes.c_double(float(np.float32(min_area)) if reject_degenerate else -1.0),
+                         _p(counts), _p(band), _p(best_H), ctypes.byref(best_index), ctypes.byref(best_count))
     return {"counts": counts, "band_counts": band, "best_H": best_H,
             "best_index": int(best_index.value), "best_count": int(best_count.value)}
 
@@ -232,7 +245,7 @@ def ransac_sample(seed: int, h0: int, n: int, n_pts: int) -> np.ndarray:
 
 
 def ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, threshold: float, confidence: float,
-                    band_rel: float = 1e-4):
+                    band_rel: float = 1e-4, reject_degenerate: bool = False, min_area: float = 0.0):
     """Sampling + rounds + adaptive termination (reading R19).  Returns dict(n_evaluated, hyp_idx [n_evaluated,4],
     counts, band_counts, best_H, best_index, best_count, margins [rounds])."""
     s = _f32(src_xy, (2,)); d = _f32(dst_xy, (2,))
@@ -245,7 +258,8 @@ def ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, thr
     bi, bc, ne = ctypes.c_int64(-1), ctypes.c_int32(-1), ctypes.c_int64(0)
     lib().hgo_ransac_adaptive(_p(s), _p(d), ctypes.c_int32(n_pts), ctypes.c_uint64(seed), ctypes.c_int64(max_hyp),
                               ctypes.c_int64(round_hyp), ctypes.c_double(float(np.float32(threshold))),
-                              ctypes.c_double(float(np.float32(confidence))), ctypes.c_double(band_rel), _p(idx), _p(counts),
+                              ctypes.c_double(float(np.float32(confidence))), ctypes.c_double(band_rel),
+                              ctypes.c_double(float(np.float32(min_area)) if reject_degenerate else -1.0), _p(idx), _p(counts),
                               _p(band), _p(best_H), ctypes.byref(bi), ctypes.byref(bc), ctypes.byref(ne), _p(margins))
     n = int(ne.value)
     return {"n_evaluated": n, "hyp_idx": idx[:n], "counts": counts[:n], "band_counts": band[:n], "best_H": best_H,

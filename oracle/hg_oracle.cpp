@@ -281,10 +281,41 @@ void hgo_offsets_to_warp(const float* offsets, float x0, float y0, float w, floa
 //   counts[h]      = #{ k : r_k <= t },  r_k = forward transfer residual in fp64, W == 0 -> outlier
 //   band_counts[h] = #{ k : |r_k - t| <= band_rel * t }   (the allowance of north_star)
 //   best: max count, ties -> lowest hypothesis index; best_H = that H in normal form.
+// Reading R20: reject flags of the 4-point samples (1 = rejected).
+void hgo_sample_check(const float* src_xy, const float* dst_xy, const int32_t* hyp_idx, int64_t n_hyp,
+                      double min_area, uint8_t* rejected)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t hI = 0; hI < n_hyp; ++hI) {
+        double s[8], d[8];
+        for (int k = 0; k < 4; ++k) {
+            const int32_t j = hyp_idx[4 * hI + k];
+            s[2 * k] = src_xy[2 * j];     s[2 * k + 1] = src_xy[2 * j + 1];
+            d[2 * k] = dst_xy[2 * j];     d[2 * k + 1] = dst_xy[2 * j + 1];
+        }
+        rejected[hI] = hgo::sample_rejected(s, d, min_area) ? 1 : 0;
+    }
+}
+
+// reject_min_area < 0: no sample check (reading R9); >= 0: samples rejected by reading R20 score 0.
+void hgo_ransac_opt(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                    const int32_t* hyp_idx, int64_t n_hyp, double t, double band_rel, int solver,
+                    double reject_min_area, int32_t* counts, int32_t* band_counts,
+                    double* best_H, int64_t* best_index, int32_t* best_count);
+
 void hgo_ransac(const float* src_xy, const float* dst_xy, int32_t n_pts,
                 const int32_t* hyp_idx, int64_t n_hyp, double t, double band_rel, int solver,
                 int32_t* counts, int32_t* band_counts,
                 double* best_H, int64_t* best_index, int32_t* best_count)
+{
+    hgo_ransac_opt(src_xy, dst_xy, n_pts, hyp_idx, n_hyp, t, band_rel, solver, -1.0, counts, band_counts, best_H, best_index,
+                   best_count);
+}
+
+void hgo_ransac_opt(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                    const int32_t* hyp_idx, int64_t n_hyp, double t, double band_rel, int solver,
+                    double reject_min_area, int32_t* counts, int32_t* band_counts,
+                    double* best_H, int64_t* best_index, int32_t* best_count)
 {
 #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t hI = 0; hI < n_hyp; ++hI) {
@@ -295,8 +326,9 @@ void hgo_ransac(const float* src_xy, const float* dst_xy, int32_t n_pts,
             d[2 * k] = dst_xy[2 * j];     d[2 * k + 1] = dst_xy[2 * j + 1];
         }
         bool good = true;
-        if (solver == 0) good = hgo::dlt_ge(s, d, H);
-        else             hgo::aca<double>(s, d, H);
+        if (reject_min_area >= 0.0 && hgo::sample_rejected(s, d, reject_min_area)) good = false;
+        else if (solver == 0) good = hgo::dlt_ge(s, d, H);
+        else                  hgo::aca<double>(s, d, H);
         int32_t c = 0, bc = 0;
         if (good) {
             for (int32_t k = 0; k < n_pts; ++k) {
@@ -343,7 +375,7 @@ void hgo_ransac_sample(uint64_t seed, int64_t h0, int64_t n, int32_t n_pts, int3
 // n_evaluated are left untouched); margins[r] = s after round r (NaN when not computed).
 void hgo_ransac_adaptive(const float* src_xy, const float* dst_xy, int32_t n_pts, uint64_t seed,
                          int64_t max_hyp, int64_t round_hyp, double t, double confidence, double band_rel,
-                         int32_t* idx_out, int32_t* counts, int32_t* band_counts, double* best_H,
+                         double reject_min_area, int32_t* idx_out, int32_t* counts, int32_t* band_counts, double* best_H,
                          int64_t* best_index, int32_t* best_count, int64_t* n_evaluated, double* margins)
 {
     int64_t bi = -1, done = 0, round = 0;
@@ -353,8 +385,8 @@ void hgo_ransac_adaptive(const float* src_xy, const float* dst_xy, int32_t n_pts
         hgo_ransac_sample(seed, done, m, n_pts, idx_out + 4 * done);
         int64_t rbi = -1;
         int32_t rbc = -1;
-        hgo_ransac(src_xy, dst_xy, n_pts, idx_out + 4 * done, m, t, band_rel, 1, counts + done,
-                   band_counts ? band_counts + done : nullptr, nullptr, &rbi, &rbc);
+        hgo_ransac_opt(src_xy, dst_xy, n_pts, idx_out + 4 * done, m, t, band_rel, 1, reject_min_area, counts + done,
+                       band_counts ? band_counts + done : nullptr, nullptr, &rbi, &rbc);
         if (rbc > bc) { bc = rbc; bi = done + rbi; }          // ties keep the lowest index
         done += m;
         double s = NAN;

@@ -414,6 +414,41 @@ inline double transfer_residual(const double H[9], double x, double y, double u,
 }
 
 // ---------------------------------------------------------------------------
+// Sample check of the hypothesise-and-verify loop (reading R20).
+// The paper names what a degenerate minimal sample is -- three of the four points collinear, or two of them
+// the same ("both of which are degenerate configurations") -- but gives no test; R20 fixes one:
+//   A_ijk = (p_j - p_i) x (p_k - p_i)   (twice the signed area of triangle i,j,k), for the four triangles
+//   (0,1,2), (0,1,3), (0,2,3), (1,2,3) of the source quadruple and of the target quadruple;
+//   reject  iff  some |A_ijk| <= 2 * min_area on either plane            (degenerate)
+//            or  sign(A_ijk(source)) != sign(A_ijk(target)) for some triangle   (H would have to send part of
+//                the quadruple through its line at infinity, or mirror the plane: not a view of that plane).
+// Arithmetic: coordinates are fp32 values promoted to fp64; every difference, product and the final subtraction is
+// one IEEE fp64 operation, in exactly this order (the comparison is a decision: both sides of a parity test take
+// it in the same precision).  Returns true when the sample is REJECTED.
+// ---------------------------------------------------------------------------
+inline double signed_area2(const double* p, int i, int j, int k)
+{
+    const double ux = p[2 * j] - p[2 * i], uy = p[2 * j + 1] - p[2 * i + 1];
+    const double vx = p[2 * k] - p[2 * i], vy = p[2 * k + 1] - p[2 * i + 1];
+    const double a = ux * vy;
+    const double b = uy * vx;
+    return a - b;
+}
+
+inline bool sample_rejected(const double s[8], const double d[8], double min_area)
+{
+    static const int tri[4][3] = { {0, 1, 2}, {0, 1, 3}, {0, 2, 3}, {1, 2, 3} };
+    const double lim = 2.0 * min_area;
+    for (int t = 0; t < 4; ++t) {
+        const double a1 = signed_area2(s, tri[t][0], tri[t][1], tri[t][2]);
+        const double a2 = signed_area2(d, tri[t][0], tri[t][1], tri[t][2]);
+        if (!(std::fabs(a1) > lim) || !(std::fabs(a2) > lim)) return true;     // also rejects NaN
+        if ((a1 > 0.0) != (a2 > 0.0)) return true;
+    }
+    return false;
+}
+
+// ---------------------------------------------------------------------------
 // Scalar type that counts arithmetic the way the paper does:
 // add / sub / mul = 1 FLOP, division = 4 FLOPs.  Unary minus is free.
 // ---------------------------------------------------------------------------

@@ -171,3 +171,112 @@ def test_grid_degenerate_sizes():
     assert np.abs(g[:, 0, 0] - off[:, 0].astype(np.float64)).max() <= 1e-9   # pixel (x0,y0) -> TL + offset
     H2, none = oracle.offsets_to_grid(off, 0.0, 0.0, 127.0, 127.0, 128, 128, want_grid=False)
     assert none is None and np.array_equal(H, H2)
+
+
+# ---- reading R20: the sample check (degenerate configurations of P:786 + orientation) -----------------------------
+def _area2_int(p, i, j, k):
+    return (p[j][0] - p[i][0]) * (p[k][1] - p[i][1]) - (p[j][1] - p[i][1]) * (p[k][0] - p[i][0])
+
+
+def _rejected_by_definition(src, dst, lim2):
+    """R20 written out on exact integers: lim2 = 2 * min_area."""
+    for tri in ((0, 1, 2), (0, 1, 3), (0, 2, 3), (1, 2, 3)):
+        a1, a2 = _area2_int(src, *tri), _area2_int(dst, *tri)
+        if abs(a1) <= lim2 or abs(a2) <= lim2:
+            return True
+        if (a1 > 0) != (a2 > 0):
+            return True
+    return False
+
+
+def test_sample_check_brute_force_on_integer_points():
+    """Every 4-subset (in 3 different orders each) of a small seeded integer table, against the definition evaluated with
+    Python integers (exact): same flags, same number of rejections."""
+    import itertools, random
+    rng = random.Random(20)
+    n = 14
+    src = [(rng.randint(-9, 9), rng.randint(-9, 9)) for _ in range(n)]
+    dst = [(rng.randint(-9, 9), rng.randint(-9, 9)) for _ in range(n)]
+    dst[:7] = [(2 * x - y + 3, x + 3 * y - 1) for x, y in src[:7]]          # an orientation-preserving affine map on half the table
+    quads = []
+    for q in itertools.combinations(range(n), 4):
+        quads += [q, (q[2], q[0], q[3], q[1]), (q[3], q[2], q[1], q[0])]
+    idx = np.array(quads, dtype=np.int32)
+    for min_area in (0.0, 1.0, 7.5):
+        want = np.array([_rejected_by_definition([src[i] for i in q], [dst[i] for i in q], 2 * min_area) for q in quads])
+        got = oracle.sample_check(np.array(src, np.float32), np.array(dst, np.float32), idx, min_area)
+        assert np.array_equal(got, want), (min_area, int((got != want).sum()))
+        assert 0 < want.sum() < len(quads)
+    # the planted affine half: accepted whenever the source quadruple itself is non-degenerate
+    acc = [q for q in quads if max(q) < 7 and not _rejected_by_definition([src[i] for i in q], [dst[i] for i in q], 0)]
+    assert len(acc) > 20
+
+
+def test_sample_check_planted_cases_and_invariances():
+    rect = np.array([[0, 0], [40, 0], [40, 30], [0, 30]], dtype=np.float32)
+    import itertools
+    perms = np.array(list(itertools.permutations(range(4))), dtype=np.int32)
+    # all 24 orders of a rectangle mapped onto a translated, scaled copy of itself (same order): accepted
+    assert not oracle.sample_check(rect, rect * 1.5 + 7.0, perms).any()
+    assert oracle.sample_check(rect, rect * 1.5 + 7.0, perms, min_area=601.0).all()           # every triangle has area 600
+    assert not oracle.sample_check(rect, rect * 1.5 + 7.0, perms, min_area=599.0).any()
+    # mirrored target: all four orientations flip -> rejected; two target points swapped: mixed -> rejected
+    mirror = rect * np.array([-1.0, 1.0], dtype=np.float32)
+    assert oracle.sample_check(rect, mirror, perms).all()
+    twisted = rect[[0, 2, 1, 3]]
+    assert oracle.sample_check(rect, twisted, perms).all()
+    # three collinear points / two coincident points on either plane
+    col = np.array([[0, 0], [10, 10], [20, 20], [5, 30]], dtype=np.float32)
+    dup = np.array([[0, 0], [40, 0], [40, 0], [0, 30]], dtype=np.float32)
+    base = np.arange(4, dtype=np.int32)[None]
+    assert oracle.sample_check(col, rect, base)[0] and oracle.sample_check(rect, col, base)[0]
+    assert oracle.sample_check(dup, rect, base)[0] and oracle.sample_check(rect, dup, base)[0]
+    nan = rect.copy(); nan[2, 0] = np.nan
+    assert oracle.sample_check(nan, rect, base)[0]
+    # invariances: the same permutation on both planes, exchanging the planes, a common translation
+    s, d = W.general_sets(4096, seed=31)
+    s, d = s.numpy().reshape(-1, 2), d.numpy().reshape(-1, 2)
+    d[::3] = d[::3][:, ::-1]                                                  # make a third of the sets inconsistent
+    idx = np.arange(4 * 4096, dtype=np.int32).reshape(-1, 4)
+    f0 = oracle.sample_check(s, d, idx, 50.0)
+    assert 0.2 < f0.mean() < 0.9
+    assert np.array_equal(f0, oracle.sample_check(s, d, idx[:, [2, 0, 3, 1]], 50.0))
+    assert np.array_equal(f0, oracle.sample_check(d, s, idx, 50.0))
+
+
+def test_sample_check_means_w_keeps_one_sign():
+    """What the orientation rule says about H (pins it against the homography itself, computed by the DLT oracle):
+    sign(A_dst) = sign(det H) * sign(W_i W_j W_k) * sign(A_src) for every triangle, so all four orientations are
+    preserved iff W has one sign on the four source points and det(H) * W^3 > 0."""
+    s, d = W.general_sets(1 << 13, seed=41)
+    s, d = s.numpy().copy(), d.numpy().copy()
+    rng = np.random.default_rng(3)
+    k = rng.integers(0, 4, size=s.shape[0])
+    bad = rng.random(s.shape[0]) < 0.5
+    d[bad, k[bad]] = rng.random((int(bad.sum()), 2)).astype(np.float32) * np.array([640.0, 480.0], dtype=np.float32)   # an outlier
+    idx = np.arange(4 * s.shape[0], dtype=np.int32).reshape(-1, 4)
+    rej = oracle.sample_check(s.reshape(-1, 2), d.reshape(-1, 2), idx, 0.0)
+    H, ok = oracle.solve(oracle.METHOD_DLT, s, d, return_ok=True)
+    x = np.concatenate([s.astype(np.float64), np.ones(s.shape[:2] + (1,))], axis=-1)
+    Wk = np.einsum("nj,nkj->nk", H[:, 2, :], x)
+    same = (np.sign(Wk) == np.sign(Wk[:, :1])).all(axis=1)
+    keeps = same & (np.linalg.det(H) * Wk[:, 0] > 0)
+    # compare away from the decision boundary (|W| tiny or a nearly collinear triple): there the two must agree exactly
+    clear = ok & (np.abs(Wk).min(axis=1) > 1e-6 * np.abs(Wk).max(axis=1))
+    assert clear.mean() > 0.95
+    assert np.array_equal(~rej[clear], keeps[clear])
+    assert 0.2 < rej.mean() < 0.8
+
+
+def test_ransac_with_sample_check_scores_rejected_hypotheses_zero():
+    wl = W.ransac_workload(n_pts=300, n_hyp=2000, seed=9)
+    s, d, idx = wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy()
+    plain = oracle.ransac(s, d, idx, 3.0)
+    chk = oracle.ransac(s, d, idx, 3.0, reject_degenerate=True, min_area=25.0)
+    rej = oracle.sample_check(s, d, idx, 25.0)
+    assert 0.1 < rej.mean() < 0.9
+    assert (chk["counts"][rej] == 0).all() and (chk["band_counts"][rej] == 0).all()
+    assert np.array_equal(chk["counts"][~rej], plain["counts"][~rej])
+    assert chk["best_count"] == chk["counts"].max() and not rej[chk["best_index"]]
+    # all-inlier samples are never rejected for a small epsilon: the best model survives
+    assert chk["best_count"] >= 0.9 * plain["best_count"]

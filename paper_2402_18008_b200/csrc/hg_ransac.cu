@@ -94,6 +94,30 @@ __device__ __forceinline__ void gather_sets(const float2* __restrict__ src_xy, c
     }
 }
 
+// ---- sample check (reading R20; degenerate configurations P:786) ---------------------------------
+// Twice the signed area of triangle (i, j, k); one IEEE operation per difference, product and subtraction (no FMA
+// contraction): the comparison below is a decision, taken in the same arithmetic as the oracle's.
+__device__ __forceinline__ double signed_area2(const double p[8], int i, int j, int k)
+{
+    const double ux = __dsub_rn(p[2 * j], p[2 * i]), uy = __dsub_rn(p[2 * j + 1], p[2 * i + 1]);
+    const double vx = __dsub_rn(p[2 * k], p[2 * i]), vy = __dsub_rn(p[2 * k + 1], p[2 * i + 1]);
+    return __dsub_rn(__dmul_rn(ux, vy), __dmul_rn(uy, vx));
+}
+
+// true: reject.  Some triangle of the source or target quadruple has area <= min_area (lim2 = 2 * min_area), or a
+// triangle's orientation differs between the planes.
+__device__ __forceinline__ bool sample_rejected(const double s[8], const double d[8], double lim2)
+{
+    bool rej = false;
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+        const int i = t == 3 ? 1 : 0, j = t < 2 ? 1 : 2, k = t == 0 ? 2 : 3;           // (0,1,2) (0,1,3) (0,2,3) (1,2,3)
+        const double a1 = signed_area2(s, i, j, k), a2 = signed_area2(d, i, j, k);
+        rej = rej || !(fabs(a1) > lim2) || !(fabs(a2) > lim2) || ((a1 > 0.0) != (a2 > 0.0));
+    }
+    return rej;
+}
+
 // ---- where the hypotheses of a launch come from ----------------------------------------------
 struct HypSource {
     const int4* idx;            // caller-supplied indices [n_hyp][4], or nullptr: sample on the device
@@ -101,6 +125,7 @@ struct HypSource {
     unsigned long long seed;    // sampling mode
     long long h0, h1;           // this launch scores hypotheses [h0, h1)
     unsigned flags;             // HG_RANSAC_* option bits
+    double reject_lim2;         // HG_RANSAC_REJECT_DEGENERATE: 2 * min_area_px2
     int check_stop;             // 1: return at once when hdr->stop is set (adaptive termination)
     int part_entries;           // table entries per blockIdx.y part (a multiple of 8); >= n_pairs: no split
     int* acc;                   // split mode: partial counts are added here (zeroed before the launch)
@@ -442,8 +467,8 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     }
 
     // hypothesis set-up (overlaps the first table copies)
-    const long long hidx = hs.h0 + static_cast<long long>(blockIdx.x) * kRBlock + threadIdx.x;
-    const bool active = hidx < hs.h1;
+    long long hidx = hs.h0 + static_cast<long long>(blockIdx.x) * kRBlock + threadIdx.x;
+    bool active = hidx < hs.h1;
     HypConst hc;
     SlowCtx cx;
     bool ok = false;
@@ -454,8 +479,51 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
         cx.id = active ? hypothesis_indices(hs, hidx, n_pts) : make_int4(0, 0, 0, 0);   // inactive: degenerate => sure outliers
         if (active && hs.idx_out && blockIdx.y == 0) hs.idx_out[hidx] = cx.id;
         gather_sets(src_xy, dst_xy, cx.id, s, d);
+        if (hs.flags & HG_RANSAC_REJECT_DEGENERATE) {
+            // Reading R20.  A rejected hypothesis scores 0 at once; the accepted ones are compacted onto the first threads
+            // of the CTA, so that whole warps fall idle and skip the sweep (the queue area is free until the sweep starts).
+            __shared__ unsigned warp_accepted[kRBlock / 32];
+            int4* ids = reinterpret_cast<int4*>(queue);                                   // [kRBlock]
+            unsigned* owners = queue + 4 * kRBlock;                                       // [kRBlock]
+            const bool accept = active && !sample_rejected(s, d, hs.reject_lim2);
+            const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
+            const unsigned bal = __ballot_sync(0xffffffffu, accept);
+            if (active && !accept) {
+                if (!split && counts) counts[hidx] = 0;
+            }
+            {   // rejected hypotheses still take part in the argmax with count 0; statistics
+                unsigned long long key = (active && !accept && !split) ? pack_key(0u, static_cast<unsigned>(hidx)) : 0ull;
+                key = warp_max_u64(key);
+                const unsigned nrej = __popc(__ballot_sync(0xffffffffu, active && !accept));
+                if (lane == 0) {
+                    if (key != 0ull) atomicMax(&hdr->best_key, key);
+                    if (nrej && blockIdx.y == 0) atomicAdd(&hdr->n_rejected, static_cast<unsigned long long>(nrej));
+                    warp_accepted[wid] = __popc(bal);
+                }
+            }
+            __syncthreads();
+            unsigned before = 0, total = 0;
+#pragma unroll
+            for (unsigned w = 0; w < kRBlock / 32; ++w) { const unsigned c = warp_accepted[w]; before += (w < wid) ? c : 0u; total += c; }
+            if (accept) {
+                const unsigned rank = before + __popc(bal & ((1u << lane) - 1u));
+                ids[rank] = cx.id;
+                owners[rank] = threadIdx.x;
+            }
+            __syncthreads();
+            active = threadIdx.x < total;
+            if (active) {
+                cx.id = ids[threadIdx.x];
+                hidx = hs.h0 + static_cast<long long>(blockIdx.x) * kRBlock + owners[threadIdx.x];
+            } else {
+                cx.id = make_int4(0, 0, 0, 0);
+            }
+            __syncthreads();                                                              // the queue area is reused by the sweep
+            gather_sets(src_xy, dst_xy, cx.id, s, d);
+        }
         ok = make_hypothesis(s, d, inv_t, cx.bounds, Hn, hc) && active;
     }
+    const bool warp_live = __any_sync(0xffffffffu, active);    // a warp without hypotheses skips the sweep (not the barriers)
     cx.src_xy = src_xy; cx.dst_xy = dst_xy; cx.table = table; cx.inv_t = inv_t; cx.t = t;
     cx.queue = queue + threadIdx.x; cx.n64 = 0u;
 
@@ -464,7 +532,7 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     if (hs.flags & HG_RANSAC_DECIDE_ALL_F64) {
         // verification mode: no fp32 sweep, every pair of this part by the definition in fp64
         const int p0 = 2 * e_begin, p1 = min(n_pts, 2 * e_end);
-        n_in = count_all_f64(cx, p0, p1);
+        if (active) n_in = count_all_f64(cx, p0, p1);
     } else if (CONST) {
         const int e_two = min(e_end, full_pairs);          // entries [e_begin, e_two) hold two distinct points
         int k = e_begin;
@@ -474,17 +542,23 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
 #pragma unroll 1
         for (int w_end = e_begin; k + kGroup <= e_two; ) {
             w_end = min(e_two, w_end + kSyncEntries);
+            if (warp_live) {
 #pragma unroll 1
-            for (; k + kGroup <= w_end; k += kGroup)
-                sweep_group<kGroup, false, true>(hc, nullptr, 2 * k, 2 * k, cx, n_in, qn, n_band);
+                for (; k + kGroup <= w_end; k += kGroup)
+                    sweep_group<kGroup, false, true>(hc, nullptr, 2 * k, 2 * k, cx, n_in, qn, n_band);
+            } else {
+                k += (w_end - k) / kGroup * kGroup;
+            }
             if (w_end < e_two) __syncthreads();
             else break;
         }
+        if (warp_live) {
 #pragma unroll 1
-        for (; k < e_two; ++k)
-            sweep_group<1, false, true>(hc, nullptr, 2 * k, 2 * k, cx, n_in, qn, n_band);
-        if ((n_pts & 1) && full_pairs >= e_begin && full_pairs < e_end)         // odd tail point: counts once
-            sweep_group<1, true, true>(hc, nullptr, 2 * full_pairs, 2 * full_pairs, cx, n_in, qn, n_band);
+            for (; k < e_two; ++k)
+                sweep_group<1, false, true>(hc, nullptr, 2 * k, 2 * k, cx, n_in, qn, n_band);
+            if ((n_pts & 1) && full_pairs >= e_begin && full_pairs < e_end)     // odd tail point: counts once
+                sweep_group<1, true, true>(hc, nullptr, 2 * full_pairs, 2 * full_pairs, cx, n_in, qn, n_band);
+        }
     } else {
         for (int c = 0; c < n_chunks; ++c) {
             const int st = c % kStages;
@@ -492,16 +566,18 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
             const float4* tb = stage_buf + size_t(st) * kChunkPairs * 2;
             const int first = e_begin + c * kChunkPairs;
             const int pairs = min(min(kChunkPairs, e_end - first), full_pairs - first);   // may be <= 0 in a tail-only chunk
-            int k = 0;
+            if (warp_live) {
+                int k = 0;
 #pragma unroll 1
-            for (; k + kGroup <= pairs; k += kGroup)
-                sweep_group<kGroup, false, false>(hc, tb, 2 * k, 2 * (first + k), cx, n_in, qn, n_band);
+                for (; k + kGroup <= pairs; k += kGroup)
+                    sweep_group<kGroup, false, false>(hc, tb, 2 * k, 2 * (first + k), cx, n_in, qn, n_band);
 #pragma unroll 1
-            for (; k < pairs; ++k)
-                sweep_group<1, false, false>(hc, tb, 2 * k, 2 * (first + k), cx, n_in, qn, n_band);
-            // odd tail point: the duplicated entry counts once
-            if ((n_pts & 1) && full_pairs >= first && full_pairs < min(first + kChunkPairs, e_end))
-                sweep_group<1, true, false>(hc, tb, 2 * (full_pairs - first), 2 * full_pairs, cx, n_in, qn, n_band);
+                for (; k < pairs; ++k)
+                    sweep_group<1, false, false>(hc, tb, 2 * k, 2 * (first + k), cx, n_in, qn, n_band);
+                // odd tail point: the duplicated entry counts once
+                if ((n_pts & 1) && full_pairs >= first && full_pairs < min(first + kChunkPairs, e_end))
+                    sweep_group<1, true, false>(hc, tb, 2 * (full_pairs - first), 2 * full_pairs, cx, n_in, qn, n_band);
+            }
             if (c + kStages < n_chunks) {                      // refill this stage (uniform branch)
                 __syncthreads();
                 if (threadIdx.x == 0) {
@@ -680,7 +756,7 @@ private:
 // confidence <= 0 give the single-launch behaviour of hg_ransac_hypothesize_score.
 static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, const int32_t* hyp_idx, int32_t* hyp_idx_out,
                       unsigned long long seed, int64_t n_hyp, int64_t round_hyp, float threshold_px, double confidence,
-                      bool adaptive, unsigned flags, int32_t* counts, float* best_H, int64_t* best_index, int32_t* best_count,
+                      bool adaptive, unsigned flags, double reject_lim2, int32_t* counts, float* best_H, int64_t* best_index, int32_t* best_count,
                       int64_t* n_evaluated, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -724,6 +800,7 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     hs.idx_out = reinterpret_cast<int4*>(hyp_idx_out);
     hs.seed = seed;
     hs.flags = flags;
+    hs.reject_lim2 = reject_lim2;
     hs.check_stop = adaptive ? 1 : 0;
     // split mode needs the accumulator, which the workspace holds only when the whole call is small (may_split(n_hyp))
     hs.acc = acc_bytes ? reinterpret_cast<int*>(ws + kHeaderBytes) : nullptr;
@@ -754,11 +831,16 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     return HG_OK;
 }
 
-static int check_options(const hg_ransac_options_t* o, unsigned* flags)
+static int check_options(const hg_ransac_options_t* o, unsigned* flags, double* reject_lim2)
 {
     *flags = 0u;
+    *reject_lim2 = 0.0;
     if (!o) return HG_OK;
     if (o->flags & ~(HG_RANSAC_REJECT_DEGENERATE | HG_RANSAC_DECIDE_ALL_F64)) return HG_ERR_INVALID_ARG;
+    if (o->flags & HG_RANSAC_REJECT_DEGENERATE) {
+        if (!(o->min_area_px2 >= 0.0f) || !(o->min_area_px2 < 3.0e38f)) return HG_ERR_INVALID_ARG;
+        *reject_lim2 = 2.0 * static_cast<double>(o->min_area_px2);
+    }
     *flags = o->flags;
     return HG_OK;
 }
@@ -774,10 +856,11 @@ extern "C" int hg_ransac_hypothesize_score_ex(const float* src_xy, const float* 
 {
     using namespace hg;
     unsigned flags = 0u;
+    double reject_lim2 = 0.0;
     if (n_hyp < 0 || n_hyp > 0x7fffffffLL) return HG_ERR_INVALID_ARG;
     if (n_pts < 4) return HG_ERR_INVALID_ARG;
     if (!(threshold_px > 0.0f) || !(threshold_px < 3.0e38f)) return HG_ERR_INVALID_ARG;
-    if (check_options(options, &flags) != HG_OK) return HG_ERR_INVALID_ARG;
+    if (check_options(options, &flags, &reject_lim2) != HG_OK) return HG_ERR_INVALID_ARG;
     if (n_hyp == 0) return HG_OK;
     if (!src_xy || !dst_xy || !hyp_idx || !workspace) return HG_ERR_INVALID_ARG;
     if (!aligned16(src_xy) || !aligned16(dst_xy) || !aligned16(hyp_idx) || !aligned16(workspace)) return HG_ERR_ALIGNMENT;
@@ -785,7 +868,7 @@ extern "C" int hg_ransac_hypothesize_score_ex(const float* src_xy, const float* 
         (best_index && (reinterpret_cast<uintptr_t>(best_index) & 7u)) || (best_count && !aligned4(best_count)))
         return HG_ERR_ALIGNMENT;
     if (workspace_bytes < hg_ransac_workspace_bytes(n_pts, n_hyp)) return HG_ERR_WORKSPACE;
-    return ransac_run(src_xy, dst_xy, n_pts, hyp_idx, nullptr, 0ull, n_hyp, n_hyp, threshold_px, 0.0, false, flags, counts, best_H,
+    return ransac_run(src_xy, dst_xy, n_pts, hyp_idx, nullptr, 0ull, n_hyp, n_hyp, threshold_px, 0.0, false, flags, reject_lim2, counts, best_H,
                       best_index, best_count, nullptr, workspace, workspace_bytes, cuda_stream);
 }
 
@@ -807,11 +890,12 @@ extern "C" int hg_ransac_adaptive_ex(const float* src_xy, const float* dst_xy, i
 {
     using namespace hg;
     unsigned flags = 0u;
+    double reject_lim2 = 0.0;
     if (max_hyp < 0 || max_hyp > 0x7fffffffLL || round_hyp < 1) return HG_ERR_INVALID_ARG;
     if (n_pts < 4) return HG_ERR_INVALID_ARG;
     if (!(threshold_px > 0.0f) || !(threshold_px < 3.0e38f)) return HG_ERR_INVALID_ARG;
     if (!(confidence < 1.0f) || !(confidence == confidence)) return HG_ERR_INVALID_ARG;
-    if (check_options(options, &flags) != HG_OK) return HG_ERR_INVALID_ARG;
+    if (check_options(options, &flags, &reject_lim2) != HG_OK) return HG_ERR_INVALID_ARG;
     if (max_hyp == 0) return HG_OK;
     if ((max_hyp + round_hyp - 1) / round_hyp > 65536) return HG_ERR_INVALID_ARG;          // launches per call
     if (!src_xy || !dst_xy || !workspace) return HG_ERR_INVALID_ARG;
@@ -822,7 +906,7 @@ extern "C" int hg_ransac_adaptive_ex(const float* src_xy, const float* dst_xy, i
         return HG_ERR_ALIGNMENT;
     if (workspace_bytes < hg_ransac_workspace_bytes(n_pts, max_hyp)) return HG_ERR_WORKSPACE;
     return ransac_run(src_xy, dst_xy, n_pts, nullptr, hyp_idx_out, seed, max_hyp, round_hyp, threshold_px,
-                      static_cast<double>(confidence), true, flags, counts, best_H, best_index, best_count, n_evaluated, workspace,
+                      static_cast<double>(confidence), true, flags, reject_lim2, counts, best_H, best_index, best_count, n_evaluated, workspace,
                       workspace_bytes, cuda_stream);
 }
 

@@ -240,3 +240,57 @@ def test_ransac_degenerate_and_non_finite_inputs():
     assert (both(s, d, 1e-6) >= 4).all()                         # the four sampled correspondences always fit exactly
     assert (both(s, d, 1e9) >= 999).all()
     both(s * 1e6, d * 1e6, 3e6)
+
+
+# ---- reading R20: sample check (HG_RANSAC_REJECT_DEGENERATE) -----------------------------------------------------------
+@pytest.mark.parametrize("n_pts,n_hyp,min_area", [(4096, 100000, 0.0),      # constant-bank path
+                                                  (4096, 100000, 400.0),
+                                                  (1000, 3000, 25.0),        # split shared-memory path
+                                                  (6001, 80000, 100.0),      # staged shared-memory path
+                                                  (4, 24, 0.0), (37, 513, 1e4)])
+def test_ransac_sample_check_matches_oracle(n_pts, n_hyp, min_area):
+    """Reject flags are integer/sign decisions on fp64 values both sides compute with the same IEEE operations: bit-exact.
+    A rejected hypothesis scores 0; every other count equals the plain call's."""
+    wl = W.ransac_workload(n_pts=n_pts, n_hyp=n_hyp, seed=W.SEED_BASE + 120 + n_pts)
+    s, d, idx = wl["src_xy"], wl["dst_xy"], wl["hyp_idx"]
+    if n_pts == 4:                                            # all 24 orders of the only sample
+        import itertools
+        idx = torch.tensor(list(itertools.permutations(range(4))), dtype=torch.int32)
+    rej = oracle.sample_check(s.numpy(), d.numpy(), idx.numpy(), min_area)
+    out = hg.hg_ransac_hypothesize_score(s.to(DEV), d.to(DEV), idx.to(DEV), 3.0, reject_degenerate=True, min_area_px2=min_area)
+    plain = hg.hg_ransac_hypothesize_score(s.to(DEV), d.to(DEV), idx.to(DEV), 3.0)
+    counts, pc = out["counts"].cpu().numpy(), plain["counts"].cpu().numpy()
+    st = hg.ransac_stats(out["workspace"])
+    assert st["n_rejected"] == int(rej.sum())
+    assert (counts[rej] == 0).all()
+    assert np.array_equal(counts[~rej], pc[~rej])            # same kernel arithmetic for the accepted ones: identical
+    assert (counts[~rej] >= 4).all() or n_pts == 4           # an accepted sample fits its own four points
+    ref = oracle.ransac(s.numpy(), d.numpy(), idx.numpy(), 3.0, band_rel=1e-4, reject_degenerate=True, min_area=min_area)
+    diff = np.abs(counts.astype(np.int64) - ref["counts"])
+    assert (diff <= ref["band_counts"]).all()
+    bi, bc = int(out["best_index"].item()), int(out["best_count"].item())
+    assert bc == counts.max() and bi == int(np.argmax(counts))
+    print(n_pts, n_hyp, min_area, "rejected", int(rej.sum()), "of", len(rej))
+
+
+def test_ransac_sample_check_all_rejected_and_adaptive():
+    wl = W.ransac_workload(n_pts=800, n_hyp=5000, seed=77, inlier_frac=1.0, noise_var=1e-6)
+    s, d, idx = wl["src_xy"], wl["dst_xy"].clone(), wl["hyp_idx"]
+    d[:, 0] = 640.0 - d[:, 0]                                                   # mirrored target plane: every sample flips
+    assert oracle.sample_check(s.numpy(), d.numpy(), idx.numpy(), 0.0).all()
+    out = hg.hg_ransac_hypothesize_score(s.to(DEV), d.to(DEV), idx.to(DEV), 3.0, reject_degenerate=True)
+    assert (out["counts"] == 0).all() and out["best_count"].item() == 0 and out["best_index"].item() == 0
+    assert hg.ransac_stats(out["workspace"])["n_rejected"] == 5000
+    # adaptive entry point with the check, against the oracle's loop with the same rule
+    wl = W.ransac_workload(n_pts=3000, n_hyp=4, seed=78, inlier_frac=0.4)
+    a = hg.hg_ransac_adaptive(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), 1234, 1 << 17, 1 << 16, 3.0, 0.0, want_idx=True,
+                              reject_degenerate=True, min_area_px2=50.0)
+    ref = oracle.ransac_adaptive(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), 1234, 1 << 17, 1 << 16, 3.0, 0.0,
+                                 reject_degenerate=True, min_area=50.0)
+    assert int(a["n_evaluated"].item()) == ref["n_evaluated"] == 1 << 17
+    assert np.array_equal(a["hyp_idx"].cpu().numpy(), ref["hyp_idx"])
+    rej = oracle.sample_check(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), ref["hyp_idx"], 50.0)
+    counts = a["counts"].cpu().numpy()
+    assert (counts[rej] == 0).all() and hg.ransac_stats(a["workspace"])["n_rejected"] == int(rej.sum())
+    assert (np.abs(counts.astype(np.int64) - ref["counts"]) <= ref["band_counts"]).all()
+    assert 0.3 < rej.mean() < 0.99

@@ -378,9 +378,15 @@ def run_next_rows(hg, W, dev, peak, peak_src):
     g = torch.randn((n, 3, 3), device=dev)
     go = torch.empty((n, 4, 2), dtype=torch.float32, device=dev)
     leg("rect_backward_2p26", lambda: hg.hg_aca_rect_backward(off, 0.0, 0.0, 127.0, 127.0, g, grad_offsets=go), 100, n, kernel="hg::rect_backward_kernel")
-    del g, go, Haos
+    del go, Haos
     osoa = off.reshape(n, 8).t().contiguous()
     del off
+    gsoa = g.reshape(n, 9).t().contiguous()
+    del g
+    gosoa = torch.empty((8, n), dtype=torch.float32, device=dev)
+    leg("rect_backward_soa_2p26", lambda: hg.hg_aca_rect_backward_soa(osoa, 0.0, 0.0, 127.0, 127.0, gsoa, grad_offsets=gosoa), 100, n,
+        kernel="hg::rect_backward_soa_kernel<4>")
+    del gsoa, gosoa
     Hsoa = torch.empty((9, n), dtype=torch.float32, device=dev)
     leg("rect_soa_2p26", lambda: hg.hg_aca_rect_batched(osoa, 0.0, 0.0, 127.0, 127.0, H=Hsoa, layout=hg.SOA, norm=hg.NORM_H33), 68, n, kernel="hg::rect_soa_kernel<double,4>")
     a = torch.rand((6, n), device=dev) * 600.0

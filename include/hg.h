@@ -183,6 +183,12 @@ HG_API int hg_aca_rect_batched(const float* offsets, float x0, float y0, float w
 HG_API int hg_aca_rect_backward(const float* offsets, float x0, float y0, float w, float h,
                          const float* grad_H, float* grad_offsets, int64_t n, void* cuda_stream);
 
+/* The same backward pass on structure-of-arrays planes (the streaming layout of every other entry point):
+ *   offsets float[8][n] (planes TL.x,TL.y,TR.x,...,BL.y), grad_H float[9][n] (planes g11,g12,...,g33),
+ *   grad_offsets float[8][n].  n % 4 == 0 takes the 128-bit path.  Errors as hg_aca_rect_backward.          */
+HG_API int hg_aca_rect_backward_soa(const float* offsets, float x0, float y0, float w, float h,
+                         const float* grad_H, float* grad_offsets, int64_t n, void* cuda_stream);
+
 /* --------------------------------------------------------------------------------------------
  * hg_affine_batched -- 2D affine transformation from THREE correspondences by the ACA route
  * (Sec. 5.2, Eq. 41 first row): H_A = H_A2^-1 * H_A1, the core transformation being the

@@ -19,7 +19,7 @@ from . import _build
 __all__ = [
     "HgError", "lib", "lib_path", "SOA", "AOS", "NORM_NONE", "NORM_H33", "NORM_FROBENIUS",
     "PREC_F64", "PREC_F32", "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host",
-    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
+    "hg_sks_batched_host", "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_aca_rect_backward_soa",
     "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
     "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
     "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex", "RANSAC_REJECT_DEGENERATE", "RANSAC_DECIDE_ALL_F64",
@@ -37,7 +37,7 @@ RANSAC_REJECT_DEGENERATE, RANSAC_DECIDE_ALL_F64 = 1, 2
 # every symbol include/hg.h declares
 EXPORTS = [
     "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-    "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_affine_batched",
+    "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_aca_rect_backward_soa", "hg_affine_batched",
     "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
     "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive", "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex",
     "hg_status_string", "hg_version", "hg_built_for_sm",
@@ -80,6 +80,7 @@ def lib() -> ctypes.CDLL:
                                          _c_i64, _c_int, _vp]
         L.hg_aca_rect_batched.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
         L.hg_aca_rect_backward.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _vp, _c_i64, _vp]
+        L.hg_aca_rect_backward_soa.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _vp, _c_i64, _vp]
         L.hg_offsets_to_warp.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _c_i32, _c_i32, _vp, _c_i32, _c_i32, _c_i32,
                                          _vp, _vp, _c_i64, _c_int, _vp]
         L.hg_affine_batched.argtypes = solve_args
@@ -102,7 +103,7 @@ def lib() -> ctypes.CDLL:
         L.hg_status_string.restype = ctypes.c_char_p
         for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
                      "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
-                     "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
+                     "hg_aca_rect_backward_soa", "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
                      "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
                      "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex", "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
@@ -339,6 +340,25 @@ def hg_aca_rect_backward(offsets, x0: float, y0: float, w: float, h: float, grad
     with _on(offsets.device):
         st = lib().hg_aca_rect_backward(po, x0, y0, w, h, pg, pr, n, _stream(stream))
     _check(st, "hg_aca_rect_backward")
+    return grad_offsets
+
+
+def hg_aca_rect_backward_soa(offsets, x0: float, y0: float, w: float, h: float, grad_H, grad_offsets=None,
+                             stream=None) -> torch.Tensor:
+    """The backward pass on planes: offsets [8,n], grad_H [9,n] -> grad_offsets [8,n]."""
+    n = _n_sets(offsets, SOA)
+    if tuple(grad_H.shape) != (9, n):
+        raise ValueError("grad_H must be [9,n]")
+    if grad_offsets is None:
+        grad_offsets = torch.empty((8, n), dtype=torch.float32, device=offsets.device)
+    elif tuple(grad_offsets.shape) != (8, n):
+        raise ValueError("grad_offsets must be [8,n]")
+    po, pg, pr = (_ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(grad_H, torch.float32, "cuda", "grad_H"),
+                  _ptr(grad_offsets, torch.float32, "cuda", "grad_offsets"))
+    _same_device(offsets, grad_H, grad_offsets)
+    with _on(offsets.device):
+        st = lib().hg_aca_rect_backward_soa(po, x0, y0, w, h, pg, pr, n, _stream(stream))
+    _check(st, "hg_aca_rect_backward_soa")
     return grad_offsets
 
 

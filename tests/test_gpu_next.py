@@ -87,6 +87,21 @@ def test_rect_backward_matches_oracle(rect, n, max_off):
     assert (np.abs(go - ref) <= 4e-7 * scale + 1e-30).all(), (np.abs(go - ref) / scale).max()
 
 
+@pytest.mark.parametrize("n", [4096, 4099, 1])
+def test_rect_backward_soa_matches_oracle_and_the_aos_entry_point(n):
+    rect = (16.0, 40.0, 300.0, 120.0)
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 31 + n, max_offset=30.0)
+    g = torch.randn((n, 3, 3), generator=torch.Generator().manual_seed(n), dtype=torch.float32)
+    o_soa, g_soa = off.reshape(n, 8).t().contiguous(), g.reshape(n, 9).t().contiguous()
+    go = hg.hg_aca_rect_backward_soa(o_soa.to(DEV), *rect, g_soa.to(DEV))
+    assert tuple(go.shape) == (8, n)
+    aos = hg.hg_aca_rect_backward(off.to(DEV), *rect, g.to(DEV))
+    assert torch.equal(go.t().reshape(n, 4, 2), aos)                     # the same arithmetic in both layouts
+    ref = oracle.aca_rect_backward(off.numpy(), *rect, g.numpy().astype(np.float64))
+    scale = np.abs(ref).reshape(n, 8).max(axis=1)[:, None, None]
+    assert (np.abs(go.t().reshape(n, 4, 2).cpu().numpy().astype(np.float64) - ref) <= 4e-7 * scale + 1e-30).all()
+
+
 def test_rect_backward_is_the_gradient_of_the_forward_entry_point():
     """Directional derivative of the library's own forward (H33-normalised) against <grad, direction>."""
     n = 512

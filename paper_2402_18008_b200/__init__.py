@@ -448,10 +448,11 @@ def _ransac_options(reject_degenerate, min_area_px2, decide_all_f64):
 
 def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, counts=None, workspace=None,
                                 want_counts: bool = True, stream=None, reject_degenerate: bool = False,
-                                min_area_px2: float = 0.0, decide_all_f64: bool = False):
+                                min_area_px2: float = 0.0, decide_all_f64: bool = False, best=None):
     """src_xy, dst_xy float32 [n_pts,2]; hyp_idx int32 [n_hyp,4] (all on the GPU).
     Returns dict(counts int32 [n_hyp] or None, best_H float32 [3,3], best_index int64 [1],
     best_count int32 [1], workspace uint8) -- device tensors, produced asynchronously.
+    best: optional (best_H [3,3] f32, best_index [1] i64, best_count [1] i32) tensors to write into.
     reject_degenerate / min_area_px2 / decide_all_f64: hg_ransac_options_t (the call goes through
     hg_ransac_hypothesize_score_ex when any is set)."""
     n_pts, n_hyp = int(src_xy.shape[0]), int(hyp_idx.shape[0])
@@ -466,10 +467,13 @@ def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, co
     need = hg_ransac_workspace_bytes(n_pts, n_hyp)
     if workspace is None:
         workspace = torch.empty((max(need, 16),), dtype=torch.uint8, device=dev)
-    best_H = torch.empty((3, 3), dtype=torch.float32, device=dev)
-    best_index = torch.empty((1,), dtype=torch.int64, device=dev)
-    best_count = torch.empty((1,), dtype=torch.int32, device=dev)
-    _same_device(src_xy, dst_xy, hyp_idx, counts, workspace)
+    if best is not None:          # (best_H, best_index, best_count) of an earlier call, reused: no allocation on the latency path
+        best_H, best_index, best_count = best
+    else:
+        best_H = torch.empty((3, 3), dtype=torch.float32, device=dev)
+        best_index = torch.empty((1,), dtype=torch.int64, device=dev)
+        best_count = torch.empty((1,), dtype=torch.int32, device=dev)
+    _same_device(src_xy, dst_xy, hyp_idx, counts, workspace, best_H, best_index, best_count)
     opt = _ransac_options(reject_degenerate, min_area_px2, decide_all_f64)
     head = (_ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
             _ptr(hyp_idx, torch.int32, "cuda", "hyp_idx"), n_hyp, float(threshold_px))

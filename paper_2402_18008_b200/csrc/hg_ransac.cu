@@ -43,7 +43,8 @@ struct RansacHeader {               // first 128 bytes of the workspace
     unsigned long long reserved[2];
     unsigned int bound_bits[4];     // float bits of max|sx|, max|sy|, max|dx/t|, max|dy/t|
     unsigned int stop;              // adaptive mode: set by the round kernel, later rounds return at once
-    unsigned int pad[11];
+    unsigned int blocks_done;       // tiny-call kernel: CTAs whose counts and candidate are complete
+    unsigned int pad[10];
 };
 static_assert(sizeof(RansacHeader) == kHeaderBytes, "header layout");
 
@@ -349,6 +350,9 @@ __device__ __noinline__ unsigned count_all_f64(SlowCtx& cx, int p0, int p1)
 // sitting exactly on the threshold): the whole warp recounts lane L's hypothesis over points [p0, p1) -- every lane
 // re-derives that hypothesis (deterministic, so identical), takes every 32nd point, applies the per-pair band to the
 // sweep's own fp32 arithmetic and the fp64 definition to what stays undecided.  Returns the count (same on all lanes).
+// FROM_RAW = false: the sweep's fp32 operands are read from the packed table in global memory; true (tiny-call kernel, which
+// has no global table) they are rebuilt from the raw points with the arithmetic that packed them.
+template <bool FROM_RAW>
 __device__ __noinline__ unsigned recount_warp(SlowCtx& cx, int L, int p0, int p1)
 {
     const int4 id = make_int4(__shfl_sync(0xffffffffu, cx.id.x, L), __shfl_sync(0xffffffffu, cx.id.y, L),
@@ -360,9 +364,15 @@ __device__ __noinline__ unsigned recount_warp(SlowCtx& cx, int L, int p0, int p1
     const int lane = threadIdx.x & 31;
     unsigned c = 0, n64 = 0;
     for (int pt = p0 + lane; pt < p1; pt += 32) {
-        const float4 A = __ldg(cx.table + 2 * (pt >> 1)), B = __ldg(cx.table + 2 * (pt >> 1) + 1);
-        const bool hi = pt & 1;
-        unsigned r = recheck_f32(hc, hi ? A.y : A.x, hi ? A.w : A.z, hi ? B.y : B.x, hi ? B.w : B.z);
+        unsigned r;
+        if (FROM_RAW) {
+            const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
+            r = recheck_f32(hc, sp.x, sp.y, static_cast<float>(-double(dq.x) * cx.inv_t), static_cast<float>(-double(dq.y) * cx.inv_t));
+        } else {
+            const float4 A = __ldg(cx.table + 2 * (pt >> 1)), B = __ldg(cx.table + 2 * (pt >> 1) + 1);
+            const bool hi = pt & 1;
+            r = recheck_f32(hc, hi ? A.y : A.x, hi ? A.w : A.z, hi ? B.y : B.x, hi ? B.w : B.z);
+        }
         if (r == 2u) {
             const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
             r = inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, cx.t) ? 1u : 0u;
@@ -598,7 +608,7 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
         while (ovf) {                                       // warp-uniform
             const int L = __ffs(ovf) - 1;
             ovf &= ovf - 1u;
-            const unsigned c = recount_warp(cx, L, 2 * e_begin, min(n_pts, 2 * e_end));
+            const unsigned c = recount_warp<false>(cx, L, 2 * e_begin, min(n_pts, 2 * e_end));
             if ((threadIdx.x & 31) == L) n_in = c;
         }
     }
@@ -626,6 +636,163 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
         }
     }
     if (band_tot && (threadIdx.x & 31) == 0) atomicAdd(&hdr->n_band, static_cast<unsigned long long>(band_tot));
+}
+
+// ---- 2a. tiny calls (the regime of the paper's Table 6): 32 hypotheses per CTA, every warp a slice of the table
+// A call of a few thousand hypotheses on a table that fits shared memory is latency-, not throughput-bound: memset + prep +
+// score + best + finalize are five dependent graph nodes for a few microseconds of arithmetic.  Here a CTA owns 32 hypotheses (lane = hypothesis) and packs the WHOLE table into its own
+// shared memory; warp w sweeps slice w of it for those 32 hypotheses (every warp derives them itself: no exchange), the
+// 16 partial counts meet in shared memory, warp 0 emits counts[], the CTA's best (count, index) and -- from its own
+// registers -- the unit-Frobenius H of that hypothesis as the CTA's candidate; one global ticket later the last CTA copies
+// the winning candidate.  One memset node (the 128-byte header) + this kernel.
+constexpr int kTinyHyp = 32;                      // hypotheses per CTA
+constexpr int kTinySlices = kRBlock / 32;         // warps = table slices
+
+__global__ void __launch_bounds__(kRBlock, 1)
+ransac_tiny_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts, int n_pairs, HypSource hs,
+                   double inv_t, double t, int* __restrict__ counts, RansacHeader* __restrict__ hdr, float* __restrict__ cand,
+                   float* __restrict__ best_H, long long* __restrict__ best_index, int* __restrict__ best_count)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float4* tb = reinterpret_cast<float4*>(smem_raw);                                   // n_pairs * 2 float4: the whole table
+    unsigned* queue = reinterpret_cast<unsigned*>(tb + 2 * n_pairs);                    // [kQueueCap][kRBlock]
+    __shared__ float red[4][kRBlock / 32];
+    __shared__ unsigned partial[kTinySlices][kTinyHyp];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+
+    const long long hidx = hs.h0 + static_cast<long long>(blockIdx.x) * kTinyHyp + lane;
+    const bool active = hidx < hs.h1;
+    SlowCtx cx;
+    cx.id = active ? hypothesis_indices(hs, hidx, n_pts) : make_int4(0, 0, 0, 0);
+    double s[8], d[8];
+    gather_sets(src_xy, dst_xy, cx.id, s, d);
+
+    float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;
+    for (int k = threadIdx.x; k < n_pairs; k += kRBlock) {
+        const int i0 = 2 * k, i1 = (2 * k + 1 < n_pts) ? 2 * k + 1 : 2 * k;
+        const float2 s0 = __ldg(src_xy + i0), s1 = __ldg(src_xy + i1);
+        const float2 d0 = __ldg(dst_xy + i0), d1 = __ldg(dst_xy + i1);
+        const float4 A = make_float4(s0.x, s1.x, s0.y, s1.y);
+        const float4 B = make_float4(static_cast<float>(-double(d0.x) * inv_t), static_cast<float>(-double(d1.x) * inv_t),
+                                     static_cast<float>(-double(d0.y) * inv_t), static_cast<float>(-double(d1.y) * inv_t));
+        tb[2 * k] = A; tb[2 * k + 1] = B;
+        m0 = fmaxf(m0, fmaxf(fabsf(A.x), fabsf(A.y)));
+        m1 = fmaxf(m1, fmaxf(fabsf(A.z), fabsf(A.w)));
+        m2 = fmaxf(m2, fmaxf(fabsf(B.x), fabsf(B.y)));
+        m3 = fmaxf(m3, fmaxf(fabsf(B.z), fabsf(B.w)));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, o));
+        m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, o));
+        m2 = fmaxf(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+        m3 = fmaxf(m3, __shfl_xor_sync(0xffffffffu, m3, o));
+    }
+    if (lane == 0) { red[0][wid] = m0; red[1][wid] = m1; red[2][wid] = m2; red[3][wid] = m3; }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        float m = 0.f;
+#pragma unroll
+        for (int w = 0; w < kRBlock / 32; ++w) m = fmaxf(m, red[q][w]);
+        cx.bounds[q] = m;
+    }
+
+    HypConst hc;
+    double Hn[9];
+    bool ok = make_hypothesis(s, d, inv_t, cx.bounds, Hn, hc) && active;
+    bool rejected = false;
+    if ((hs.flags & HG_RANSAC_REJECT_DEGENERATE) && active && sample_rejected(s, d, hs.reject_lim2)) {
+        ok = false; rejected = true;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) hc.h[k] = 0.f;
+        hc.h[2] = 1.f; hc.Bc = 0.f; hc.thr = 0u; hc.K = 0.f; hc.K0 = 0.f;
+    }
+    cx.src_xy = src_xy; cx.dst_xy = dst_xy; cx.table = nullptr; cx.inv_t = inv_t; cx.t = t;
+    cx.queue = queue + threadIdx.x; cx.n64 = 0u;
+
+    // slice of this warp: whole groups of kGroup entries, the last slice takes the remainder and the odd tail point
+    const int full_pairs = n_pts >> 1;
+    const int per = ((n_pairs + kTinySlices - 1) / kTinySlices + kGroup - 1) / kGroup * kGroup;
+    const int e_begin = min(n_pairs, wid * per), e_end = min(n_pairs, e_begin + per);
+    unsigned n_in = 0, qn = 0, n_band = 0;
+    if (hs.flags & HG_RANSAC_DECIDE_ALL_F64) {
+        if (active) n_in = count_all_f64(cx, 2 * e_begin, min(n_pts, 2 * e_end));
+    } else {
+        const int e_two = min(e_end, full_pairs);
+        int k = e_begin;
+#pragma unroll 1
+        for (; k + kGroup <= e_two; k += kGroup)
+            sweep_group<kGroup, false, false>(hc, tb, 2 * k, 2 * k, cx, n_in, qn, n_band);
+#pragma unroll 1
+        for (; k < e_two; ++k)
+            sweep_group<1, false, false>(hc, tb, 2 * k, 2 * k, cx, n_in, qn, n_band);
+        if ((n_pts & 1) && full_pairs >= e_begin && full_pairs < e_end)
+            sweep_group<1, true, false>(hc, tb, 2 * full_pairs, 2 * full_pairs, cx, n_in, qn, n_band);
+        if (__any_sync(0xffffffffu, qn != 0u)) {
+            unsigned ovf = __ballot_sync(0xffffffffu, qn > kQueueCap);
+            if (rejected) cx.id = make_int4(0, 0, 0, 0);
+            if (qn != 0u && qn <= kQueueCap) n_in += drain_queue(cx, qn);
+            while (ovf) {
+                const int L = __ffs(ovf) - 1;
+                ovf &= ovf - 1u;
+                const unsigned c = recount_warp<true>(cx, L, 2 * e_begin, min(n_pts, 2 * e_end));
+                if (lane == L) n_in = c;
+            }
+        }
+    }
+    partial[wid][lane] = ok ? n_in : 0u;
+    {   // statistics
+        const unsigned n64 = active ? cx.n64 : 0u;
+        const unsigned amb_mask = __ballot_sync(0xffffffffu, n64 != 0u);
+        const unsigned tot = __reduce_add_sync(0xffffffffu, n64);
+        const unsigned band_tot = __reduce_add_sync(0xffffffffu, active ? n_band : 0u);
+        if (lane == 0) {
+            if (amb_mask) { atomicAdd(&hdr->n_fixup, static_cast<unsigned long long>(__popc(amb_mask)));
+                            atomicAdd(&hdr->n_pairs_f64, static_cast<unsigned long long>(tot)); }
+            if (band_tot) atomicAdd(&hdr->n_band, static_cast<unsigned long long>(band_tot));
+        }
+    }
+    __syncthreads();
+    if (wid != 0) return;
+    unsigned total = 0;
+#pragma unroll
+    for (int w = 0; w < kTinySlices; ++w) total += partial[w][lane];
+    unsigned long long key = 0ull;
+    if (active) {
+        if (counts) counts[hidx] = static_cast<int>(total);
+        key = pack_key(total, static_cast<unsigned>(hidx));
+    }
+    const unsigned nrej = __popc(__ballot_sync(0xffffffffu, rejected));
+    const unsigned long long cta_key = warp_max_u64(key);
+    if (key == cta_key && active && best_H) {                // the CTA's candidate: this lane's own H, unit Frobenius
+        double H[9];
+        aca_solve<double>(s, d, H);                           // raw scale, as ransac_finalize_kernel normalises it
+        normalise<double>(H, 2);
+#pragma unroll
+        for (int k = 0; k < 9; ++k) cand[9 * blockIdx.x + k] = static_cast<float>(H[k]);
+    }
+    if (lane == 0) {
+        if (cta_key != 0ull) atomicMax(&hdr->best_key, cta_key);
+        if (nrej) atomicAdd(&hdr->n_rejected, static_cast<unsigned long long>(nrej));
+    }
+    __threadfence();
+    __syncwarp();
+    unsigned ticket = 0;
+    if (lane == 0) ticket = atomicAdd(&hdr->blocks_done, 1u);
+    ticket = __shfl_sync(0xffffffffu, ticket, 0);
+    if (ticket != gridDim.x - 1) return;
+    __threadfence();
+    const unsigned long long best = *reinterpret_cast<volatile unsigned long long*>(&hdr->best_key);
+    const unsigned bidx = 0xFFFFFFFFu - static_cast<unsigned>(best & 0xFFFFFFFFull);
+    if (lane == 0) {
+        if (best_index) *best_index = static_cast<long long>(bidx);
+        if (best_count) *best_count = static_cast<int>(best >> 32);
+    }
+    if (best_H && lane < 9) {
+        const unsigned blk = static_cast<unsigned>((static_cast<long long>(bidx) - hs.h0) / kTinyHyp);
+        best_H[lane] = __ldcg(cand + 9 * blk + lane);
+    }
 }
 
 // ---- 2b. best (split mode): total counts of hypotheses [h0, h1) -> counts[] and the packed maximum --------
@@ -687,15 +854,18 @@ static size_t table_bytes(int32_t n_pts) { return size_t((n_pts + 1) / 2) * 32; 
 
 // Launches with fewer hypothesis CTAs than half the machine also split the table over blockIdx.y.
 constexpr int kSplitBelowCtas = 148;
-constexpr int kMinPartEntries = 32;
+constexpr int kMinPartEntries = 8;
+constexpr int kFusedMaxPts = 4096;      // the one-kernel path packs the whole table in every CTA: tables that fit shared memory
+constexpr int kTinyMaxCtas = 296;         // tiny path: at most two CTAs per SM's worth of 32-hypothesis blocks
+constexpr size_t kTicketBytes = 64;     // so that the accumulator area of the smallest call still holds one 36-byte candidate
 static bool may_split(int64_t n_hyp) { return (n_hyp + kRBlock - 1) / kRBlock < kSplitBelowCtas; }
 
 // entries per part for a launch of n_hyp hypotheses (>= n_pairs: one part)
-static int part_entries_for(int n_pairs, int64_t n_hyp)
+static int part_entries_for(int n_pairs, int64_t n_hyp, int ctas_per_sm = 2)
 {
     const int64_t ctas = (n_hyp + kRBlock - 1) / kRBlock;
     if (ctas >= kSplitBelowCtas) return n_pairs;
-    int64_t parts = (2 * kSplitBelowCtas + ctas - 1) / ctas;                 // aim at two CTAs per SM
+    int64_t parts = (ctas_per_sm * kSplitBelowCtas + ctas - 1) / ctas;       // aim at ctas_per_sm CTAs per SM
     const int64_t max_parts = n_pairs / kMinPartEntries > 0 ? n_pairs / kMinPartEntries : 1;
     if (parts > max_parts) parts = max_parts;
     if (parts <= 1) return n_pairs;
@@ -710,7 +880,7 @@ extern "C" size_t hg_ransac_workspace_bytes(int32_t n_pts, int64_t n_hyp)
 {
     if (n_pts < 0 || n_hyp < 0) return 0;
     // small batches accumulate partial counts (4 B per hypothesis) when the table is split over CTAs
-    const size_t acc = hg::may_split(n_hyp) ? hg::align16(size_t(n_hyp) * sizeof(int)) : 0;
+    const size_t acc = hg::may_split(n_hyp) ? hg::align16(size_t(n_hyp) * sizeof(int)) + hg::kTicketBytes : 0;
     return hg::kHeaderBytes + hg::align16(hg::table_bytes(n_pts)) + acc;
 }
 
@@ -762,8 +932,9 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     unsigned char* ws = static_cast<unsigned char*>(workspace);
     RansacHeader* hdr = reinterpret_cast<RansacHeader*>(ws);
-    // workspace layout: header | partial-count accumulator (small calls only) | packed table
-    const size_t acc_bytes = may_split(n_hyp) ? align16(size_t(n_hyp) * sizeof(int)) : 0;
+    // workspace layout: header | partial-count accumulator / tiny-call candidates (small calls only) | packed table
+    const size_t acc_only = may_split(n_hyp) ? align16(size_t(n_hyp) * sizeof(int)) : 0;
+    const size_t acc_bytes = acc_only ? acc_only + kTicketBytes : 0;
     float4* table = reinterpret_cast<float4*>(ws + kHeaderBytes + acc_bytes);
     const float2* s2 = reinterpret_cast<const float2*>(src_xy);
     const float2* d2 = reinterpret_cast<const float2*>(dst_xy);
@@ -772,7 +943,29 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     const double inv_t = 1.0 / t;
     (void)workspace_bytes;
 
-    if (cudaMemsetAsync(hdr, 0, kHeaderBytes + acc_bytes, st) != cudaSuccess) return HG_ERR_CUDA;     // header and accumulator
+    if (cudaMemsetAsync(hdr, 0, kHeaderBytes + acc_bytes, st) != cudaSuccess) return HG_ERR_CUDA;     // header, accumulator
+    const int64_t tiny_ctas = (n_hyp + kTinyHyp - 1) / kTinyHyp;
+    if (!adaptive && acc_bytes && n_pts <= kFusedMaxPts && tiny_ctas <= kTinyMaxCtas &&
+        size_t(tiny_ctas) * 9 * sizeof(float) <= acc_bytes) {
+        // tiny call: 32 hypotheses per CTA, the table sliced over its warps; the accumulator area holds the candidates
+        HypSource hs;
+        hs.idx = reinterpret_cast<const int4*>(hyp_idx);
+        hs.idx_out = nullptr;
+        hs.seed = seed;
+        hs.flags = flags;
+        hs.reject_lim2 = reject_lim2;
+        hs.check_stop = 0;
+        hs.acc = nullptr;
+        hs.h0 = 0; hs.h1 = n_hyp;
+        hs.part_entries = n_pairs;
+        const size_t smem = size_t(n_pairs) * 32 + size_t(kQueueCap) * kRBlock * sizeof(unsigned);
+        if (cudaFuncSetAttribute(ransac_tiny_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
+            return HG_ERR_CUDA;
+        ransac_tiny_kernel<<<static_cast<unsigned>(tiny_ctas), kRBlock, smem, st>>>(
+            s2, d2, n_pts, n_pairs, hs, inv_t, t, counts, hdr, reinterpret_cast<float*>(ws + kHeaderBytes), best_H,
+            reinterpret_cast<long long*>(best_index), best_count);
+        return launch_status();
+    }
     {
         int blocks = (n_pairs + 255) / 256;
         if (blocks > 1184) blocks = 1184;

@@ -203,11 +203,3 @@ def distinct_indices(n_hyp: int, n_pts: int, g: torch.Generator, device) -> torc
     else:
         raise RuntimeError("distinct index draw did not converge")
     return idx.to(torch.int32).contiguous()
-
-
-def shard_range(n: int, rank: int, world: int):
-    """Contiguous [begin,end) slice of n independent units owned by `rank` of `world`
-    (the path shards with no data-path collective)."""
-    base, rem = divmod(n, world)
-    begin = rank * base + min(rank, rem)
-    return begin, begin + base + (1 if rank < rem else 0)

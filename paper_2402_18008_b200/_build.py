@@ -31,28 +31,39 @@ def is_stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
-    """Compile every .cu of csrc/ into one shared library (static cudart)."""
+    """Compile every .cu of csrc/ into one shared library (static cudart).  Safe when several processes call it at once
+    (one rank per GPU under torchrun): the build runs under an exclusive file lock, objects go to a per-process
+    directory and the library is moved into place atomically, so no rank ever dlopens a half-written file."""
     if not force and not is_stale():
         return LIB
-    objs = []
     build_dir = PKG / "build"
     build_dir.mkdir(exist_ok=True)
-    log = []
-    for s in SOURCES:
-        obj = build_dir / (s + ".o")
-        cmd = [_nvcc(), *NVCC_FLAGS, "-c", str(CSRC / s), "-o", str(obj)]
-        r = subprocess.run(cmd, capture_output=True, text=True)
-        log.append(r.stderr)
-        if r.returncode != 0:
-            raise RuntimeError("nvcc failed for %s:\n%s" % (s, r.stderr))
-        objs.append(str(obj))
-    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", str(LIB), *objs, "-cudart", "static"]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode != 0:
-        raise RuntimeError("link failed:\n" + r.stderr)
-    (build_dir / "ptxas.log").write_text("\n".join(log))
-    if verbose:
-        print("\n".join(log))
+    import fcntl
+    with open(build_dir / ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and not is_stale():            # another process built it while this one waited
+                return LIB
+            objs, log = [], []
+            for s in SOURCES:
+                obj = build_dir / (s + ".o")
+                cmd = [_nvcc(), *NVCC_FLAGS, "-c", str(CSRC / s), "-o", str(obj)]
+                r = subprocess.run(cmd, capture_output=True, text=True)
+                log.append(r.stderr)
+                if r.returncode != 0:
+                    raise RuntimeError("nvcc failed for %s:\n%s" % (s, r.stderr))
+                objs.append(str(obj))
+            tmp = PKG / ("libhg.so.tmp.%d" % os.getpid())
+            cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", str(tmp), *objs, "-cudart", "static"]
+            r = subprocess.run(cmd, capture_output=True, text=True)
+            if r.returncode != 0:
+                raise RuntimeError("link failed:\n" + r.stderr)
+            os.replace(tmp, LIB)
+            (build_dir / "ptxas.log").write_text("\n".join(log))
+            if verbose:
+                print("\n".join(log))
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
     return LIB
 
 

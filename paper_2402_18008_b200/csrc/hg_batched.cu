@@ -142,11 +142,20 @@ int solve_batched(int method, const float* src, const float* dst, float* H, int6
 // `n` floats): cudaMemcpy2DAsync moves them into chunk-local device planes.
 // ------------------------------------------------------------------------------------------
 // Device-visible alias of a page-locked host pointer, if it is one.
-static bool mapped_host_pointer(const void* host, void** dev)
+// Both ends of [host, host + bytes) must belong to page-locked, mapped memory, and map to one contiguous device range
+// (a buffer registered only in part would otherwise take the zero-copy path and fault in the kernel).
+static bool mapped_host_pointer(const void* host, size_t bytes, void** dev)
 {
-    cudaPointerAttributes a;
+    cudaPointerAttributes a, z;
     if (cudaPointerGetAttributes(&a, host) != cudaSuccess) { cudaGetLastError(); return false; }
     if (a.type != cudaMemoryTypeHost || a.devicePointer == nullptr) return false;
+    if (bytes > 1) {
+        const char* last = static_cast<const char*>(host) + (bytes - 1);
+        if (cudaPointerGetAttributes(&z, last) != cudaSuccess) { cudaGetLastError(); return false; }
+        if (z.type != cudaMemoryTypeHost || z.devicePointer == nullptr) return false;
+        if (static_cast<const char*>(z.devicePointer) - static_cast<const char*>(a.devicePointer) != static_cast<ptrdiff_t>(bytes - 1))
+            return false;
+    }
     *dev = a.devicePointer;
     return true;
 }
@@ -165,7 +174,8 @@ static int solve_batched_host(int method, const float* src, const float* dst, fl
     // memory.  Measured equal to the best of the staged pipeline (PCIe-bound) and steadier.  chunk_sets is ignored.
     {
         void *ds = nullptr, *dd = nullptr, *dh = nullptr;
-        if (mapped_host_pointer(src, &ds) && mapped_host_pointer(dst, &dd) && mapped_host_pointer(H, &dh) &&
+        const size_t in_bytes = size_t(n) * 8 * sizeof(float), out_bytes = size_t(n) * 9 * sizeof(float);
+        if (mapped_host_pointer(src, in_bytes, &ds) && mapped_host_pointer(dst, in_bytes, &dd) && mapped_host_pointer(H, out_bytes, &dh) &&
             aligned16(ds) && aligned16(dd) && aligned16(dh)) {
             cudaStream_t zs = nullptr;
             int rc = cuda_status(cudaStreamCreateWithFlags(&zs, cudaStreamNonBlocking));

@@ -298,3 +298,39 @@ def test_ransac_adaptive_agrees_with_explicit_indices():
     assert torch.equal(plain["counts"], out["counts"])
     assert plain["best_index"].item() == out["best_index"].item()
     assert torch.equal(plain["best_H"], out["best_H"])
+
+
+@pytest.mark.parametrize("n_pts,max_hyp,round_hyp", [(4, 10, 1000), (1001, 700, 5000), (37, 1, 1), (2049, 3000, 2999)])
+def test_ransac_adaptive_boundary_shapes(n_pts, max_hyp, round_hyp):
+    """round_hyp > max_hyp (one ragged round), odd tables, the smallest table: same rule as the oracle's loop."""
+    wl = W.ransac_workload(n_pts=n_pts, n_hyp=4, seed=W.SEED_BASE + 200 + n_pts, inlier_frac=0.6)
+    out = hg.hg_ransac_adaptive(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), 42, max_hyp, round_hyp, 3.0, 0.0, want_idx=True)
+    ref = oracle.ransac_adaptive(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), 42, max_hyp, round_hyp, 3.0, 0.0)
+    assert int(out["n_evaluated"].item()) == ref["n_evaluated"] == max_hyp
+    assert np.array_equal(out["hyp_idx"].cpu().numpy(), ref["hyp_idx"])
+    diff = np.abs(out["counts"].cpu().numpy().astype(np.int64) - ref["counts"])
+    assert (diff <= ref["band_counts"]).all()
+    assert int(out["best_count"].item()) == int(out["counts"].max().item())
+
+
+def test_combine_best_on_cuda_tensors_over_nccl():
+    """The multi-GPU pick of the best hypothesis (sharding.combine_best) on device tensors through NCCL -- with the one
+    GPU this box has, a world of size 1: it exercises the CUDA/NCCL code path, not scaling."""
+    import os
+    import torch.distributed as dist
+    from paper_2402_18008_b200.sharding import combine_best, shard_range
+    if dist.is_initialized():
+        pytest.skip("a process group already exists in this process")
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29541")
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device(DEV, 0))
+    try:
+        wl = W.ransac_workload(n_pts=500, n_hyp=2000, seed=3)
+        b, e = shard_range(2000, 0, 1)
+        out = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"][b:e].to(DEV), 3.0)
+        c, i, H = combine_best(out["best_count"], out["best_index"] + b, out["best_H"])
+        assert c.is_cuda and i.is_cuda and H.is_cuda
+        assert int(c.item()) == int(out["best_count"].item()) and int(i.item()) == int(out["best_index"].item())
+        assert torch.equal(H, out["best_H"])
+    finally:
+        dist.destroy_process_group()

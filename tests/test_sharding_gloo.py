@@ -23,7 +23,6 @@ def test_shard_range_partitions():
                 assert a[1] == b[0]
             sizes = [e - b for b, e in edges]
             assert max(sizes) - min(sizes) <= 1
-    assert shard_range(10, 1, 2) == W.shard_range(10, 1, 2)
     with pytest.raises(ValueError):
         shard_range(10, 2, 2)
 

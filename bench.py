@@ -325,6 +325,15 @@ def run_extras(hg, W, dev, src, dst, H, peak, peak_src, cpu=True):
         s_np, d_np, i_np = wl["src_xy"].cpu().numpy(), wl["dst_xy"].cpu().numpy(), wl["hyp_idx"][:nh].cpu().numpy()
         ex["ransac_c4"]["cpu_baseline"] = timed_oracle(lambda: oracle.ransac(s_np, d_np, i_np, 3.0), nh * 4096, "pairs/s",
                                                        "first 2^15 of the 2^20 hypotheses x all 4096 correspondences, fp64 oracle", 3.0)
+    # the same call with the sample check of reading R20 (rejected hypotheses skip the sweep)
+    f4r = lambda: hg.hg_ransac_hypothesize_score(wl["src_xy"], wl["dst_xy"], wl["hyp_idx"], 3.0, counts=cnt, workspace=ws,
+                                                 reject_degenerate=True, min_area_px2=0.0)
+    f4r(); f4r()
+    msr = event_time_ms(f4r, 20) / 20
+    str_ = hg.ransac_stats(ws)
+    ex["ransac_c4_reject_degenerate"] = {"ms": msr, "hypotheses_per_s": (1 << 20) / msr * 1e3, "n_rejected": str_["n_rejected"],
+                                         "pairs_swept_per_s": ((1 << 20) - str_["n_rejected"]) * 4096 / msr * 1e3}
+    ex["ransac_c4"]["pairs_in_table_wide_band"] = stats.get("n_band")
     # RANSAC extras: on-device sampling, rounds of one wave (296 CTAs x 512), with and without adaptive termination
     fa = lambda conf: hg.hg_ransac_adaptive(wl["src_xy"], wl["dst_xy"], 240218008, 1 << 20, 296 * 512, 3.0, conf,
                                             want_counts=False, workspace=ws)
@@ -339,7 +348,10 @@ def run_extras(hg, W, dev, src, dst, H, peak, peak_src, cpu=True):
     for n_pts_s, n_hyp_s in ((1000, 1024), (500, 256)):
         wls = W.ransac_workload(n_pts=n_pts_s, n_hyp=n_hyp_s, seed=W.SEED_BASE + 44, device=dev)
         wss = torch.empty(hg.hg_ransac_workspace_bytes(n_pts_s, n_hyp_s), dtype=torch.uint8, device=dev)
-        fs = lambda: hg.hg_ransac_hypothesize_score(wls["src_xy"], wls["dst_xy"], wls["hyp_idx"], 3.0, want_counts=False, workspace=wss)
+        o0 = hg.hg_ransac_hypothesize_score(wls["src_xy"], wls["dst_xy"], wls["hyp_idx"], 3.0, want_counts=False, workspace=wss)
+        keep = (o0["best_H"], o0["best_index"], o0["best_count"])          # outputs reused: no allocation on the timed path
+        fs = lambda: hg.hg_ransac_hypothesize_score(wls["src_xy"], wls["dst_xy"], wls["hyp_idx"], 3.0, want_counts=False, workspace=wss,
+                                                    best=keep)
         for _ in range(5):
             fs()
         row = {"n_pts": n_pts_s, "n_hyp": n_hyp_s, "us_per_call_launch": event_time_ms(fs, 100) / 100 * 1e3}

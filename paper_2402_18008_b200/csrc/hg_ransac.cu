@@ -170,12 +170,11 @@ __device__ __forceinline__ int4 hypothesis_indices(const HypSource& hs, long lon
     return hs.idx ? __ldg(hs.idx + hidx) : sample4(hs.seed, static_cast<unsigned long long>(hidx), n_pts);
 }
 
-// fp64 ACA solve, max-abs normalisation, threshold folding and the error band.
+// fp64 ACA solve (raw scale in H), max-abs normalisation (Hn) and threshold folding (c.h).
 // Returns false for an unusable H (all zero or non-finite): such a hypothesis scores 0 (R9: W == 0).
-__device__ __forceinline__ bool make_hypothesis(const double s[8], const double d[8], double inv_t,
-                                                const float bounds[4], double Hn[9], HypConst& c)
+__device__ __forceinline__ bool solve_for_sweep(const double s[8], const double d[8], double inv_t, double H[9], double Hn[9],
+                                                HypConst& c)
 {
-    double H[9];
     aca_solve<double>(s, d, H);
     double m = 0.0;
 #pragma unroll
@@ -189,6 +188,12 @@ __device__ __forceinline__ bool make_hypothesis(const double s[8], const double 
     for (int k = 0; k < 6; ++k) c.h[k] = static_cast<float>(Hn[k] * rt);
 #pragma unroll
     for (int k = 6; k < 9; ++k) c.h[k] = static_cast<float>(Hn[k]);
+    return ok;
+}
+
+// The error band of the fp32 sweep for the folded H in c.h and the coordinate bounds of the table.
+__device__ __forceinline__ void error_band(const float bounds[4], bool ok, HypConst& c)
+{
     // Error band, u = 2^-24:
     //   A_r = |h_r1| Sx + |h_r2| Sy + |h_r3|;  c1 = u (3 A1 + 4 Dx A3), c2 = u (3 A2 + 4 Dy A3), eW = 3 u A3
     //   C = c1 + c2 + eW;  K = 4 C + 16 u A3;  K0 = 32 C^2      (evaluated in fp64, rounded up)
@@ -210,6 +215,14 @@ __device__ __forceinline__ bool make_hypothesis(const double s[8], const double 
         for (int k = 0; k < 9; ++k) c.h[k] = 0.f;
         c.h[2] = 1.f; c.Bc = 0.f; c.thr = 0u;
     }
+}
+
+__device__ __forceinline__ bool make_hypothesis(const double s[8], const double d[8], double inv_t,
+                                                const float bounds[4], double Hn[9], HypConst& c)
+{
+    double H[9];
+    const bool ok = solve_for_sweep(s, d, inv_t, H, Hn, c);
+    error_band(bounds, ok, c);
     return ok;
 }
 
@@ -222,6 +235,20 @@ __device__ __forceinline__ bool inlier_f64(const double H[9], double sx, double 
     if (W == 0.0) return false;
     const double ex = X / W - dx, ey = Y / W - dy;
     return sqrt(fma(ex, ex, ey * ey)) <= t;
+}
+
+// The definition (reading R9: ||pi(H s) - d||_2 <= t, W == 0 -> outlier) in fp64, multiplied through by W^2 so that it
+// needs no division and no square root:  (X - dx W)^2 + (Y - dy W)^2 <= (t W)^2.  Same decision as the quotient form
+// except within a few fp64 ulps of the threshold; ~12 dependent fp64 operations instead of two divisions and a root,
+// which is what a warp waits for when one of its lanes has a pair inside the band.
+__device__ __forceinline__ bool inlier_f64_nodiv(const double H[9], double sx, double sy, double dx, double dy, double t)
+{
+    const double X = fma(H[0], sx, fma(H[1], sy, H[2]));
+    const double Y = fma(H[3], sx, fma(H[4], sy, H[5]));
+    const double W = fma(H[6], sx, fma(H[7], sy, H[8]));
+    if (W == 0.0) return false;
+    const double ex = fma(-dx, W, X), ey = fma(-dy, W, Y), tw = t * W;
+    return fma(ex, ex, ey * ey) <= tw * tw;
 }
 
 // ---- 1. prep ---------------------------------------------------------------------------------
@@ -350,9 +377,6 @@ __device__ __noinline__ unsigned count_all_f64(SlowCtx& cx, int p0, int p1)
 // sitting exactly on the threshold): the whole warp recounts lane L's hypothesis over points [p0, p1) -- every lane
 // re-derives that hypothesis (deterministic, so identical), takes every 32nd point, applies the per-pair band to the
 // sweep's own fp32 arithmetic and the fp64 definition to what stays undecided.  Returns the count (same on all lanes).
-// FROM_RAW = false: the sweep's fp32 operands are read from the packed table in global memory; true (tiny-call kernel, which
-// has no global table) they are rebuilt from the raw points with the arithmetic that packed them.
-template <bool FROM_RAW>
 __device__ __noinline__ unsigned recount_warp(SlowCtx& cx, int L, int p0, int p1)
 {
     const int4 id = make_int4(__shfl_sync(0xffffffffu, cx.id.x, L), __shfl_sync(0xffffffffu, cx.id.y, L),
@@ -364,15 +388,9 @@ __device__ __noinline__ unsigned recount_warp(SlowCtx& cx, int L, int p0, int p1
     const int lane = threadIdx.x & 31;
     unsigned c = 0, n64 = 0;
     for (int pt = p0 + lane; pt < p1; pt += 32) {
-        unsigned r;
-        if (FROM_RAW) {
-            const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
-            r = recheck_f32(hc, sp.x, sp.y, static_cast<float>(-double(dq.x) * cx.inv_t), static_cast<float>(-double(dq.y) * cx.inv_t));
-        } else {
-            const float4 A = __ldg(cx.table + 2 * (pt >> 1)), B = __ldg(cx.table + 2 * (pt >> 1) + 1);
-            const bool hi = pt & 1;
-            r = recheck_f32(hc, hi ? A.y : A.x, hi ? A.w : A.z, hi ? B.y : B.x, hi ? B.w : B.z);
-        }
+        const float4 A = __ldg(cx.table + 2 * (pt >> 1)), B = __ldg(cx.table + 2 * (pt >> 1) + 1);
+        const bool hi = pt & 1;
+        unsigned r = recheck_f32(hc, hi ? A.y : A.x, hi ? A.w : A.z, hi ? B.y : B.x, hi ? B.w : B.z);
         if (r == 2u) {
             const float2 sp = __ldg(cx.src_xy + pt), dq = __ldg(cx.dst_xy + pt);
             r = inlier_f64(Hn, sp.x, sp.y, dq.x, dq.y, cx.t) ? 1u : 0u;
@@ -608,7 +626,7 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
         while (ovf) {                                       // warp-uniform
             const int L = __ffs(ovf) - 1;
             ovf &= ovf - 1u;
-            const unsigned c = recount_warp<false>(cx, L, 2 * e_begin, min(n_pts, 2 * e_end));
+            const unsigned c = recount_warp(cx, L, 2 * e_begin, min(n_pts, 2 * e_end));
             if ((threadIdx.x & 31) == L) n_in = c;
         }
     }
@@ -638,48 +656,193 @@ ransac_score_kernel(const float2* __restrict__ src_xy, const float2* __restrict_
     if (band_tot && (threadIdx.x & 31) == 0) atomicAdd(&hdr->n_band, static_cast<unsigned long long>(band_tot));
 }
 
-// ---- 2a. tiny calls (the regime of the paper's Table 6): 32 hypotheses per CTA, every warp a slice of the table
-// A call of a few thousand hypotheses on a table that fits shared memory is latency-, not throughput-bound: memset + prep +
-// score + best + finalize are five dependent graph nodes for a few microseconds of arithmetic.  Here a CTA owns 32 hypotheses (lane = hypothesis) and packs the WHOLE table into its own
-// shared memory; warp w sweeps slice w of it for those 32 hypotheses (every warp derives them itself: no exchange), the
-// 16 partial counts meet in shared memory, warp 0 emits counts[], the CTA's best (count, index) and -- from its own
-// registers -- the unit-Frobenius H of that hypothesis as the CTA's candidate; one global ticket later the last CTA copies
-// the winning candidate.  One memset node (the 128-byte header) + this kernel.
-constexpr int kTinyHyp = 32;                      // hypotheses per CTA
-constexpr int kTinySlices = kRBlock / 32;         // warps = table slices
+// ---- 2a. tiny calls (the regime of the paper's Table 6) --------------------------------------------------
+// A call of a few thousand hypotheses on a table that fits shared memory is latency-, not throughput-bound: what it costs
+// is the number of dependent round trips to L2 (~450 ns each at this clock), barriers and launches on its critical path,
+// not its arithmetic.  The call is two launches that overlap: a one-CTA kernel that zeroes the header and the slots and
+// releases its dependent at once (programmatic dependent launch), and this kernel, which touches them only after
+// `griddepcontrol.wait` -- its whole set-up and sweep run meanwhile.  (A memset node instead costs 3 us in a graph.)
+// Decomposition: blockIdx.x = a group of 32 hypotheses (lane = hypothesis), blockIdx.y = a part of the table; the CTAs
+// of one group form a thread-block cluster (1 x P x 1, P <= 8, chosen so that the call covers the machine).  Critical path:
+//   1. one round trip: the hypothesis indices and the whole table (every CTA packs all of it into shared memory; the
+//      sampled correspondences are then gathered from there instead of by a second, dependent round trip);
+//   2. every warp derives the 32 hypotheses itself (fp64 solve: latency, not throughput, at one warp per scheduler -- no
+//      exchange is cheaper than recomputing) and sweeps a quarter of its CTA's part; pairs inside the band are only noted
+//      and decided after the sweep, all lanes side by side;
+//   3. partial counts reach the cluster's rank-0 CTA by st.async into its shared memory, completing on its mbarrier (no
+//      cluster-wide barrier: ~400 cycles instead of ~1900);
+//   4. that CTA emits counts[] and publishes the group's best (count, index) with -- from its own registers -- the
+//      unit-Frobenius H of that hypothesis in a slot of stamped words, taking a global ticket in the same breath (no fence);
+//   5. the last group reads the slots (one more round trip) and writes the winner.
+constexpr int kTinyHyp = 32;                      // hypotheses per group
+constexpr int kTinyThreads = 128;
+constexpr int kTinyWarps = kTinyThreads / 32;     // warps of a CTA = quarters of its part of the table
+constexpr int kTinyMaxParts = 8;                  // portable cluster size
 
-__global__ void __launch_bounds__(kRBlock, 1)
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void cluster_arrive_release() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait_acquire() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+// Zeroes the first `n16` 16-byte words of the workspace; its dependent launch may start at once.
+__global__ void __launch_bounds__(256) ransac_zero_kernel(uint4* __restrict__ p, int n16)
+{
+    grid_launch_dependents();
+    for (int i = threadIdx.x; i < n16; i += 256) p[i] = make_uint4(0u, 0u, 0u, 0u);
+}
+
+// What a group leaves for the final step: its best (count, index) and that hypothesis' unit-Frobenius H.
+// Every 64-bit word carries its own stamp (high half) beside 32 bits of payload: key low, key high, h[0..8].  A relaxed
+// 64-bit store or load is single-copy atomic, so a word whose stamp reads kSlotStamp is this call's (the zero kernel
+// cleared the slots) -- the final step can therefore take its ticket WITHOUT first waiting for the slot stores to be
+// acknowledged (no fence: one round trip to L2 instead of two), and the last group simply re-reads a word whose stamp has
+// not landed yet.  The stores were issued before the ticket, so they land whatever the issuing CTA does next: the wait is
+// bounded by a memory latency and depends on no other CTA being scheduled.
+constexpr int kSlotWords = 11;
+constexpr unsigned kSlotStamp = 0x5EED0001u;
+struct __align__(16) TinySlot { unsigned long long w[kSlotWords + 1]; };
+static_assert(sizeof(TinySlot) == 96, "slot layout");
+__device__ __forceinline__ void st_relaxed_gpu_u64(unsigned long long* p, unsigned long long v)
+{ asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory"); }
+__device__ __forceinline__ unsigned long long ld_relaxed_gpu_u64(const unsigned long long* p)
+{ unsigned long long v; asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory"); return v; }
+__device__ __forceinline__ unsigned long long stamped(unsigned payload) { return (static_cast<unsigned long long>(kSlotStamp) << 32) | payload; }
+
+// Table entry of the tiny kernel: the two float4 of the packed table plus the raw targets (dx0, dx1, dy0, dy1), so that a
+// pair inside the band is decided by the definition from shared memory and the fp64 H the thread still holds, and the
+// sampled correspondences are gathered from it.
+constexpr int kTinyEntry = 3;                     // float4 per entry
+
+// One 32-bit word into the shared memory of CTA `rank` of this cluster, counted (4 bytes) on that CTA's mbarrier when it has
+// landed: the consumer waits on its own mbarrier and then reads its own shared memory -- no cluster-wide barrier.
+__device__ __forceinline__ void st_async_cluster_u32(const void* local_data, const uint64_t* local_bar, unsigned rank, unsigned v)
+{
+    unsigned rd, rb;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rd) : "r"(smem_u32(local_data)), "r"(rank));
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rb) : "r"(smem_u32(local_bar)), "r"(rank));
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.u32 [%0], %1, [%2];" :: "r"(rd), "r"(v), "r"(rb) : "memory");
+}
+
+// Point `hi` of table entry `e` by the definition in fp64 (reading R9); the entry holds the raw coordinates.
+__device__ __forceinline__ unsigned tiny_inlier_f64(const double Hn[9], double t, const float4* __restrict__ e, unsigned hi)
+{
+    const float4 A = e[0], D = e[2];
+    return inlier_f64_nodiv(Hn, hi ? A.y : A.x, hi ? A.w : A.z, hi ? D.y : D.x, hi ? D.w : D.z, t) ? 1u : 0u;
+}
+
+// G consecutive entries (2G points) from entry k0 of the table `tb`, against one hypothesis.  The fast path is the one of
+// sweep_group.  When a pair of the group lies inside the table-wide band the thread only notes (k0, which of the 2G points)
+// in its own queue -- branch-free flags and one store: what a lone warp per scheduler pays for a divergent excursion is
+// its latency, not its instruction count -- and the warp decides the noted pairs after the sweep, all lanes side by side,
+// straight by the definition in fp64 (cheap since it needs no division; the per-pair fp32 band of the big kernel would
+// cost as much as it saves here).  `qn` counts the groups noted; beyond kQueueCap they are dropped and the thread
+// recounts its slice afterwards.
+template <int G, bool ONLY_X>
+__device__ __forceinline__ void tiny_group(const HypConst& hc, const float4* __restrict__ tb, int k0, unsigned* __restrict__ queue,
+                                           unsigned& n_in, unsigned& qn)
+{
+    float2 a[G];
+    bool amb = false;
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        const float4 A = tb[kTinyEntry * (k0 + g)], B = tb[kTinyEntry * (k0 + g) + 1];
+        a[g] = score2(hc, make_float2(A.x, A.y), make_float2(A.z, A.w), make_float2(B.x, B.y), make_float2(B.z, B.w));
+        n_in += sign_bit(a[g].x);
+        amb |= (__float_as_uint(a[g].x) <= hc.thr);
+        if (!ONLY_X) {
+            n_in += sign_bit(a[g].y);
+            amb |= (__float_as_uint(a[g].y) <= hc.thr);
+        }
+    }
+    if (amb) {
+        unsigned mask = 0u;                                   // bit 2g + j: point j of entry k0 + g is in the band
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            mask |= (__float_as_uint(a[g].x) <= hc.thr) ? (1u << (2 * g)) : 0u;
+            if (!ONLY_X) mask |= (__float_as_uint(a[g].y) <= hc.thr) ? (2u << (2 * g)) : 0u;
+        }
+        if (qn < kQueueCap) queue[qn * kTinyThreads] = (static_cast<unsigned>(k0) << 16) | mask;
+        ++qn;
+    }
+}
+
+// statistics words of one warp (the header is zero by now)
+__device__ __forceinline__ void tiny_stats(RansacHeader* __restrict__ hdr, unsigned n64, unsigned n_band)
+{
+    const unsigned amb_mask = __ballot_sync(0xffffffffu, n64 != 0u);
+    const unsigned tot = __reduce_add_sync(0xffffffffu, n64);
+    const unsigned band_tot = __reduce_add_sync(0xffffffffu, n_band);
+    if ((threadIdx.x & 31) == 0) {
+        if (amb_mask) { atomicAdd(&hdr->n_fixup, static_cast<unsigned long long>(__popc(amb_mask)));
+                        atomicAdd(&hdr->n_pairs_f64, static_cast<unsigned long long>(tot)); }
+        if (band_tot) atomicAdd(&hdr->n_band, static_cast<unsigned long long>(band_tot));
+    }
+}
+
+__global__ void __launch_bounds__(kTinyThreads)
 ransac_tiny_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts, int n_pairs, HypSource hs,
-                   double inv_t, double t, int* __restrict__ counts, RansacHeader* __restrict__ hdr, float* __restrict__ cand,
+                   double inv_t, double t, int* __restrict__ counts, RansacHeader* __restrict__ hdr, TinySlot* __restrict__ slots,
                    float* __restrict__ best_H, long long* __restrict__ best_index, int* __restrict__ best_count)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4* tb = reinterpret_cast<float4*>(smem_raw);                                   // n_pairs * 2 float4: the whole table
-    unsigned* queue = reinterpret_cast<unsigned*>(tb + 2 * n_pairs);                    // [kQueueCap][kRBlock]
-    __shared__ float red[4][kRBlock / 32];
-    __shared__ unsigned partial[kTinySlices][kTinyHyp];
+    float4* tb = reinterpret_cast<float4*>(smem_raw);                   // n_pairs * kTinyEntry float4: the whole table
+    unsigned* queue = reinterpret_cast<unsigned*>(tb + size_t(n_pairs) * kTinyEntry) + threadIdx.x;   // [kQueueCap][kTinyThreads]
+    __shared__ float red[4][kTinyWarps];
+    __shared__ unsigned partial[kTinyWarps][kTinyHyp];
+    __shared__ unsigned cl_partial[kTinyMaxParts][kTinyHyp];            // rank 0: the counts of the other parts land here
+    __shared__ __align__(8) uint64_t cl_bar;                            // rank 0: completes when all of them have
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int part = blockIdx.y, parts = gridDim.y;                     // cluster = (1, parts, 1): rank = part
+    if (parts > 1) {
+        if (part == 0 && threadIdx.x == 0) {
+            mbar_init(&cl_bar, 1);
+            fence_barrier_init();
+            mbar_arrive_expect_tx(&cl_bar, static_cast<uint32_t>(parts - 1) * kTinyHyp * 4u);
+        }
+        cluster_arrive_release();                   // waited for by the senders: rank 0 runs and its mbarrier is armed
+    }
 
+    // first loads: the hypothesis (lane = hypothesis, every warp its own copy) and the table
     const long long hidx = hs.h0 + static_cast<long long>(blockIdx.x) * kTinyHyp + lane;
     const bool active = hidx < hs.h1;
-    SlowCtx cx;
-    cx.id = active ? hypothesis_indices(hs, hidx, n_pts) : make_int4(0, 0, 0, 0);
-    double s[8], d[8];
-    gather_sets(src_xy, dst_xy, cx.id, s, d);
+    int4 id = make_int4(0, 0, 0, 0);                                    // beyond the last hypothesis: a degenerate sample
+    if (active) id = __ldg(hs.idx + hidx);
 
+    // One pass over the table: every CTA packs all of it into its shared memory (the sampled correspondences are gathered
+    // from there, one memory latency earlier than a dependent global gather) and takes the coordinate bounds; it sweeps only
+    // its part.  Two points per 128-bit load, four loads of each plane in flight per thread.
+    const int e0 = min(n_pairs, part * hs.part_entries), e1 = min(n_pairs, e0 + hs.part_entries);
+    const int full_pairs = n_pts >> 1;
+    const float4* s4 = reinterpret_cast<const float4*>(src_xy);
+    const float4* d4 = reinterpret_cast<const float4*>(dst_xy);
     float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;
-    for (int k = threadIdx.x; k < n_pairs; k += kRBlock) {
-        const int i0 = 2 * k, i1 = (2 * k + 1 < n_pts) ? 2 * k + 1 : 2 * k;
-        const float2 s0 = __ldg(src_xy + i0), s1 = __ldg(src_xy + i1);
-        const float2 d0 = __ldg(dst_xy + i0), d1 = __ldg(dst_xy + i1);
-        const float4 A = make_float4(s0.x, s1.x, s0.y, s1.y);
-        const float4 B = make_float4(static_cast<float>(-double(d0.x) * inv_t), static_cast<float>(-double(d1.x) * inv_t),
-                                     static_cast<float>(-double(d0.y) * inv_t), static_cast<float>(-double(d1.y) * inv_t));
-        tb[2 * k] = A; tb[2 * k + 1] = B;
-        m0 = fmaxf(m0, fmaxf(fabsf(A.x), fabsf(A.y)));
-        m1 = fmaxf(m1, fmaxf(fabsf(A.z), fabsf(A.w)));
-        m2 = fmaxf(m2, fmaxf(fabsf(B.x), fabsf(B.y)));
-        m3 = fmaxf(m3, fmaxf(fabsf(B.z), fabsf(B.w)));
+    unsigned n_in = 0, n64 = 0, n_band = 0;
+    for (int base = 0; base < n_pairs; base += 4 * kTinyThreads) {
+        float4 sv[4], dv[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int k = base + u * kTinyThreads + threadIdx.x;
+            if (k < full_pairs) { sv[u] = __ldg(s4 + k); dv[u] = __ldg(d4 + k); }
+            else if (k < n_pairs) {                                                       // odd tail point, duplicated
+                const float2 a = __ldg(src_xy + 2 * k), b = __ldg(dst_xy + 2 * k);
+                sv[u] = make_float4(a.x, a.y, a.x, a.y); dv[u] = make_float4(b.x, b.y, b.x, b.y);
+            } else { sv[u] = make_float4(0.f, 0.f, 0.f, 0.f); dv[u] = sv[u]; }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int k = base + u * kTinyThreads + threadIdx.x;
+            const float4 A = make_float4(sv[u].x, sv[u].z, sv[u].y, sv[u].w);
+            const float4 B = make_float4(static_cast<float>(-double(dv[u].x) * inv_t), static_cast<float>(-double(dv[u].z) * inv_t),
+                                         static_cast<float>(-double(dv[u].y) * inv_t), static_cast<float>(-double(dv[u].w) * inv_t));
+            if (k < n_pairs) {
+                float4* e = tb + kTinyEntry * k;
+                e[0] = A; e[1] = B; e[2] = make_float4(dv[u].x, dv[u].z, dv[u].y, dv[u].w);
+            }
+            m0 = fmaxf(m0, fmaxf(fabsf(A.x), fabsf(A.y)));
+            m1 = fmaxf(m1, fmaxf(fabsf(A.z), fabsf(A.w)));
+            m2 = fmaxf(m2, fmaxf(fabsf(B.x), fabsf(B.y)));
+            m3 = fmaxf(m3, fmaxf(fabsf(B.z), fabsf(B.w)));
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -690,108 +853,185 @@ ransac_tiny_kernel(const float2* __restrict__ src_xy, const float2* __restrict__
     }
     if (lane == 0) { red[0][wid] = m0; red[1][wid] = m1; red[2][wid] = m2; red[3][wid] = m3; }
     __syncthreads();
+
+    // lane = hypothesis: gather from the table in shared memory, solve, sample check, band
+    float bounds[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
         float m = 0.f;
 #pragma unroll
-        for (int w = 0; w < kRBlock / 32; ++w) m = fmaxf(m, red[q][w]);
-        cx.bounds[q] = m;
+        for (int w = 0; w < kTinyWarps; ++w) m = fmaxf(m, red[q][w]);
+        bounds[q] = m;
     }
-
     HypConst hc;
-    double Hn[9];
-    bool ok = make_hypothesis(s, d, inv_t, cx.bounds, Hn, hc) && active;
-    bool rejected = false;
-    if ((hs.flags & HG_RANSAC_REJECT_DEGENERATE) && active && sample_rejected(s, d, hs.reject_lim2)) {
-        ok = false; rejected = true;
+    double Hraw[9], Hn[9];
+    bool usable, rejected = false;                   // usable: H finite and non-zero, sample not rejected
+    {
+        double s[8], d[8];
+        const int ids[4] = { id.x, id.y, id.z, id.w };
 #pragma unroll
-        for (int k = 0; k < 9; ++k) hc.h[k] = 0.f;
-        hc.h[2] = 1.f; hc.Bc = 0.f; hc.thr = 0u; hc.K = 0.f; hc.K0 = 0.f;
+        for (int k = 0; k < 4; ++k) {                // point p: entry p >> 1, half p & 1 of A = (sx0, sx1, sy0, sy1), D = (dx0, dx1, dy0, dy1)
+            const float* e = reinterpret_cast<const float*>(tb + kTinyEntry * (ids[k] >> 1)) + (ids[k] & 1);
+            s[2 * k] = e[0]; s[2 * k + 1] = e[2]; d[2 * k] = e[8]; d[2 * k + 1] = e[10];
+        }
+        usable = solve_for_sweep(s, d, inv_t, Hraw, Hn, hc);
+        if ((hs.flags & HG_RANSAC_REJECT_DEGENERATE) && active && sample_rejected(s, d, hs.reject_lim2)) { usable = false; rejected = true; }
     }
-    cx.src_xy = src_xy; cx.dst_xy = dst_xy; cx.table = nullptr; cx.inv_t = inv_t; cx.t = t;
-    cx.queue = queue + threadIdx.x; cx.n64 = 0u;
+    const bool ok = usable && active;
+    error_band(bounds, usable, hc);                  // unusable: every point a sure outlier
 
-    // slice of this warp: whole groups of kGroup entries, the last slice takes the remainder and the odd tail point
-    const int full_pairs = n_pts >> 1;
-    const int per = ((n_pairs + kTinySlices - 1) / kTinySlices + kGroup - 1) / kGroup * kGroup;
-    const int e_begin = min(n_pairs, wid * per), e_end = min(n_pairs, e_begin + per);
-    unsigned n_in = 0, qn = 0, n_band = 0;
-    if (hs.flags & HG_RANSAC_DECIDE_ALL_F64) {
-        if (active) n_in = count_all_f64(cx, 2 * e_begin, min(n_pts, 2 * e_end));
+    // quarter of this warp: whole groups of kGroup entries; the last non-empty quarter takes the remainder and the odd tail point
+    const int per = ((e1 - e0 + kTinyWarps - 1) / kTinyWarps + kGroup - 1) / kGroup * kGroup;
+    const int w0 = min(e1, e0 + wid * per), w1 = min(e1, w0 + per);
+    unsigned qn = 0;
+    if (hs.flags & HG_RANSAC_DECIDE_ALL_F64) {       // verification mode: every pair by the definition in fp64
+        if (active) {
+            for (int k = w0; k < w1; ++k) {
+                const float4* e = tb + kTinyEntry * k;
+                const float4 A = e[0], D = e[2];
+                n_in += inlier_f64_nodiv(Hn, A.x, A.z, D.x, D.z, t) ? 1u : 0u;
+                ++n64;
+                if (2 * k + 1 < n_pts) { n_in += inlier_f64_nodiv(Hn, A.y, A.w, D.y, D.w, t) ? 1u : 0u; ++n64; }
+            }
+        }
     } else {
-        const int e_two = min(e_end, full_pairs);
-        int k = e_begin;
+        const int e_two = min(w1, full_pairs);
+        int k = w0;
 #pragma unroll 1
         for (; k + kGroup <= e_two; k += kGroup)
-            sweep_group<kGroup, false, false>(hc, tb, 2 * k, 2 * k, cx, n_in, qn, n_band);
+            tiny_group<kGroup, false>(hc, tb, k, queue, n_in, qn);
 #pragma unroll 1
         for (; k < e_two; ++k)
-            sweep_group<1, false, false>(hc, tb, 2 * k, 2 * k, cx, n_in, qn, n_band);
-        if ((n_pts & 1) && full_pairs >= e_begin && full_pairs < e_end)
-            sweep_group<1, true, false>(hc, tb, 2 * full_pairs, 2 * full_pairs, cx, n_in, qn, n_band);
+            tiny_group<1, false>(hc, tb, k, queue, n_in, qn);
+        if ((n_pts & 1) && full_pairs >= w0 && full_pairs < w1)
+            tiny_group<1, true>(hc, tb, full_pairs, queue, n_in, qn);
+        // the pairs noted during the sweep, all lanes of the warp side by side
         if (__any_sync(0xffffffffu, qn != 0u)) {
-            unsigned ovf = __ballot_sync(0xffffffffu, qn > kQueueCap);
-            if (rejected) cx.id = make_int4(0, 0, 0, 0);
-            if (qn != 0u && qn <= kQueueCap) n_in += drain_queue(cx, qn);
-            while (ovf) {
-                const int L = __ffs(ovf) - 1;
-                ovf &= ovf - 1u;
-                const unsigned c = recount_warp<true>(cx, L, 2 * e_begin, min(n_pts, 2 * e_end));
-                if (lane == L) n_in = c;
+            if (qn <= kQueueCap) {
+                for (unsigned j = 0; j < qn; ++j) {
+                    const unsigned item = queue[j * kTinyThreads];
+                    unsigned m = item & 0xffffu;
+                    while (m) {
+                        const int i = __ffs(m) - 1;
+                        m &= m - 1u;
+                        // (a noted pair has a value >= 0: the sweep has not counted it)
+                        n_in += tiny_inlier_f64(Hn, t, tb + kTinyEntry * ((item >> 16) + (i >> 1)), i & 1);
+                        ++n64;
+                    }
+                }
+            } else {                                  // queue overflow: this thread's slice again, every pair in fp64
+                n_in = 0;
+                for (int e = w0; e < w1; ++e)
+                    for (unsigned hi = 0; hi < 2u && 2 * e + static_cast<int>(hi) < n_pts; ++hi) { n_in += tiny_inlier_f64(Hn, t, tb + kTinyEntry * e, hi); ++n64; }
             }
+            n_band = n64;
         }
     }
     partial[wid][lane] = ok ? n_in : 0u;
-    {   // statistics
-        const unsigned n64 = active ? cx.n64 : 0u;
-        const unsigned amb_mask = __ballot_sync(0xffffffffu, n64 != 0u);
-        const unsigned tot = __reduce_add_sync(0xffffffffu, n64);
-        const unsigned band_tot = __reduce_add_sync(0xffffffffu, active ? n_band : 0u);
-        if (lane == 0) {
-            if (amb_mask) { atomicAdd(&hdr->n_fixup, static_cast<unsigned long long>(__popc(amb_mask)));
-                            atomicAdd(&hdr->n_pairs_f64, static_cast<unsigned long long>(tot)); }
-            if (band_tot) atomicAdd(&hdr->n_band, static_cast<unsigned long long>(band_tot));
-        }
+    // the group's leader warp: every lane's candidate, the unit-Frobenius H (raw ACA scale normalised, as ransac_finalize_kernel does)
+    float hcand[9];
+    if (part == 0 && wid == 0) {
+        normalise<double>(Hraw, 2);
+#pragma unroll
+        for (int k = 0; k < 9; ++k) hcand[k] = static_cast<float>(Hraw[k]);
     }
+    grid_dependency_wait();                                   // the header is zero from here on
     __syncthreads();
-    if (wid != 0) return;
     unsigned total = 0;
+    if (wid == 0) {
 #pragma unroll
-    for (int w = 0; w < kTinySlices; ++w) total += partial[w][lane];
-    unsigned long long key = 0ull;
-    if (active) {
-        if (counts) counts[hidx] = static_cast<int>(total);
-        key = pack_key(total, static_cast<unsigned>(hidx));
+        for (int w = 0; w < kTinyWarps; ++w) total += partial[w][lane];
     }
-    const unsigned nrej = __popc(__ballot_sync(0xffffffffu, rejected));
-    const unsigned long long cta_key = warp_max_u64(key);
-    if (key == cta_key && active && best_H) {                // the CTA's candidate: this lane's own H, unit Frobenius
-        double H[9];
-        aca_solve<double>(s, d, H);                           // raw scale, as ransac_finalize_kernel normalises it
-        normalise<double>(H, 2);
-#pragma unroll
-        for (int k = 0; k < 9; ++k) cand[9 * blockIdx.x + k] = static_cast<float>(H[k]);
+    if (parts > 1) {                                          // the parts of this group meet in the rank-0 CTA
+        if (wid != 0) { tiny_stats(hdr, n64, n_band); return; }
+        if (part != 0) {
+            cluster_wait_acquire();
+            st_async_cluster_u32(&cl_partial[part][lane], &cl_bar, 0u, total);
+            tiny_stats(hdr, n64, n_band);
+            return;
+        }
+        mbar_wait(&cl_bar, 0);
+        for (int q = 1; q < parts; ++q) total += cl_partial[q][lane];
     }
-    if (lane == 0) {
-        if (cta_key != 0ull) atomicMax(&hdr->best_key, cta_key);
-        if (nrej) atomicAdd(&hdr->n_rejected, static_cast<unsigned long long>(nrej));
-    }
-    __threadfence();
-    __syncwarp();
+    if (wid != 0) { tiny_stats(hdr, n64, n_band); return; }
+    // The lane that holds the group's best hypothesis (largest count, lowest index = lowest lane) publishes the slot and, in
+    // the same breath, takes the ticket (see TinySlot: stamped words, no fence in between).
+    const unsigned cnt_max = __reduce_max_sync(0xffffffffu, active ? total : 0u);
+    const int wl = __ffs(__ballot_sync(0xffffffffu, active && total == cnt_max)) - 1;
     unsigned ticket = 0;
-    if (lane == 0) ticket = atomicAdd(&hdr->blocks_done, 1u);
-    ticket = __shfl_sync(0xffffffffu, ticket, 0);
-    if (ticket != gridDim.x - 1) return;
-    __threadfence();
-    const unsigned long long best = *reinterpret_cast<volatile unsigned long long*>(&hdr->best_key);
-    const unsigned bidx = 0xFFFFFFFFu - static_cast<unsigned>(best & 0xFFFFFFFFull);
-    if (lane == 0) {
-        if (best_index) *best_index = static_cast<long long>(bidx);
-        if (best_count) *best_count = static_cast<int>(best >> 32);
+    if (lane == wl) {
+        const unsigned long long key = pack_key(total, static_cast<unsigned>(hidx));
+        unsigned long long* sl = slots[blockIdx.x].w;
+        st_relaxed_gpu_u64(sl + 0, stamped(static_cast<unsigned>(key)));
+        st_relaxed_gpu_u64(sl + 1, stamped(static_cast<unsigned>(key >> 32)));
+#pragma unroll
+        for (int k = 0; k < 9; ++k) st_relaxed_gpu_u64(sl + 2 + k, stamped(__float_as_uint(hcand[k])));
+        ticket = atomicAdd(&hdr->blocks_done, 1u);
     }
-    if (best_H && lane < 9) {
-        const unsigned blk = static_cast<unsigned>((static_cast<long long>(bidx) - hs.h0) / kTinyHyp);
-        best_H[lane] = __ldcg(cand + 9 * blk + lane);
+    if (active && counts) counts[hidx] = static_cast<int>(total);
+    const unsigned nrej = __popc(__ballot_sync(0xffffffffu, rejected));
+    if (lane == 0 && nrej) atomicAdd(&hdr->n_rejected, static_cast<unsigned long long>(nrej));
+    tiny_stats(hdr, n64, n_band);
+    ticket = __shfl_sync(0xffffffffu, ticket, wl);
+    if (ticket != gridDim.x - 1) return;
+    // the last group: every group has issued its slot; the best slot of all
+    const int n_groups = static_cast<int>(gridDim.x);
+    if (n_groups <= 32) {                                     // one slot per lane, key and H in one round trip
+        unsigned long long w[kSlotWords];
+        unsigned long long bk = 0ull;
+        if (lane < n_groups) {
+            const unsigned long long* sl = slots[lane].w;
+            bool all;
+            do {
+                all = true;
+#pragma unroll
+                for (int k = 0; k < kSlotWords; ++k) { w[k] = ld_relaxed_gpu_u64(sl + k); all = all && static_cast<unsigned>(w[k] >> 32) == kSlotStamp; }
+            } while (!all);
+            bk = (static_cast<unsigned long long>(static_cast<unsigned>(w[1])) << 32) | static_cast<unsigned>(w[0]);
+        }
+        const unsigned long long best = warp_max_u64(bk);
+        if (bk == best && best != 0ull) {
+            hdr->best_key = best;
+            if (best_index) *best_index = static_cast<long long>(0xFFFFFFFFu - static_cast<unsigned>(best & 0xFFFFFFFFull));
+            if (best_count) *best_count = static_cast<int>(best >> 32);
+            if (best_H) {
+#pragma unroll
+                for (int k = 0; k < 9; ++k) best_H[k] = __uint_as_float(static_cast<unsigned>(w[2 + k]));
+            }
+        }
+    } else {                                                  // keys first (four slots per lane in flight), then the winner's H
+        unsigned long long bk = 0ull;
+        int bg = 0;
+        for (int base = 0; base < n_groups; base += 128) {
+            unsigned long long lo[4], hi[4];
+            bool all;
+            do {
+                all = true;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int g = min(base + 32 * u + lane, n_groups - 1);
+                    lo[u] = ld_relaxed_gpu_u64(slots[g].w); hi[u] = ld_relaxed_gpu_u64(slots[g].w + 1);
+                    all = all && static_cast<unsigned>(lo[u] >> 32) == kSlotStamp && static_cast<unsigned>(hi[u] >> 32) == kSlotStamp;
+                }
+            } while (!all);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const unsigned long long k64 = (static_cast<unsigned long long>(static_cast<unsigned>(hi[u])) << 32) | static_cast<unsigned>(lo[u]);
+                if (k64 > bk) { bk = k64; bg = min(base + 32 * u + lane, n_groups - 1); }
+            }
+        }
+        const unsigned long long best = warp_max_u64(bk);
+        bg = __shfl_sync(0xffffffffu, bg, __ffs(__ballot_sync(0xffffffffu, bk == best)) - 1);
+        if (lane < 9 && best_H) {
+            unsigned long long w;
+            do { w = ld_relaxed_gpu_u64(slots[bg].w + 2 + lane); } while (static_cast<unsigned>(w >> 32) != kSlotStamp);
+            best_H[lane] = __uint_as_float(static_cast<unsigned>(w));
+        }
+        if (lane == 0) {
+            hdr->best_key = best;
+            if (best_index) *best_index = static_cast<long long>(0xFFFFFFFFu - static_cast<unsigned>(best & 0xFFFFFFFFull));
+            if (best_count) *best_count = static_cast<int>(best >> 32);
+        }
     }
 }
 
@@ -856,9 +1096,19 @@ static size_t table_bytes(int32_t n_pts) { return size_t((n_pts + 1) / 2) * 32; 
 constexpr int kSplitBelowCtas = 148;
 constexpr int kMinPartEntries = 8;
 constexpr int kFusedMaxPts = 4096;      // the one-kernel path packs the whole table in every CTA: tables that fit shared memory
-constexpr int kTinyMaxCtas = 296;         // tiny path: at most two CTAs per SM's worth of 32-hypothesis blocks
-constexpr size_t kTicketBytes = 64;     // so that the accumulator area of the smallest call still holds one 36-byte candidate
+constexpr int kTinyFillCtas = 128;       // tiny path: the table is split further while the call has fewer CTAs than this
+constexpr int kTinyMaxGroups = 296;     // tiny path: at most two CTAs per SM's worth of 32-hypothesis groups
+constexpr size_t kTicketBytes = 128;    // so that the accumulator area of the smallest call still holds one TinySlot
 static bool may_split(int64_t n_hyp) { return (n_hyp + kRBlock - 1) / kRBlock < kSplitBelowCtas; }
+
+// Tiny path: CTAs (table parts) per group of 32 hypotheses -- a power of two <= 8 (the cluster size), doubled while the
+// call does not yet cover the machine and every warp of the last part still gets table entries.
+static int tiny_parts(int n_pairs, int64_t groups)
+{
+    int p = 1;
+    while (p < kTinyMaxParts && groups * p < kTinyFillCtas && n_pairs > (2 * p - 1) * kTinyWarps * kGroup) p *= 2;
+    return p;
+}
 
 // entries per part for a launch of n_hyp hypotheses (>= n_pairs: one part)
 static int part_entries_for(int n_pairs, int64_t n_hyp, int ctas_per_sm = 2)
@@ -943,11 +1193,11 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     const double inv_t = 1.0 / t;
     (void)workspace_bytes;
 
-    if (cudaMemsetAsync(hdr, 0, kHeaderBytes + acc_bytes, st) != cudaSuccess) return HG_ERR_CUDA;     // header, accumulator
-    const int64_t tiny_ctas = (n_hyp + kTinyHyp - 1) / kTinyHyp;
-    if (!adaptive && acc_bytes && n_pts <= kFusedMaxPts && tiny_ctas <= kTinyMaxCtas &&
-        size_t(tiny_ctas) * 9 * sizeof(float) <= acc_bytes) {
-        // tiny call: 32 hypotheses per CTA, the table sliced over its warps; the accumulator area holds the candidates
+    const int64_t tiny_groups = (n_hyp + kTinyHyp - 1) / kTinyHyp;
+    if (!adaptive && acc_bytes && n_pts <= kFusedMaxPts && tiny_groups <= kTinyMaxGroups &&
+        size_t(tiny_groups) * sizeof(TinySlot) <= acc_bytes) {
+        // tiny call: a cluster of CTAs per 32 hypotheses, the table split over the cluster and over the warps of each
+        // CTA; the accumulator area holds the candidates
         HypSource hs;
         hs.idx = reinterpret_cast<const int4*>(hyp_idx);
         hs.idx_out = nullptr;
@@ -957,15 +1207,34 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
         hs.check_stop = 0;
         hs.acc = nullptr;
         hs.h0 = 0; hs.h1 = n_hyp;
-        hs.part_entries = n_pairs;
-        const size_t smem = size_t(n_pairs) * 32 + size_t(kQueueCap) * kRBlock * sizeof(unsigned);
+        const int parts = tiny_parts(n_pairs, tiny_groups);
+        hs.part_entries = ((n_pairs + parts - 1) / parts + 7) & ~7;
+        const size_t smem = size_t(n_pairs) * kTinyEntry * sizeof(float4) + size_t(kQueueCap) * kTinyThreads * sizeof(unsigned);
         if (cudaFuncSetAttribute(ransac_tiny_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
             return HG_ERR_CUDA;
-        ransac_tiny_kernel<<<static_cast<unsigned>(tiny_ctas), kRBlock, smem, st>>>(
-            s2, d2, n_pts, n_pairs, hs, inv_t, t, counts, hdr, reinterpret_cast<float*>(ws + kHeaderBytes), best_H,
-            reinterpret_cast<long long*>(best_index), best_count);
+        ransac_zero_kernel<<<1, 256, 0, st>>>(reinterpret_cast<uint4*>(hdr), int((kHeaderBytes + size_t(tiny_groups) * sizeof(TinySlot)) / 16));
+        if (launch_status() != HG_OK) return HG_ERR_CUDA;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(static_cast<unsigned>(tiny_groups), static_cast<unsigned>(parts), 1);
+        cfg.blockDim = dim3(kTinyThreads, 1, 1);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attrs[2];
+        attrs[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;      // may start while the zero kernel runs
+        attrs[0].val.programmaticStreamSerializationAllowed = 1;
+        attrs[1].id = cudaLaunchAttributeClusterDimension;
+        attrs[1].val.clusterDim.x = 1; attrs[1].val.clusterDim.y = static_cast<unsigned>(parts); attrs[1].val.clusterDim.z = 1;
+        cfg.attrs = attrs;
+        cfg.numAttrs = parts > 1 ? 2 : 1;
+        TinySlot* cand = reinterpret_cast<TinySlot*>(ws + kHeaderBytes);
+        if (cudaLaunchKernelEx(&cfg, ransac_tiny_kernel, s2, d2, n_pts, n_pairs, hs, inv_t, t, counts, hdr, cand, best_H,
+                               reinterpret_cast<long long*>(best_index), best_count) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return HG_ERR_CUDA;
+        }
         return launch_status();
     }
+    if (cudaMemsetAsync(hdr, 0, kHeaderBytes + acc_bytes, st) != cudaSuccess) return HG_ERR_CUDA;     // header, accumulator
     {
         int blocks = (n_pairs + 255) / 256;
         if (blocks > 1184) blocks = 1184;

@@ -207,3 +207,30 @@ def test_build_log_has_no_warnings_and_no_unexpected_spills():
         m = re.search(r"(\d+) bytes spill stores, (\d+) bytes spill loads", line)
         if m and (int(m.group(1)) or int(m.group(2))):
             assert current is not None and any(a in current for a in allowed), (current, line.strip())
+
+
+def test_sass_of_the_hot_loops_keeps_its_operand_paths():
+    """Codegen that the measured numbers rest on and that an unrelated edit can silently change (it happened: a shorter
+    cold-path helper made ptxas move the table operands of the RANSAC sweep from uniform registers to per-thread constant
+    loads, 1.67 -> 2.25 ms on C4).  Checked on the built library with cuobjdump: the constant-bank sweep reads its table
+    with LDCU.64 (uniform datapath), the staged sweep and the bulk copies are there, the tiny-call kernel has its cluster /
+    async-store / dependent-launch instructions and no spill."""
+    import shutil
+    import subprocess
+    from paper_2402_18008_b200 import _build
+    exe = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    lib = _build.build()
+
+    def sass(fun):
+        r = subprocess.run([exe, "-sass", "-fun", fun, str(lib)], capture_output=True, text=True)
+        assert r.returncode == 0 and "Function" in r.stdout, r.stderr[:300]
+        return r.stdout
+
+    const = sass("_ZN2hg19ransac_score_kernelILb1EEEvPK6float2S3_iPK6float4iNS_9HypSourceEddPiPNS_12RansacHeaderE")
+    assert const.count("LDCU.64") >= 32 and const.count("c[0x3]") >= 32      # 8 entries x (2 + 2) 64-bit halves per group
+    assert const.count("FFMA2") >= 88
+    staged = sass("_ZN2hg19ransac_score_kernelILb0EEEvPK6float2S3_iPK6float4iNS_9HypSourceEddPiPNS_12RansacHeaderE")
+    assert "UBLKCP" in staged and "SYNCS" in staged and staged.count("FFMA2") >= 88
+    tiny = sass("_ZN2hg18ransac_tiny_kernelEPK6float2S2_iiNS_9HypSourceEddPiPNS_12RansacHeaderEPNS_8TinySlotEPfPxS4_")
+    assert "UCGABAR_ARV" in tiny and "ACQBULK" in tiny and tiny.count("FFMA2") >= 88
+    assert "MEMBAR.SC" not in tiny                                           # no fence between the slot stores and the ticket

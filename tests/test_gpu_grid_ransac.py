@@ -294,3 +294,68 @@ def test_ransac_sample_check_all_rejected_and_adaptive():
     assert (counts[rej] == 0).all() and hg.ransac_stats(a["workspace"])["n_rejected"] == int(rej.sum())
     assert (np.abs(counts.astype(np.int64) - ref["counts"]) <= ref["band_counts"]).all()
     assert 0.3 < rej.mean() < 0.99
+
+
+# ---- tiny calls (the scale of the paper's Table 6): zero kernel + clustered one-kernel path ---------------------
+# (n_pts, n_hyp) chosen so that every cluster size of the tiny path is taken: 1 (many groups / tiny tables), 2, 4, 8
+@pytest.mark.parametrize("n_pts,n_hyp", [(1000, 1024), (500, 256), (4096, 9472), (4096, 40), (999, 33), (4095, 2100),
+                                         (64, 5000), (37, 31), (131, 200), (263, 96), (5, 7)])
+def test_ransac_tiny_calls_every_cluster_size(n_pts, n_hyp):
+    wl = W.ransac_workload(n_pts=n_pts, n_hyp=n_hyp, seed=W.SEED_BASE + 300 + n_pts + n_hyp)
+    s, d, idx = wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV)
+    out = hg.hg_ransac_hypothesize_score(s, d, idx, 3.0)
+    ref = oracle.ransac(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy(), 3.0, band_rel=1e-4)
+    check_ransac(wl, 3.0, out, ref)
+    slow = hg.hg_ransac_hypothesize_score(s, d, idx, 3.0, decide_all_f64=True)            # the band, bit for bit
+    assert torch.equal(out["counts"], slow["counts"]) and torch.equal(out["best_H"], slow["best_H"])
+    assert out["best_index"].item() == slow["best_index"].item()
+    assert hg.ransac_stats(slow["workspace"])["n_pairs_f64"] == n_pts * n_hyp
+    rej = oracle.sample_check(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy(), 50.0)
+    chk = hg.hg_ransac_hypothesize_score(s, d, idx, 3.0, reject_degenerate=True, min_area_px2=50.0)
+    cc = chk["counts"].cpu().numpy()
+    assert hg.ransac_stats(chk["workspace"])["n_rejected"] == int(rej.sum())
+    assert (cc[rej] == 0).all() and np.array_equal(cc[~rej], out["counts"].cpu().numpy()[~rej])
+    assert chk["best_count"].item() == cc.max() and chk["best_index"].item() == int(np.argmax(cc))
+
+
+def test_ransac_tiny_call_replayed_in_a_cuda_graph():
+    """The zero kernel and its programmatic dependent are captured as two graph nodes; every replay must start from a
+    clean header (ticket, packed maximum) and see the inputs of that replay."""
+    n_pts, n_hyp = 1000, 1024
+    wls = [W.ransac_workload(n_pts=n_pts, n_hyp=n_hyp, seed=900 + k) for k in range(3)]
+    s, d, idx = (wls[0][k].to(DEV).clone() for k in ("src_xy", "dst_xy", "hyp_idx"))
+    ws = torch.empty(hg.hg_ransac_workspace_bytes(n_pts, n_hyp), dtype=torch.uint8, device=DEV)
+    first = hg.hg_ransac_hypothesize_score(s, d, idx, 3.0, workspace=ws)
+    keep = (first["best_H"], first["best_index"], first["best_count"])
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(3):                                  # back-to-back calls on one workspace inside the graph
+                hg.hg_ransac_hypothesize_score(s, d, idx, 3.0, counts=first["counts"], workspace=ws, best=keep)
+    for wl in wls[::-1]:
+        s.copy_(wl["src_xy"]); d.copy_(wl["dst_xy"]); idx.copy_(wl["hyp_idx"])
+        g.replay()
+        torch.cuda.synchronize()
+        ref = oracle.ransac(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy(), 3.0, band_rel=1e-4)
+        check_ransac(wl, 3.0, first, ref)
+
+
+@pytest.mark.parametrize("n_pts,n_hyp", [(1200, 2048), (601, 320), (4096, 64)])
+def test_ransac_tiny_call_pairs_exactly_at_the_threshold(n_pts, n_hyp):
+    """The at-threshold adversary on the tiny path: half the points have residual t (1 +- 1e-16) under every hypothesis, so
+    every thread's queue of noted pairs overflows and it recounts its slice in fp64; counts must equal the all-fp64 mode."""
+    t = 2.0
+    g = torch.Generator().manual_seed(11 + n_pts)
+    s = torch.rand((n_pts, 2), generator=g) * 600.0
+    d = s.clone()
+    d[n_pts // 2:, 0] += t
+    idx = torch.stack([torch.randperm(n_pts // 2, generator=g)[:4] for _ in range(n_hyp)]).to(torch.int32)
+    fast = hg.hg_ransac_hypothesize_score(s.to(DEV), d.to(DEV), idx.to(DEV), t)
+    slow = hg.hg_ransac_hypothesize_score(s.to(DEV), d.to(DEV), idx.to(DEV), t, decide_all_f64=True)
+    assert torch.equal(fast["counts"], slow["counts"]) and torch.equal(fast["best_H"], slow["best_H"])
+    assert fast["best_index"].item() == slow["best_index"].item() and (fast["counts"] >= n_pts // 2).all()
+    assert hg.ransac_stats(fast["workspace"])["n_pairs_f64"] >= 0.4 * n_pts * n_hyp
+    ref = oracle.ransac(s.numpy(), d.numpy(), idx.numpy(), t, band_rel=1e-4)
+    assert (np.abs(fast["counts"].cpu().numpy().astype(np.int64) - ref["counts"]) <= ref["band_counts"]).all()

@@ -457,13 +457,13 @@ def run_next_rows(hg, W, dev, peak, peak_src):
     img = torch.rand((k, 1, 128, 128), device=dev)
     out = torch.empty_like(img)
     leg("warp_c5_1ch", lambda: hg.hg_offsets_to_warp(off5, 0.0, 0.0, 127.0, 127.0, 128, 128, img, warped=out), 8, k * 128 * 128,
-        unit="pixels", kernel="hg::offsets_to_warp_kernel<1,true>")
+        unit="pixels", kernel="hg::offsets_to_warp_plane_kernel")
     del img, out
     k3 = 4096
     img3 = torch.rand((k3, 3, 128, 128), device=dev)
     out3 = torch.empty_like(img3)
     leg("warp_c5_3ch", lambda: hg.hg_offsets_to_warp(off5[:k3], 0.0, 0.0, 127.0, 127.0, 128, 128, img3, warped=out3), 8, k3 * 3 * 128 * 128,
-        unit="pixels x channels", kernel="hg::offsets_to_warp_kernel<3,...>")
+        unit="pixels x channels", kernel="hg::offsets_to_warp_plane_kernel (one CTA per item and channel)")
     return ex
 
 

@@ -730,16 +730,36 @@ __device__ __forceinline__ unsigned tiny_inlier_f64(const double Hn[9], double t
     return inlier_f64_nodiv(Hn, hi ? A.y : A.x, hi ? A.w : A.z, hi ? D.y : D.x, hi ? D.w : D.z, t) ? 1u : 0u;
 }
 
+// The noted pairs of this thread (queue items: first entry of the group << 16 | 16 flags, bit 2g + j = point j of entry
+// k0 + g) by the definition in fp64; returns the number of inliers among them.  Out of line and with H by value: one copy
+// of the code, H stays in registers at the call sites.
+__device__ __noinline__ unsigned tiny_drain(const float4* __restrict__ tb, const unsigned* __restrict__ queue, unsigned qn, double t,
+                                            double h0, double h1, double h2, double h3, double h4, double h5, double h6, double h7, double h8)
+{
+    const double Hn[9] = { h0, h1, h2, h3, h4, h5, h6, h7, h8 };
+    unsigned n = 0;
+    for (unsigned j = 0; j < qn; ++j) {
+        const unsigned item = queue[j * kTinyThreads];
+        unsigned m = item & 0xffffu;
+        while (m) {
+            const int i = __ffs(m) - 1;
+            m &= m - 1u;
+            n += tiny_inlier_f64(Hn, t, tb + kTinyEntry * ((item >> 16) + (i >> 1)), i & 1);   // (a noted pair has a value >= 0: the sweep has not counted it)
+        }
+    }
+    return n;
+}
+
 // G consecutive entries (2G points) from entry k0 of the table `tb`, against one hypothesis.  The fast path is the one of
 // sweep_group.  When a pair of the group lies inside the table-wide band the thread only notes (k0, which of the 2G points)
 // in its own queue -- branch-free flags and one store: what a lone warp per scheduler pays for a divergent excursion is
 // its latency, not its instruction count -- and the warp decides the noted pairs after the sweep, all lanes side by side,
 // straight by the definition in fp64 (cheap since it needs no division; the per-pair fp32 band of the big kernel would
-// cost as much as it saves here).  `qn` counts the groups noted; beyond kQueueCap they are dropped and the thread
-// recounts its slice afterwards.
+// cost as much as it saves here).  A thread whose queue is full (a hypothesis with a horizon line through the table)
+// drains it on the spot and goes on.  `n64` counts the pairs noted = decided in fp64.
 template <int G, bool ONLY_X>
-__device__ __forceinline__ void tiny_group(const HypConst& hc, const float4* __restrict__ tb, int k0, unsigned* __restrict__ queue,
-                                           unsigned& n_in, unsigned& qn)
+__device__ __forceinline__ void tiny_group(const HypConst& hc, const double Hn[9], double t, const float4* __restrict__ tb, int k0,
+                                           unsigned* __restrict__ queue, unsigned& n_in, unsigned& qn, unsigned& n64)
 {
     float2 a[G];
     bool amb = false;
@@ -761,8 +781,13 @@ __device__ __forceinline__ void tiny_group(const HypConst& hc, const float4* __r
             mask |= (__float_as_uint(a[g].x) <= hc.thr) ? (1u << (2 * g)) : 0u;
             if (!ONLY_X) mask |= (__float_as_uint(a[g].y) <= hc.thr) ? (2u << (2 * g)) : 0u;
         }
-        if (qn < kQueueCap) queue[qn * kTinyThreads] = (static_cast<unsigned>(k0) << 16) | mask;
+        if (qn == kQueueCap) {
+            n_in += tiny_drain(tb, queue, qn, t, Hn[0], Hn[1], Hn[2], Hn[3], Hn[4], Hn[5], Hn[6], Hn[7], Hn[8]);
+            qn = 0u;
+        }
+        queue[qn * kTinyThreads] = (static_cast<unsigned>(k0) << 16) | mask;
         ++qn;
+        n64 += __popc(mask);
     }
 }
 
@@ -899,33 +924,15 @@ ransac_tiny_kernel(const float2* __restrict__ src_xy, const float2* __restrict__
         int k = w0;
 #pragma unroll 1
         for (; k + kGroup <= e_two; k += kGroup)
-            tiny_group<kGroup, false>(hc, tb, k, queue, n_in, qn);
+            tiny_group<kGroup, false>(hc, Hn, t, tb, k, queue, n_in, qn, n64);
 #pragma unroll 1
         for (; k < e_two; ++k)
-            tiny_group<1, false>(hc, tb, k, queue, n_in, qn);
+            tiny_group<1, false>(hc, Hn, t, tb, k, queue, n_in, qn, n64);
         if ((n_pts & 1) && full_pairs >= w0 && full_pairs < w1)
-            tiny_group<1, true>(hc, tb, full_pairs, queue, n_in, qn);
+            tiny_group<1, true>(hc, Hn, t, tb, full_pairs, queue, n_in, qn, n64);
         // the pairs noted during the sweep, all lanes of the warp side by side
-        if (__any_sync(0xffffffffu, qn != 0u)) {
-            if (qn <= kQueueCap) {
-                for (unsigned j = 0; j < qn; ++j) {
-                    const unsigned item = queue[j * kTinyThreads];
-                    unsigned m = item & 0xffffu;
-                    while (m) {
-                        const int i = __ffs(m) - 1;
-                        m &= m - 1u;
-                        // (a noted pair has a value >= 0: the sweep has not counted it)
-                        n_in += tiny_inlier_f64(Hn, t, tb + kTinyEntry * ((item >> 16) + (i >> 1)), i & 1);
-                        ++n64;
-                    }
-                }
-            } else {                                  // queue overflow: this thread's slice again, every pair in fp64
-                n_in = 0;
-                for (int e = w0; e < w1; ++e)
-                    for (unsigned hi = 0; hi < 2u && 2 * e + static_cast<int>(hi) < n_pts; ++hi) { n_in += tiny_inlier_f64(Hn, t, tb + kTinyEntry * e, hi); ++n64; }
-            }
-            n_band = n64;
-        }
+        if (qn) n_in += tiny_drain(tb, queue, qn, t, Hn[0], Hn[1], Hn[2], Hn[3], Hn[4], Hn[5], Hn[6], Hn[7], Hn[8]);
+        n_band = n64;
     }
     partial[wid][lane] = ok ? n_in : 0u;
     // the group's leader warp: every lane's candidate, the unit-Frobenius H (raw ACA scale normalised, as ransac_finalize_kernel does)
@@ -1097,7 +1104,9 @@ constexpr int kSplitBelowCtas = 148;
 constexpr int kMinPartEntries = 8;
 constexpr int kFusedMaxPts = 4096;      // the one-kernel path packs the whole table in every CTA: tables that fit shared memory
 constexpr int kTinyFillCtas = 128;       // tiny path: the table is split further while the call has fewer CTAs than this
-constexpr int kTinyMaxGroups = 296;     // tiny path: at most two CTAs per SM's worth of 32-hypothesis groups
+constexpr int kTinyMaxGroups = 296;     // tiny path: at most two CTAs per SM's worth of 32-hypothesis groups ...
+constexpr int kTinyMaxGroupsWide = 640; // ... and up to 20 480 hypotheses on tables of <= kTinyWidePts points, where it still beats the
+constexpr int kTinyWidePts = 2048;      //     five launches of the generic path (16 384 x 2000: 30.6 vs 36.5 us; 37 888 x 2000: 56 vs 52)
 constexpr size_t kTicketBytes = 128;    // so that the accumulator area of the smallest call still holds one TinySlot
 static bool may_split(int64_t n_hyp) { return (n_hyp + kRBlock - 1) / kRBlock < kSplitBelowCtas; }
 
@@ -1194,7 +1203,7 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     (void)workspace_bytes;
 
     const int64_t tiny_groups = (n_hyp + kTinyHyp - 1) / kTinyHyp;
-    if (!adaptive && acc_bytes && n_pts <= kFusedMaxPts && tiny_groups <= kTinyMaxGroups &&
+    if (!adaptive && acc_bytes && n_pts <= kFusedMaxPts && tiny_groups <= (n_pts <= kTinyWidePts ? kTinyMaxGroupsWide : kTinyMaxGroups) &&
         size_t(tiny_groups) * sizeof(TinySlot) <= acc_bytes) {
         // tiny call: a cluster of CTAs per 32 hypotheses, the table split over the cluster and over the warps of each
         // CTA; the accumulator area holds the candidates

@@ -299,7 +299,8 @@ def test_ransac_sample_check_all_rejected_and_adaptive():
 # ---- tiny calls (the scale of the paper's Table 6): zero kernel + clustered one-kernel path ---------------------
 # (n_pts, n_hyp) chosen so that every cluster size of the tiny path is taken: 1 (many groups / tiny tables), 2, 4, 8
 @pytest.mark.parametrize("n_pts,n_hyp", [(1000, 1024), (500, 256), (4096, 9472), (4096, 40), (999, 33), (4095, 2100),
-                                         (64, 5000), (37, 31), (131, 200), (263, 96), (5, 7)])
+                                         (64, 5000), (37, 31), (131, 200), (263, 96), (5, 7),
+                                         (2000, 16384), (2047, 20480)])               # the wide range of the one-kernel path
 def test_ransac_tiny_calls_every_cluster_size(n_pts, n_hyp):
     wl = W.ransac_workload(n_pts=n_pts, n_hyp=n_hyp, seed=W.SEED_BASE + 300 + n_pts + n_hyp)
     s, d, idx = wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV)

@@ -279,6 +279,9 @@ def run_extras(hg, W, dev, src, dst, H, peak, peak_src, cpu=True):
         for _ in range(5):
             f1()
         row = {"us_per_call_launch": event_time_ms(f1, 200) / 200 * 1e3}
+        with hg.CallPlan() as plan1:              # the same call recorded once: a ctypes call per iteration, no marshalling
+            f1()
+        row["us_per_call_plan"] = event_time_ms(plan1, 200) / 200 * 1e3
         try:
             g = graph_of([f1] * 20)
             row["us_per_call_graph"] = event_time_ms(g.replay, 20) / (20 * 20) * 1e3
@@ -355,6 +358,9 @@ def run_extras(hg, W, dev, src, dst, H, peak, peak_src, cpu=True):
         for _ in range(5):
             fs()
         row = {"n_pts": n_pts_s, "n_hyp": n_hyp_s, "us_per_call_launch": event_time_ms(fs, 100) / 100 * 1e3}
+        with hg.CallPlan() as plan_s:
+            fs()
+        row["us_per_call_plan"] = event_time_ms(plan_s, 100) / 100 * 1e3
         try:
             gs = graph_of([fs] * 10)
             row["us_per_call_graph"] = event_time_ms(gs.replay, 20) / 200 * 1e3

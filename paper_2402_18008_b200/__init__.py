@@ -123,6 +123,56 @@ def hg_built_for_sm() -> int:
     return int(lib().hg_built_for_sm())
 
 
+# ---- recorded calls: the latency path without the marshalling ---------------------------------------
+_plan = None          # the CallPlan being recorded, if any
+
+
+class CallPlan:
+    """Records the C calls the binding makes inside `with hg.CallPlan() as plan:` -- function, pointers, sizes, stream, as
+    marshalled and checked once -- and re-issues exactly those calls on `plan()`.  For loops that call the library on the
+    same buffers every iteration (the paper's Table 6 / Table 7 regime): a 1 us kernel then costs a ctypes call, not the
+    8 us of tensor checks and conversions.  The caller keeps the tensors alive and at their addresses; the stream is the
+    one that was current while recording.  (A CUDA graph of the same calls is cheaper still; this needs no capture.)"""
+
+    def __init__(self):
+        self._calls = []
+        self._keep = []
+
+    def __enter__(self):
+        global _plan
+        if _plan is not None:
+            raise RuntimeError("a CallPlan is already being recorded")
+        _plan = self
+        return self
+
+    def __exit__(self, *exc):
+        global _plan
+        _plan = None
+        return False
+
+    def __len__(self):
+        return len(self._calls)
+
+    def __call__(self):
+        for f, args, name in self._calls:
+            st = f(*args)
+            if st != HG_OK:
+                raise HgError(st, name)
+
+
+def _c(name: str):
+    """The C entry point `name`; while a CallPlan is being recorded, a wrapper that also notes the call."""
+    f = getattr(lib(), name)
+    if _plan is None:
+        return f
+    plan = _plan
+
+    def recorded(*args):
+        plan._calls.append((f, args, name))
+        return f(*args)
+    return recorded
+
+
 # ---- argument marshalling -----------------------------------------------------------------------
 def _ptr(t, dtype, device_type: str, name: str):
     if t is None:
@@ -209,7 +259,7 @@ def _solve(fn_name: str, src, dst, H, layout, norm, prec, stream):
         H = torch.empty(_h_shape(n, layout), dtype=torch.float32, device=src.device)
     elif tuple(H.shape) != _h_shape(n, layout):
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
-    fn = getattr(lib(), fn_name)
+    fn = _c(fn_name)
     ps, pd, ph = (_ptr(src, torch.float32, "cuda", "src"), _ptr(dst, torch.float32, "cuda", "dst"),
                   _ptr(H, torch.float32, "cuda", "H"))
     _same_device(src, dst, H)
@@ -240,7 +290,7 @@ def _solve_host(fn_name: str, src, dst, H, layout, norm, prec, chunk_sets):
         H = torch.empty(_h_shape(n, layout), dtype=torch.float32, pin_memory=True)
     elif tuple(H.shape) != _h_shape(n, layout):
         raise ValueError("H must have shape %s" % (_h_shape(n, layout),))
-    st = getattr(lib(), fn_name)(_ptr(src, torch.float32, "cpu", "src"), _ptr(dst, torch.float32, "cpu", "dst"),
+    st = _c(fn_name)(_ptr(src, torch.float32, "cpu", "src"), _ptr(dst, torch.float32, "cpu", "dst"),
                                  _ptr(H, torch.float32, "cpu", "H"), n, int(layout), int(norm), int(prec),
                                  int(chunk_sets))
     _check(st, fn_name)
@@ -277,7 +327,7 @@ def hg_offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w
         raise ValueError("grid must be [n,grid_h,grid_w,2]")
     _same_device(offsets, H, grid)
     with _on(offsets.device):
-        st = lib().hg_offsets_to_grid(po, x0, y0, w, h,
+        st = _c("hg_offsets_to_grid")(po, x0, y0, w, h,
                                       int(grid_w), int(grid_h), _ptr(H, torch.float32, "cuda", "H"),
                                       _ptr(grid, torch.float32, "cuda", "grid"), n, int(norm), _stream(stream))
     _check(st, "hg_offsets_to_grid")
@@ -300,7 +350,7 @@ def hg_offsets_to_warp(offsets, x0: float, y0: float, w: float, h: float, out_w:
     H = torch.empty((n, 3, 3), dtype=torch.float32, device=offsets.device) if want_H else None
     _same_device(offsets, image, warped, H)
     with _on(offsets.device):
-        st = lib().hg_offsets_to_warp(_ptr(offsets, torch.float32, "cuda", "offsets"), x0, y0, w, h, int(out_w), int(out_h),
+        st = _c("hg_offsets_to_warp")(_ptr(offsets, torch.float32, "cuda", "offsets"), x0, y0, w, h, int(out_w), int(out_h),
                                       _ptr(image, torch.float32, "cuda", "image"), C, iw, ih,
                                       _ptr(warped, torch.float32, "cuda", "warped"), _ptr(H, torch.float32, "cuda", "H"),
                                       n, int(norm), _stream(stream))
@@ -319,7 +369,7 @@ def hg_aca_rect_batched(offsets, x0: float, y0: float, w: float, h: float, H=Non
     po, ph = _ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(H, torch.float32, "cuda", "H")
     _same_device(offsets, H)
     with _on(offsets.device):
-        st = lib().hg_aca_rect_batched(po, x0, y0, w, h, ph, n, int(layout), int(norm), int(prec), _stream(stream))
+        st = _c("hg_aca_rect_batched")(po, x0, y0, w, h, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, "hg_aca_rect_batched")
     return H
 
@@ -338,7 +388,7 @@ def hg_aca_rect_backward(offsets, x0: float, y0: float, w: float, h: float, grad
                   _ptr(grad_offsets, torch.float32, "cuda", "grad_offsets"))
     _same_device(offsets, grad_H, grad_offsets)
     with _on(offsets.device):
-        st = lib().hg_aca_rect_backward(po, x0, y0, w, h, pg, pr, n, _stream(stream))
+        st = _c("hg_aca_rect_backward")(po, x0, y0, w, h, pg, pr, n, _stream(stream))
     _check(st, "hg_aca_rect_backward")
     return grad_offsets
 
@@ -357,7 +407,7 @@ def hg_aca_rect_backward_soa(offsets, x0: float, y0: float, w: float, h: float, 
                   _ptr(grad_offsets, torch.float32, "cuda", "grad_offsets"))
     _same_device(offsets, grad_H, grad_offsets)
     with _on(offsets.device):
-        st = lib().hg_aca_rect_backward_soa(po, x0, y0, w, h, pg, pr, n, _stream(stream))
+        st = _c("hg_aca_rect_backward_soa")(po, x0, y0, w, h, pg, pr, n, _stream(stream))
     _check(st, "hg_aca_rect_backward_soa")
     return grad_offsets
 
@@ -386,7 +436,7 @@ def hg_affine_batched(src3, dst3, H=None, layout: int = SOA, norm: int = NORM_NO
                   _ptr(H, torch.float32, "cuda", "H"))
     _same_device(src3, dst3, H)
     with _on(src3.device):
-        st = lib().hg_affine_batched(ps, pd, ph, n, int(layout), int(norm), int(prec), _stream(stream))
+        st = _c("hg_affine_batched")(ps, pd, ph, n, int(layout), int(norm), int(prec), _stream(stream))
     _check(st, "hg_affine_batched")
     return H
 
@@ -402,7 +452,7 @@ def hg_sk_batched(P3, Q3, dst, H=None, layout: int = SOA, norm: int = NORM_NONE,
     pd, ph = _ptr(dst, torch.float32, "cuda", "dst"), _ptr(H, torch.float32, "cuda", "H")
     _same_device(dst, H)
     with _on(dst.device):
-        st = lib().hg_sk_batched(float(P3[0]), float(P3[1]), float(Q3[0]), float(Q3[1]), pd, ph, n, int(layout),
+        st = _c("hg_sk_batched")(float(P3[0]), float(P3[1]), float(Q3[0]), float(Q3[1]), pd, ph, n, int(layout),
                                  int(norm), int(prec), _stream(stream))
     _check(st, "hg_sk_batched")
     return H
@@ -420,7 +470,7 @@ def _solve_f64(fn_name: str, src, dst, H, layout, norm, stream):
                   _ptr(H, torch.float64, "cuda", "H"))
     _same_device(src, dst, H)
     with _on(src.device):
-        st = getattr(lib(), fn_name)(ps, pd, ph, n, int(layout), int(norm), _stream(stream))
+        st = _c(fn_name)(ps, pd, ph, n, int(layout), int(norm), _stream(stream))
     _check(st, fn_name)
     return H
 
@@ -475,6 +525,8 @@ def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, co
         best_count = torch.empty((1,), dtype=torch.int32, device=dev)
     _same_device(src_xy, dst_xy, hyp_idx, counts, workspace, best_H, best_index, best_count)
     opt = _ransac_options(reject_degenerate, min_area_px2, decide_all_f64)
+    if _plan is not None and opt is not None:
+        _plan._keep.append(opt)                  # the recorded call holds a pointer into it
     head = (_ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
             _ptr(hyp_idx, torch.int32, "cuda", "hyp_idx"), n_hyp, float(threshold_px))
     tail = (_ptr(counts, torch.int32, "cuda", "counts"), _ptr(best_H, torch.float32, "cuda", "best_H"),
@@ -482,9 +534,9 @@ def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, co
             _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()), _stream(stream))
     with _on(dev):
         if opt is None:
-            st = lib().hg_ransac_hypothesize_score(*head, *tail)
+            st = _c("hg_ransac_hypothesize_score")(*head, *tail)
         else:
-            st = lib().hg_ransac_hypothesize_score_ex(*head, ctypes.cast(ctypes.pointer(opt), _vp), *tail)
+            st = _c("hg_ransac_hypothesize_score_ex")(*head, ctypes.cast(ctypes.pointer(opt), _vp), *tail)
     _check(st, "hg_ransac_hypothesize_score")
     return {"counts": counts, "best_H": best_H, "best_index": best_index, "best_count": best_count,
             "workspace": workspace}
@@ -513,6 +565,8 @@ def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, 
     n_eval = torch.empty((1,), dtype=torch.int64, device=dev)
     _same_device(src_xy, dst_xy, workspace)
     opt = _ransac_options(reject_degenerate, min_area_px2, decide_all_f64)
+    if _plan is not None:
+        _plan._keep.extend([opt, counts, idx, best_H, best_index, best_count, n_eval, workspace])
     head = (_ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
             int(seed) & 0xFFFFFFFFFFFFFFFF, int(max_hyp), int(round_hyp), float(threshold_px), float(confidence))
     tail = (_ptr(counts, torch.int32, "cuda", "counts"), _ptr(idx, torch.int32, "cuda", "hyp_idx_out"),
@@ -521,9 +575,9 @@ def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, 
             _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()), _stream(stream))
     with _on(dev):
         if opt is None:
-            st = lib().hg_ransac_adaptive(*head, *tail)
+            st = _c("hg_ransac_adaptive")(*head, *tail)
         else:
-            st = lib().hg_ransac_adaptive_ex(*head, ctypes.cast(ctypes.pointer(opt), _vp), *tail)
+            st = _c("hg_ransac_adaptive_ex")(*head, ctypes.cast(ctypes.pointer(opt), _vp), *tail)
     _check(st, "hg_ransac_adaptive")
     return {"counts": counts, "hyp_idx": idx, "best_H": best_H, "best_index": best_index, "best_count": best_count,
             "n_evaluated": n_eval, "workspace": workspace}
@@ -546,7 +600,7 @@ def hg_ransac_hypothesize_score_host(src_xy, dst_xy, hyp_idx, threshold_px: floa
     best_H = torch.empty((3, 3), dtype=torch.float32)
     best_index = torch.empty((1,), dtype=torch.int64)
     best_count = torch.empty((1,), dtype=torch.int32)
-    st = lib().hg_ransac_hypothesize_score_host(
+    st = _c("hg_ransac_hypothesize_score_host")(
         _ptr(src_xy, torch.float32, "cpu", "src_xy"), _ptr(dst_xy, torch.float32, "cpu", "dst_xy"), n_pts,
         _ptr(hyp_idx, torch.int32, "cpu", "hyp_idx"), n_hyp, float(threshold_px),
         _ptr(counts, torch.int32, "cpu", "counts"), _ptr(best_H, torch.float32, "cpu", "best_H"),

@@ -334,3 +334,33 @@ def test_combine_best_on_cuda_tensors_over_nccl():
         assert torch.equal(H, out["best_H"])
     finally:
         dist.destroy_process_group()
+
+
+def test_call_plan_replays_the_recorded_calls():
+    """hg.CallPlan: the C calls recorded once (pointers, sizes, stream) and re-issued without the marshalling -- same results
+    as fresh calls after the inputs were changed in place."""
+    off = W.offsets_workload(1024, seed=3).to(DEV)
+    H = torch.empty((1024, 3, 3), dtype=torch.float32, device=DEV)
+    wl = W.ransac_workload(n_pts=1000, n_hyp=1024, seed=4)
+    s, d, idx = (wl[k].to(DEV) for k in ("src_xy", "dst_xy", "hyp_idx"))
+    with hg.CallPlan() as plan:
+        hg.hg_offsets_to_grid(off, 0.0, 0.0, 127.0, 127.0, 128, 128, H=H, want_grid=False, norm=hg.NORM_FROBENIUS)
+        out = hg.hg_ransac_hypothesize_score(s, d, idx, 3.0)
+        chk = hg.hg_ransac_hypothesize_score(s, d, idx, 3.0, reject_degenerate=True, min_area_px2=25.0)
+    assert len(plan) == 3
+    off2 = W.offsets_workload(1024, seed=5).to(DEV)
+    wl2 = W.ransac_workload(n_pts=1000, n_hyp=1024, seed=6)
+    off.copy_(off2); s.copy_(wl2["src_xy"]); d.copy_(wl2["dst_xy"]); idx.copy_(wl2["hyp_idx"])
+    plan()
+    plan()
+    H_ref, _ = hg.hg_offsets_to_grid(off2, 0.0, 0.0, 127.0, 127.0, 128, 128, want_grid=False, norm=hg.NORM_FROBENIUS)
+    assert torch.equal(H, H_ref)
+    ref = hg.hg_ransac_hypothesize_score(s, d, idx, 3.0)
+    ref_chk = hg.hg_ransac_hypothesize_score(s, d, idx, 3.0, reject_degenerate=True, min_area_px2=25.0)
+    for a, b in ((out, ref), (chk, ref_chk)):
+        assert torch.equal(a["counts"], b["counts"]) and torch.equal(a["best_H"], b["best_H"])
+        assert a["best_index"].item() == b["best_index"].item()
+    with pytest.raises(RuntimeError):
+        with hg.CallPlan():
+            with hg.CallPlan():
+                pass

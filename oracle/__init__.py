@@ -184,6 +184,19 @@ def offsets_to_grid(offsets, x0: float, y0: float, w: float, h: float, grid_w: i
     return H, grid
 
 
+def offsets_to_grid_backward(offsets, x0: float, y0: float, w: float, h: float, grad_grid) -> np.ndarray:
+    """dL/d offsets float64 [n,4,2] of the grid of offsets_to_grid given dL/d grid [n,grid_h,grid_w,2] (forward-mode dual
+    numbers through the general ACA solve and the projection of every lattice point)."""
+    o = _f32(offsets, (4, 2))
+    n = o.shape[0]
+    g = np.ascontiguousarray(np.asarray(grad_grid, dtype=np.float64))
+    assert g.ndim == 4 and g.shape[0] == n and g.shape[3] == 2
+    go = np.empty((n, 4, 2), dtype=np.float64)
+    lib().hgo_offsets_to_grid_backward(_p(o), ctypes.c_float(x0), ctypes.c_float(y0), ctypes.c_float(w), ctypes.c_float(h),
+                                       ctypes.c_int32(g.shape[2]), ctypes.c_int32(g.shape[1]), _p(g), _p(go), ctypes.c_int64(n))
+    return go
+
+
 def offsets_to_warp(offsets, x0: float, y0: float, w: float, h: float, out_w: int, out_h: int, image) -> np.ndarray:
     """image float32 [n,C,img_h,img_w] sampled bilinearly (zero padding, pixel units) at the grid of H: float64 [n,C,out_h,out_w]."""
     o = _f32(offsets, (4, 2))

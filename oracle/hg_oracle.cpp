@@ -226,6 +226,45 @@ void hgo_offsets_to_grid(const float* offsets, float x0, float y0, float w, floa
     }
 }
 
+// Backward pass of hgo_offsets_to_grid ("offsets -> H (-> grid)"; "naturally differential"):
+// given grad_grid = dL/d grid (double [n][grid_h][grid_w][2]) returns
+//   grad_off[b][k] = sum over pixels (j,i) and coordinates c of grad_grid[b][j][i][c] * d grid[b][j][i][c] / d offsets[b][k]
+// (double [n][8]).  The derivative is taken by the plain chain rule in forward mode: the eight offsets are dual-number
+// variables, the forward pass is the one of hgo_offsets_to_grid line by line (general ACA on the corners, then the
+// projection of every lattice point), and every pixel contributes its two dual parts.
+void hgo_offsets_to_grid_backward(const float* offsets, float x0, float y0, float w, float h,
+                                  int32_t grid_w, int32_t grid_h, const double* grad_grid, double* grad_off, int64_t n)
+{
+    using D = hgo::Dual<8>;
+    const double X0 = x0, Y0 = y0, Wd = w, Hd = h;
+    const double sc[8] = { X0, Y0, X0 + Wd, Y0, X0 + Wd, Y0 + Hd, X0, Y0 + Hd };
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t b = 0; b < n; ++b) {
+        D s[8], d[8], H[9];
+        for (int k = 0; k < 8; ++k) {
+            s[k] = D(sc[k]);
+            d[k] = D(sc[k]) + D::variable(static_cast<double>(offsets[8 * b + k]), k);
+        }
+        hgo::aca<D>(s, d, H);
+        double go[8] = { 0, 0, 0, 0, 0, 0, 0, 0 };
+        const double* g = grad_grid + static_cast<int64_t>(2) * grid_w * grid_h * b;
+        for (int32_t j = 0; j < grid_h; ++j) {
+            const double y = (grid_h > 1) ? Y0 + j * Hd / (grid_h - 1) : Y0;
+            for (int32_t i = 0; i < grid_w; ++i) {
+                const double x = (grid_w > 1) ? X0 + i * Wd / (grid_w - 1) : X0;
+                const D X = H[0] * D(x) + H[1] * D(y) + H[2];
+                const D Y = H[3] * D(x) + H[4] * D(y) + H[5];
+                const D W = H[6] * D(x) + H[7] * D(y) + H[8];
+                const D u = X / W, v = Y / W;
+                const double gu = g[2 * (static_cast<int64_t>(j) * grid_w + i) + 0];
+                const double gv = g[2 * (static_cast<int64_t>(j) * grid_w + i) + 1];
+                for (int k = 0; k < 8; ++k) go[k] += gu * u.g[k] + gv * v.g[k];
+            }
+        }
+        for (int k = 0; k < 8; ++k) grad_off[8 * b + k] = go[k];
+    }
+}
+
 // Offsets -> H -> warped image ("warp image with H"; reading R17):
 //   warped[b][c][j][i] = bilinear(image[b][c], pi(H_b * (x_i, y_j, 1)))
 // with the lattice (x_i, y_j) of hgo_offsets_to_grid.  The image is sampled in pixel units (pixel (col u,

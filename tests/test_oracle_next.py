@@ -84,6 +84,75 @@ def _project(H, pts):
     return q[..., :2] / q[..., 2:3]
 
 
+# ---- 8(f) row 2, second half: backward through the grid (offsets -> H -> grid) ------------------------------------------
+def _grid_case(n=6, gw=9, gh=7, rect=(3.0, -2.0, 40.0, 24.0), seed=5):
+    rng = np.random.default_rng(seed)
+    off = rng.uniform(-6.0, 6.0, size=(n, 4, 2)).astype(np.float32)
+    off = (np.round(off * 64.0) / 64.0).astype(np.float32)            # multiples of 2^-6: +-2^-6 steps stay exact in fp32
+    g = rng.standard_normal((n, gh, gw, 2))
+    return off, g, rect
+
+
+def test_grid_backward_matches_central_differences_of_the_grid():
+    """dL/d offsets with L = sum(g * grid): central differences of the oracle's own fp64 grid forward."""
+    off, g, rect = _grid_case()
+    go = oracle.offsets_to_grid_backward(off, *rect, g)
+    hstep = 2.0 ** -6
+    fd = np.zeros_like(go)
+    for k in range(4):
+        for c in range(2):
+            op, om = off.copy(), off.copy()
+            op[:, k, c] += hstep; om[:, k, c] -= hstep
+            _, gp = oracle.offsets_to_grid(op, *rect, g.shape[2], g.shape[1])
+            _, gm = oracle.offsets_to_grid(om, *rect, g.shape[2], g.shape[1])
+            fd[:, k, c] = ((gp - gm) * g).sum(axis=(1, 2, 3)) / (2 * hstep)
+    scale = np.abs(g).sum(axis=(1, 2, 3))[:, None, None]
+    assert np.abs(go - fd).max() <= 1e-5 * scale.max()                # O(h^2) truncation of a smooth map
+    assert np.abs(go).max() > 0.1
+
+
+def test_grid_backward_translation_and_corner_identities():
+    """Two identities that need no differentiation.  (i) Moving all four target corners by delta moves every grid point
+    by delta, so sum_k dL/d off_k = sum over pixels of g.  (ii) The grid at a corner pixel IS that corner + its offset, so a
+    gradient that lives on one corner pixel comes back unchanged on that corner's offset and is zero on the others."""
+    off, g, rect = _grid_case(n=5)
+    go = oracle.offsets_to_grid_backward(off, *rect, g)
+    assert np.abs(go.sum(axis=1) - g.sum(axis=(1, 2))).max() <= 1e-9 * np.abs(g).sum(axis=(1, 2, 3)).max()
+    gh, gw = g.shape[1], g.shape[2]
+    corner_pix = [(0, 0), (0, gw - 1), (gh - 1, gw - 1), (gh - 1, 0)]          # TL, TR, BR, BL as (row, col)
+    for k, (j, i) in enumerate(corner_pix):
+        g1 = np.zeros_like(g)
+        g1[:, j, i, :] = g[:, j, i, :]
+        go1 = oracle.offsets_to_grid_backward(off, *rect, g1)
+        want = np.zeros_like(go1)
+        want[:, k, :] = g[:, j, i, :]
+        assert np.abs(go1 - want).max() <= 1e-9 * np.abs(g).max()
+
+
+def test_grid_backward_equals_pixel_jacobian_through_the_h_backward():
+    """The same gradient by another route: dL/dG summed pixel by pixel from the projection's own partials (quotient rule,
+    written out here with numpy on the oracle's H), then pulled back through the offsets -> G backward of Algorithm 1
+    (hgo_aca_rect_backward, itself pinned by the implicit-function theorem above)."""
+    off, g, rect = _grid_case(n=7, gw=8, gh=5, seed=9)
+    x0, y0, w, h = rect
+    gh, gw = g.shape[1], g.shape[2]
+    H, _ = oracle.offsets_to_grid(off, *rect, gw, gh, want_grid=False)
+    G = H / H[:, 2:3, 2:3]
+    xs = x0 + np.arange(gw) * w / (gw - 1)
+    ys = y0 + np.arange(gh) * h / (gh - 1)
+    P = np.stack(np.broadcast_arrays(xs[None, :], ys[:, None], np.ones((gh, gw))), axis=-1)      # [gh, gw, 3]
+    XYW = np.einsum("nrc,jic->njir", G, P)
+    Wv = XYW[..., 2]
+    u, v = XYW[..., 0] / Wv, XYW[..., 1] / Wv
+    a, b = g[..., 0] / Wv, g[..., 1] / Wv
+    c = -(a * u + b * v)
+    dG = np.stack([np.einsum("nji,jic->nc", a, P), np.einsum("nji,jic->nc", b, P), np.einsum("nji,jic->nc", c, P)], axis=1)
+    via_h = oracle.aca_rect_backward(off, *rect, dG)
+    go = oracle.offsets_to_grid_backward(off, *rect, g)
+    assert np.abs(go - via_h).max() <= 1e-9 * np.abs(g).sum(axis=(1, 2, 3)).max()
+
+
+
 def test_affine_defining_property_textbook_solution_and_op_count():
     s, d = W.general_sets(4096, seed=W.SEED_BASE + 31)
     s3, d3 = s.numpy()[:, :3], d.numpy()[:, :3]

@@ -470,6 +470,12 @@ def run_next_rows(hg, W, dev, peak, peak_src):
     out3 = torch.empty_like(img3)
     leg("warp_c5_3ch", lambda: hg.hg_offsets_to_warp(off5[:k3], 0.0, 0.0, 127.0, 127.0, 128, 128, img3, warped=out3), 8, k3 * 3 * 128 * 128,
         unit="pixels x channels", kernel="hg::offsets_to_warp_plane_kernel (one CTA per item and channel)")
+    del img3, out3
+    # backward through the grid on C5's shape: 8192 x 128 x 128 x 2 upstream gradient (1.07 GB, larger than L2) -> 8192 x 8
+    gg = torch.randn((k, 128, 128, 2), device=dev)
+    go5 = torch.empty((k, 4, 2), dtype=torch.float32, device=dev)
+    leg("grid_backward_c5", lambda: hg.hg_offsets_to_grid_backward(off5, 0.0, 0.0, 127.0, 127.0, gg, grad_offsets=go5),
+        128 * 128 * 8 + 64, k, unit="items (128 x 128 x 2 gradient each)", kernel="hg::grid_backward_kernel<2>")
     return ex
 
 

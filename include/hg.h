@@ -189,6 +189,25 @@ HG_API int hg_aca_rect_backward(const float* offsets, float x0, float y0, float 
 HG_API int hg_aca_rect_backward_soa(const float* offsets, float x0, float y0, float w, float h,
                          const float* grad_H, float* grad_offsets, int64_t n, void* cuda_stream);
 
+/* hg_offsets_to_grid_backward -- backward pass of hg_offsets_to_grid ("offsets -> H (-> grid)"; the
+ * training use of the fused module): given grad_grid = dL/d grid, writes
+ *   grad_offsets[b][k] = sum over pixels (j,i), c in {x,y} of grad_grid[b][j][i][c] * d grid[b][j][i][c] / d offsets[b][k],
+ * grid[b][j][i] = pi(H_b (x_i, y_j, 1)) on the lattice of hg_offsets_to_grid (reading R10).  One kernel: H is re-derived from
+ * the offsets (Algorithm 1, fp64), the item's gradient is streamed once (fp32 per-pixel partials of the projection, fp64
+ * reduction), and the result goes through the reverse mode of hg_aca_rect_backward.
+ *   offsets      : float[n][4][2], corner order TL,TR,BR,BL                         (read,  32 B per item)
+ *   x0,y0,w,h, grid_w, grid_h : as hg_offsets_to_grid (w != 0, h != 0, grid_w >= 1, grid_h >= 1)
+ *   grad_grid    : float[n][grid_h][grid_w][2]                                      (read,  8 B per pixel)
+ *   grad_offsets : float[n][4][2]                                                   (write, 32 B per item)
+ *   grad_G       : nullable, float[n][3][3]: dL/dG for G = H/h33 (what hg_aca_rect_backward takes; its (3,3) entry is
+ *                  the formal partial and is not used)                              (write, 36 B per item)
+ * An item whose H sends a lattice point to infinity (W = 0) gets non-finite gradients.
+ * Errors: HG_ERR_INVALID_ARG (NULL with n > 0, n < 0, sizes < 1, w == 0 or h == 0), HG_ERR_ALIGNMENT (offsets, grad_grid,
+ * grad_offsets not 16-byte aligned, grad_G not 4-byte aligned), HG_ERR_CUDA.                                           */
+HG_API int hg_offsets_to_grid_backward(const float* offsets, float x0, float y0, float w, float h,
+                         int32_t grid_w, int32_t grid_h, const float* grad_grid, float* grad_offsets,
+                         float* grad_G, int64_t n, void* cuda_stream);
+
 /* --------------------------------------------------------------------------------------------
  * hg_affine_batched -- 2D affine transformation from THREE correspondences by the ACA route
  * (Sec. 5.2, Eq. 41 first row): H_A = H_A2^-1 * H_A1, the core transformation being the

@@ -37,7 +37,7 @@ RANSAC_REJECT_DEGENERATE, RANSAC_DECIDE_ALL_F64 = 1, 2
 # every symbol include/hg.h declares
 EXPORTS = [
     "hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
-    "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_aca_rect_backward_soa", "hg_affine_batched",
+    "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_aca_rect_backward_soa", "hg_offsets_to_grid_backward", "hg_affine_batched",
     "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
     "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive", "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex",
     "hg_status_string", "hg_version", "hg_built_for_sm",
@@ -81,6 +81,7 @@ def lib() -> ctypes.CDLL:
         L.hg_aca_rect_batched.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _c_i64, _c_int, _c_int, _c_int, _vp]
         L.hg_aca_rect_backward.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _vp, _c_i64, _vp]
         L.hg_aca_rect_backward_soa.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _vp, _vp, _c_i64, _vp]
+        L.hg_offsets_to_grid_backward.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _c_i32, _c_i32, _vp, _vp, _vp, _c_i64, _vp]
         L.hg_offsets_to_warp.argtypes = [_vp, _c_f32, _c_f32, _c_f32, _c_f32, _c_i32, _c_i32, _vp, _c_i32, _c_i32, _c_i32,
                                          _vp, _vp, _c_i64, _c_int, _vp]
         L.hg_affine_batched.argtypes = solve_args
@@ -103,7 +104,7 @@ def lib() -> ctypes.CDLL:
         L.hg_status_string.restype = ctypes.c_char_p
         for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
                      "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
-                     "hg_aca_rect_backward_soa", "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
+                     "hg_aca_rect_backward_soa", "hg_offsets_to_grid_backward", "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
                      "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
                      "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex", "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
@@ -420,6 +421,30 @@ def _n_generic(t: torch.Tensor, layout: int, scalars: int, what: str) -> int:
     if t.dim() != 3 or tuple(t.shape[1:]) != (scalars // 2, 2):
         raise ValueError("AoS %s are [n, %d, 2]" % (what, scalars // 2))
     return int(t.shape[0])
+
+
+def hg_offsets_to_grid_backward(offsets, x0: float, y0: float, w: float, h: float, grad_grid, grad_offsets=None,
+                                want_grad_G: bool = False, stream=None):
+    """Backward of hg_offsets_to_grid: offsets float32 [n,4,2], grad_grid float32 [n,grid_h,grid_w,2] (GPU) ->
+    grad_offsets float32 [n,4,2] (and, if want_grad_G, dL/dG [n,3,3] for G = H/h33 as a second return value)."""
+    n = int(offsets.shape[0])
+    if tuple(offsets.shape) != (n, 4, 2):
+        raise ValueError("offsets are float32 [n, 4, 2]")
+    if grad_grid.dim() != 4 or int(grad_grid.shape[0]) != n or int(grad_grid.shape[3]) != 2:
+        raise ValueError("grad_grid is float32 [n, grid_h, grid_w, 2]")
+    gh, gw = int(grad_grid.shape[1]), int(grad_grid.shape[2])
+    if grad_offsets is None:
+        grad_offsets = torch.empty((n, 4, 2), dtype=torch.float32, device=offsets.device)
+    elif tuple(grad_offsets.shape) != (n, 4, 2):
+        raise ValueError("grad_offsets must have shape [n, 4, 2]")
+    gG = torch.empty((n, 3, 3), dtype=torch.float32, device=offsets.device) if want_grad_G else None
+    po, pg, pr, pG = (_ptr(offsets, torch.float32, "cuda", "offsets"), _ptr(grad_grid, torch.float32, "cuda", "grad_grid"),
+                      _ptr(grad_offsets, torch.float32, "cuda", "grad_offsets"), _ptr(gG, torch.float32, "cuda", "grad_G"))
+    _same_device(offsets, grad_grid, grad_offsets, gG)
+    with _on(offsets.device):
+        st = _c("hg_offsets_to_grid_backward")(po, x0, y0, w, h, gw, gh, pg, pr, pG, n, _stream(stream))
+    _check(st, "hg_offsets_to_grid_backward")
+    return (grad_offsets, gG) if want_grad_G else grad_offsets
 
 
 def hg_affine_batched(src3, dst3, H=None, layout: int = SOA, norm: int = NORM_NONE, prec: int = PREC_F64,

@@ -298,6 +298,185 @@ static int rect_dispatch(const float* offsets, const RectSrc& rs, float* H, int6
     return launch_status();
 }
 
+// ------------------------------------------------------------------------------------------
+// Backward through the grid (second half): dL/d offsets of
+//   grid[b][j][i] = pi(G_b (x_i, y_j, 1)),  G = H / h33,  H from the offsets (Algorithm 1)
+// given dL/d grid.  One CTA per item, the shape of the forward kernel run in reverse: warp 0 solves H in fp64 and folds
+// the lattice into it (so the sweep uses integer pixel indices), every thread streams its share of the item's gradient
+// (8 B per pixel, 128-bit loads, four in flight) and accumulates, in fp32, the nine sums
+//   S_r = sum over pixels of coef_r * (i, j, 1),  coef = (g_u / W,  g_v / W,  -(g_u u + g_v v) / W)
+// (the projection's own partials, quotient rule); the CTA reduces them in fp64 and one thread unfolds the lattice
+// (dL/dG_r = L S_r) and leaves dL/dG -- its eight used entries in the item's grad_offsets record, all nine in grad_G
+// when that is asked for.  A second, thread-per-item kernel then runs the hand-written reverse mode of Algorithm 1 above
+// in place.  (Done at the end of the streaming kernel by one thread, those ~130 dependent fp64 operations held the CTA's
+// slot for 2 of its 11 microseconds and cost 80 registers: 0.77 of the copy rate; split: see DESIGN.md.)
+// Read-bound: 8 B per pixel in, 32 B per item out.
+// ------------------------------------------------------------------------------------------
+constexpr int kGridBwdDepth = 3;             // batches of four units in flight per thread (asynchronous copies)
+__device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+// One pixel.  Packed fp32 throughout: rows 1 and 2 of L as the halves of one register pair, so that (X, Y), (u, v), the
+// coefficients (g_u, g_v) / W and their three accumulators are FFMA2 / FMUL2 / FADD2 -- 14 issued instructions per pixel
+// instead of 25 (the kernel was issue-bound before: 0.86 of the copy rate).
+//   acc[0] = sum (a, b) i,  acc[1] = sum (a, b) j,  acc[2] = sum (a, b),  acc[3] = sum c' (i, j),  c0 = sum c',   c' = a u + b v
+__device__ __forceinline__ void grid_bwd_pixel(const float2 l01, const float2 l02, const float2 l03, float l6, float l7, float l8,
+                                               float fi, float fj, float2 g, float2 acc[4], float& c0)
+{
+    const float2 I = make_float2(fi, fi), J = make_float2(fj, fj);
+    const float2 XY = __ffma2_rn(l01, I, __ffma2_rn(l02, J, l03));
+    const float W = fmaf(l6, fi, fmaf(l7, fj, l8));
+    const float q = rcp_approx(W);
+    const float2 Q = make_float2(q, q);
+    const float2 uv = __fmul2_rn(XY, Q), ab = __fmul2_rn(g, Q);
+    const float2 p = __fmul2_rn(ab, uv);
+    const float c = p.x + p.y;
+    acc[0] = __ffma2_rn(ab, I, acc[0]);
+    acc[1] = __ffma2_rn(ab, J, acc[1]);
+    acc[2] = __fadd2_rn(acc[2], ab);
+    acc[3] = __ffma2_rn(make_float2(c, c), make_float2(fi, fj), acc[3]);
+    c0 += c;
+}
+
+template <int PIX>   // 2: grid_w even, one 128-bit load covers two pixels of a row; 1: 64-bit load per pixel
+__global__ void __launch_bounds__(kRectBlock)
+grid_backward_kernel(const float* __restrict__ offsets, RectSrc rs, int grid_w, int grid_h, double step_x, double step_y,
+                     const float* __restrict__ grad_grid, float* __restrict__ grad_offsets, float* __restrict__ grad_G)
+{
+    __shared__ float lh[9];
+    __shared__ double red[kRectBlock / 32][9];
+    const int64_t b = blockIdx.x;
+    const int per_row = grid_w / PIX;
+    const int total = per_row * grid_h;
+    const float* g_item = grad_grid + static_cast<int64_t>(2) * grid_w * grid_h * b;
+    const int d_row = kRectBlock / per_row, d_col = kRectBlock - d_row * per_row;
+    int row = threadIdx.x / per_row, col = threadIdx.x - row * per_row;
+    constexpr int kUnitBytes = 8 * PIX;
+    constexpr int kDepth = kGridBwdDepth;
+    extern __shared__ __align__(16) unsigned char stage_raw[];
+    unsigned char (*stage)[4][kRectBlock][kUnitBytes] = reinterpret_cast<unsigned char (*)[4][kRectBlock][kUnitBytes]>(stage_raw);
+    auto issue = [&](int batch) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int qc = min((batch * 4 + u) * kRectBlock + static_cast<int>(threadIdx.x), total - 1);   // past the end: read again, zeroed below
+            const uint32_t dst = smem_u32(&stage[batch % kDepth][u][threadIdx.x][0]);
+            const void* src = reinterpret_cast<const unsigned char*>(g_item) + static_cast<size_t>(qc) * kUnitBytes;
+            if (PIX == 2) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(src) : "memory");
+            else          asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(dst), "l"(src) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    const int n_batches = (total + 4 * kRectBlock - 1) / (4 * kRectBlock);
+    issue(0);                                    // in flight while warp 0 solves
+    if (n_batches > 1) issue(1);
+    else asm volatile("cp.async.commit_group;" ::: "memory");
+    if (threadIdx.x < 32) {
+        const float4* op = reinterpret_cast<const float4*>(offsets + 8 * b);
+        const float4 o0 = __ldg(op), o1 = __ldg(op + 1);
+        const double ov[8] = { o0.x, o0.y, o0.z, o0.w, o1.x, o1.y, o1.z, o1.w };
+        double Hd[9];
+        aca_rect_solve<double>(rs, ov, Hd);
+        const double r = K<double>::rcp(Hd[8]);
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int r3 = 0; r3 < 3; ++r3) {              // L = G * [sx 0 x0; 0 sy y0; 0 0 1]
+                const double a = Hd[3 * r3] * r, bb = Hd[3 * r3 + 1] * r, c = Hd[3 * r3 + 2] * r;
+                lh[3 * r3]     = static_cast<float>(a * step_x);
+                lh[3 * r3 + 1] = static_cast<float>(bb * step_y);
+                lh[3 * r3 + 2] = static_cast<float>(fma(a, rs.x0, fma(bb, rs.y0, c)));
+            }
+        }
+    }
+    __syncthreads();
+    const float2 l01 = make_float2(lh[0], lh[3]), l02 = make_float2(lh[1], lh[4]), l03 = make_float2(lh[2], lh[5]);
+    const float l6 = lh[6], l7 = lh[7], l8 = lh[8];
+    float2 acc[4];
+    float c0 = 0.f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) acc[k] = make_float2(0.f, 0.f);
+
+    // units of PIX pixels, row-major; this thread takes units tid, tid + 256, ...; (col, row) advance without a division.
+    // The gradient comes through per-thread asynchronous copies (LDGSTS, L1 bypassed) into the thread's own slots of shared
+    // memory, three batches of four 16-byte units in flight per thread: bytes in flight do not cost registers (with plain
+    // loads ptxas kept two of the four in flight at 54 registers and the kernel ran at 0.62 of the copy rate), and since a
+    // thread reads back only what it copied itself, no barrier is needed -- cp.async.wait_group orders it.
+    for (int k = 0; k < n_batches; ++k) {
+        if (k + 2 < n_batches) issue(k + 2);
+        else asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 2;" ::: "memory");
+        const bool full = (k + 1) * 4 * kRectBlock <= total;           // CTA-uniform: only the last batch can be ragged
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            float4 g4;
+            if (PIX == 2) g4 = *reinterpret_cast<const float4*>(&stage[k % kDepth][u][threadIdx.x][0]);
+            else { const float2 t = *reinterpret_cast<const float2*>(&stage[k % kDepth][u][threadIdx.x][0]); g4 = make_float4(t.x, t.y, 0.f, 0.f); }
+            float fj = static_cast<float>(row), fi = static_cast<float>(PIX * col);
+            if (!full && (k * 4 + u) * kRectBlock + static_cast<int>(threadIdx.x) >= total) {
+                g4 = make_float4(0.f, 0.f, 0.f, 0.f); fi = 0.f; fj = 0.f;                 // past the end: zero gradient at lattice point (0, 0)
+            }
+            grid_bwd_pixel(l01, l02, l03, l6, l7, l8, fi, fj, make_float2(g4.x, g4.y), acc, c0);
+            if (PIX == 2) grid_bwd_pixel(l01, l02, l03, l6, l7, l8, fi + 1.f, fj, make_float2(g4.z, g4.w), acc, c0);
+            col += d_col; row += d_row;
+            if (col >= per_row) { col -= per_row; ++row; }
+        }
+    }
+    // S_1 = (a i, a j, a), S_2 = (b i, b j, b), S_3 = -(c' i, c' j, c')
+    const float s[9] = { acc[0].x, acc[1].x, acc[2].x, acc[0].y, acc[1].y, acc[2].y, -acc[3].x, -acc[3].y, -c0 };
+
+    // CTA reduction: fp32 across the lanes of a warp (a 5-level tree on 32 partial sums), fp64 across warps
+    double sd[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        float t = s[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        sd[k] = static_cast<double>(t);
+    }
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int k = 0; k < 9; ++k) red[threadIdx.x >> 5][k] = sd[k];
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    double S[9], dG[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < kRectBlock / 32; ++w) t += red[w][k];
+        S[k] = t;
+    }
+#pragma unroll
+    for (int row3 = 0; row3 < 3; ++row3) {               // dL/dG_r = L S_r
+        dG[3 * row3]     = fma(step_x, S[3 * row3], rs.x0 * S[3 * row3 + 2]);
+        dG[3 * row3 + 1] = fma(step_y, S[3 * row3 + 1], rs.y0 * S[3 * row3 + 2]);
+        dG[3 * row3 + 2] = S[3 * row3 + 2];
+    }
+    float4* out = reinterpret_cast<float4*>(grad_offsets + 8 * b);       // dL/dG[0..7], finished in place by the kernel below
+    out[0] = make_float4(static_cast<float>(dG[0]), static_cast<float>(dG[1]), static_cast<float>(dG[2]), static_cast<float>(dG[3]));
+    out[1] = make_float4(static_cast<float>(dG[4]), static_cast<float>(dG[5]), static_cast<float>(dG[6]), static_cast<float>(dG[7]));
+    if (grad_G != nullptr) {
+#pragma unroll
+        for (int k = 0; k < 9; ++k) grad_G[9 * b + k] = static_cast<float>(dG[k]);
+    }
+}
+
+// grad_offsets[b] holds dL/dG[0..7] (fp32) on entry and dL/d offsets on exit: the reverse mode of Algorithm 1, thread per item.
+__global__ void __launch_bounds__(kRectBlock)
+grid_backward_finish_kernel(const float* __restrict__ offsets, RectSrc rs, float* __restrict__ grad_offsets, int64_t n)
+{
+    const int64_t b = static_cast<int64_t>(blockIdx.x) * kRectBlock + threadIdx.x;
+    if (b >= n) return;
+    const float4* op = reinterpret_cast<const float4*>(offsets + 8 * b);
+    float4* gp = reinterpret_cast<float4*>(grad_offsets + 8 * b);
+    const float4 o0 = __ldg(op), o1 = __ldg(op + 1), g0 = gp[0], g1 = gp[1];
+    const double ov[8] = { o0.x, o0.y, o0.z, o0.w, o1.x, o1.y, o1.z, o1.w };
+    const double dG[9] = { g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w, 0.0 };
+    double go[8];
+    aca_rect_backward(rs, ov, dG, go);
+    gp[0] = make_float4(static_cast<float>(go[0]), static_cast<float>(go[1]), static_cast<float>(go[2]), static_cast<float>(go[3]));
+    gp[1] = make_float4(static_cast<float>(go[4]), static_cast<float>(go[5]), static_cast<float>(go[6]), static_cast<float>(go[7]));
+}
+
 }  // namespace hg
 
 extern "C" int hg_aca_rect_batched(const float* offsets, float x0, float y0, float w, float h, float* H, int64_t n,
@@ -362,5 +541,35 @@ extern "C" int hg_aca_rect_backward(const float* offsets, float x0, float y0, fl
         return HG_ERR_CUDA;
     rect_backward_kernel<<<static_cast<unsigned>(blocks), kRectBlock, smem, static_cast<cudaStream_t>(cuda_stream)>>>(
         offsets, rs, grad_H, grad_offsets, n);
+    return launch_status();
+}
+
+extern "C" int hg_offsets_to_grid_backward(const float* offsets, float x0, float y0, float w, float h, int32_t grid_w, int32_t grid_h,
+                                           const float* grad_grid, float* grad_offsets, float* grad_G, int64_t n, void* cuda_stream)
+{
+    using namespace hg;
+    if (n < 0 || grid_w < 1 || grid_h < 1) return HG_ERR_INVALID_ARG;
+    if (static_cast<int64_t>(grid_w) * grid_h > 0x3fffffffLL) return HG_ERR_INVALID_ARG;
+    if (!(w != 0.0f) || !(h != 0.0f) || !(w == w) || !(h == h)) return HG_ERR_INVALID_ARG;
+    if (n == 0) return HG_OK;
+    if (!offsets || !grad_grid || !grad_offsets) return HG_ERR_INVALID_ARG;
+    if (!aligned16(offsets) || !aligned16(grad_grid) || !aligned16(grad_offsets) || (grad_G && !aligned4(grad_G))) return HG_ERR_ALIGNMENT;
+    if (n > 0x7fffffffLL) return HG_ERR_INVALID_ARG;
+    RectSrc rs;
+    rs.x0 = x0; rs.y0 = y0; rs.w = w; rs.h = h; rs.r = double(w) / double(h);
+    const double step_x = (grid_w > 1) ? double(w) / double(grid_w - 1) : 0.0;
+    const double step_y = (grid_h > 1) ? double(h) / double(grid_h - 1) : 0.0;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t smem = size_t(kGridBwdDepth) * 4 * kRectBlock * (grid_w % 2 == 0 ? 16 : 8);
+    if (cudaFuncSetAttribute(grid_backward_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(size_t(kGridBwdDepth) * 4 * kRectBlock * 16)) != cudaSuccess)
+        return HG_ERR_CUDA;
+    if (grid_w % 2 == 0)
+        grid_backward_kernel<2><<<static_cast<unsigned>(n), kRectBlock, smem, st>>>(offsets, rs, grid_w, grid_h, step_x, step_y, grad_grid,
+                                                                               grad_offsets, grad_G);
+    else
+        grid_backward_kernel<1><<<static_cast<unsigned>(n), kRectBlock, smem, st>>>(offsets, rs, grid_w, grid_h, step_x, step_y, grad_grid,
+                                                                               grad_offsets, grad_G);
+    if (launch_status() != HG_OK) return HG_ERR_CUDA;
+    grid_backward_finish_kernel<<<static_cast<unsigned>((n + kRectBlock - 1) / kRectBlock), kRectBlock, 0, st>>>(offsets, rs, grad_offsets, n);
     return launch_status();
 }

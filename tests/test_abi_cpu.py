@@ -112,6 +112,22 @@ def test_rect_backward_argument_validation():
     assert f(FAKE, 0.0, 0.0, 127.0, 127.0, FAKE, FAKE + 8, 4, None) == -2
 
 
+def test_grid_backward_argument_validation():
+    f = hg.lib().hg_offsets_to_grid_backward
+    ok = (FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE, None)
+    assert f(*ok, 0, None) == 0
+    assert f(*ok, -1, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 0.0, 128, 128, FAKE, FAKE, None, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 0, 128, FAKE, FAKE, None, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, -3, FAKE, FAKE, None, 4, None) == -1
+    assert f(None, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE, None, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, None, FAKE, None, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, None, None, 4, None) == -1
+    assert f(FAKE + 4, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE, None, 4, None) == -2
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE + 8, FAKE, None, 4, None) == -2
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE, FAKE + 2, 4, None) == -2
+
+
 def test_variant_argument_validation():
     L = hg.lib()
     f = L.hg_affine_batched

@@ -364,3 +364,52 @@ def test_call_plan_replays_the_recorded_calls():
         with hg.CallPlan():
             with hg.CallPlan():
                 pass
+
+
+# ---- 8(f) row 2, second half: backward through the grid --------------------------------------------------------------
+# tolerance: the per-pixel partials and the per-thread sums are fp32 -- about 12 roundings per term
+# plus a serial sum of <= 64 terms, |term| <= |g| * max|d grid / d offset| (< 2 for these quadrangles) -- the CTA
+# reduction, the lattice unfolding and the reverse mode of Algorithm 1 are fp64 (dL/dG passes through fp32 once): worst case ~1e-5 * sum|g|;
+# the sums average out -- measured 4e-9 (C5 shape) to 3e-7 (a 600 x 3 strip) -- and the tests assert 2e-6 * sum over the item of |g|.
+@pytest.mark.parametrize("n,gw,gh,rect", [(96, 128, 128, (0.0, 0.0, 127.0, 127.0)),       # C5 shape
+                                          (33, 37, 11, (5.0, -3.0, 36.0, 10.0)),            # odd width: 64-bit loads
+                                          (7, 600, 3, (0.0, 0.0, 599.0, 2.0)),              # a row wider than four blocks
+                                          (5, 1, 1, (2.0, 2.0, 8.0, 8.0)), (4, 2, 9, (0.0, 0.0, 1.0, 8.0))])
+def test_grid_backward_matches_oracle(n, gw, gh, rect):
+    g_cpu = torch.Generator().manual_seed(1000 + gw)
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 60 + gw) * (min(rect[2], rect[3]) / 127.0)
+    g = torch.randn((n, gh, gw, 2), generator=g_cpu, dtype=torch.float32)
+    go, gG = hg.hg_offsets_to_grid_backward(off.to(DEV), *rect, g.to(DEV), want_grad_G=True)
+    ref = oracle.offsets_to_grid_backward(off.numpy(), *rect, g.numpy().astype(np.float64))
+    scale = g.abs().sum(dim=(1, 2, 3)).numpy().astype(np.float64)[:, None, None]
+    err = np.abs(go.cpu().numpy().astype(np.float64) - ref)
+    assert np.isfinite(go.cpu().numpy()).all()
+    assert (err <= 2e-6 * scale).all(), float((err / scale).max())
+    # the intermediate dL/dG pulled back by the (separately tested) H backward gives the same thing
+    via = hg.hg_aca_rect_backward(off.to(DEV), *rect, gG)
+    assert (np.abs(via.cpu().numpy().astype(np.float64) - ref) <= 2e-6 * scale).all()
+    print(n, gw, gh, "max |error| / sum|g| =", float((err / scale).max()), " max |grad| =", float(np.abs(ref).max()))
+
+
+def test_grid_backward_full_config5_sampled_and_identities():
+    """C5 at BASELINE size (8192 x 128 x 128 x 2 gradient, 1.07 GB) in the launch configuration bench.py times: every
+    item checked by the translation identity (sum_k dL/d off_k = sum of g over the item, exact up to the fp32 sums), a
+    strided sample of 64 items against the oracle, and a gradient living on the four corner pixels comes back unchanged."""
+    n = 8192
+    off = W.offsets_workload(n, seed=W.SEED_BASE + 5).to(DEV)
+    g = torch.randn((n, 128, 128, 2), generator=torch.Generator(device=DEV).manual_seed(9), dtype=torch.float32, device=DEV)
+    go = hg.hg_offsets_to_grid_backward(off, 0.0, 0.0, 127.0, 127.0, g)
+    scale = g.abs().sum(dim=(1, 2, 3))
+    assert torch.isfinite(go).all()
+    assert ((go.sum(dim=1) - g.sum(dim=(1, 2))).abs().max(dim=1).values <= 1e-5 * scale).all()
+    idx = torch.arange(0, n, n // 64)
+    ref = oracle.offsets_to_grid_backward(off[idx].cpu().numpy(), 0.0, 0.0, 127.0, 127.0, g[idx].cpu().numpy().astype(np.float64))
+    err = np.abs(go[idx].cpu().numpy().astype(np.float64) - ref)
+    assert (err <= 2e-6 * scale[idx].cpu().numpy().astype(np.float64)[:, None, None]).all()
+    gc = torch.zeros_like(g)
+    corners = [(0, 0), (0, 127), (127, 127), (127, 0)]
+    for (j, i) in corners:
+        gc[:, j, i, :] = g[:, j, i, :]
+    goc = hg.hg_offsets_to_grid_backward(off, 0.0, 0.0, 127.0, 127.0, gc)
+    want = torch.stack([g[:, j, i, :] for (j, i) in corners], dim=1)
+    assert (goc - want).abs().max().item() <= 2e-5 * want.abs().max().item()

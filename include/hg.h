@@ -255,7 +255,10 @@ HG_API int hg_sks_batched_f64(const double* src, const double* dst, double* H, i
  * the correspondences whose forward transfer error ||pi(H*s) - d||_2 <= threshold_px
  * (reading R9: inclusive, W == 0 -> outlier, no degeneracy test, no local optimisation).
  * Scoring runs in fp32 with a per-hypothesis rigorous error band; every pair that falls inside
- * the band is decided in fp64 inside the same sweep, so counts equal an fp64 evaluation.
+ * the band is decided in fp64 by the same kernel, so counts equal an fp64 evaluation.
+ * Launches: a call of <= 9472 hypotheses (<= 20 480 on <= 2048 points) on <= 4096 points is one kernel behind a
+ * one-CTA zeroing kernel (7 us for 1024 x 1000); larger calls are zero + prep + score
+ * (+ best for calls of fewer than 148 x 512 hypotheses) + finalize.  Capturable in a CUDA graph; never synchronises.
  *   src_xy, dst_xy : float[n_pts][2] correspondences                  (read)
  *   hyp_idx        : int32[n_hyp][4], the 4 indices of a row distinct and in [0,n_pts)
  *                    (out-of-range indices are undefined behaviour)   (read, 16 B per hyp.)
@@ -265,10 +268,10 @@ HG_API int hg_sks_batched_f64(const double* src, const double* dst, double* H, i
  *   best_index     : nullable, int64: argmax of counts, ties -> lowest hypothesis index
  *   best_count     : nullable, int32: its count
  *   workspace      : device scratch of >= hg_ransac_workspace_bytes(n_pts, n_hyp) bytes,
- *                    16-byte aligned; contents undefined before and after the call.  (Header,
- *                    the packed table, and -- for calls too small to fill the GPU with one
- *                    hypothesis per thread, which are also split over the table -- 4 bytes per
- *                    hypothesis of partial counts.)
+ *                    16-byte aligned; contents undefined before the call (the library zeroes what it
+ *                    needs), statistics after it (below).  (Header, the packed table, and -- for calls
+ *                    too small to fill the GPU with one hypothesis per thread -- 4 bytes per hypothesis
+ *                    of partial counts, or the per-group result slots of the one-kernel path.)
  * Errors: HG_ERR_INVALID_ARG (NULL inputs, n_pts < 4, n_hyp < 0, threshold not > 0),
  * HG_ERR_ALIGNMENT, HG_ERR_WORKSPACE, HG_ERR_CUDA.
  * -------------------------------------------------------------------------------------------- */

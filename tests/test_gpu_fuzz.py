@@ -57,3 +57,30 @@ def test_random_shapes_ransac_and_warp():
         wp, _ = hg.hg_offsets_to_warp(o2.to(DEV), 1.0, 1.0, 40.0, 30.0, ow, oh, img.to(DEV))
         wr = oracle.offsets_to_warp(o2.numpy(), 1.0, 1.0, 40.0, 30.0, ow, oh, img.numpy())
         assert np.abs(wp.cpu().numpy() - wr).max() <= 2e-3, (ow, oh, iw, ih, C, m)
+
+
+def test_random_shapes_grid_backward_and_small_ransac_modes():
+    """Random grid shapes through hg_offsets_to_grid_backward (even and odd widths, single rows and columns, grids smaller
+    than one batch of the copy pipeline) and random small RANSAC calls through the one-kernel path in all three modes."""
+    rng = np.random.default_rng(777)
+    for it in range(24):
+        gw, gh, m = int(rng.integers(1, 200)), int(rng.integers(1, 90)), int(rng.integers(1, 12))
+        rect = (float(rng.uniform(-5, 5)), float(rng.uniform(-5, 5)), float(rng.uniform(20, 130)), float(rng.uniform(20, 130)))
+        off = W.offsets_workload(m, seed=500 + it, max_offset=0.2 * min(rect[2], rect[3]))
+        g = torch.randn((m, gh, gw, 2), generator=torch.Generator().manual_seed(it))
+        go = hg.hg_offsets_to_grid_backward(off.to(DEV), *rect, g.to(DEV)).cpu().numpy().astype(np.float64)
+        ref = oracle.offsets_to_grid_backward(off.numpy(), *rect, g.numpy().astype(np.float64))
+        sc = g.abs().sum(dim=(1, 2, 3)).numpy().astype(np.float64)[:, None, None]
+        assert (np.abs(go - ref) <= 2e-6 * sc).all(), (gw, gh, m, float((np.abs(go - ref) / sc).max()))
+    for it in range(12):
+        npts, nh = int(rng.integers(4, 4097)), int(rng.integers(1, 9000))
+        wl = W.ransac_workload(n_pts=npts, n_hyp=nh, seed=7000 + it)
+        s, d, idx = wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV)
+        fast = hg.hg_ransac_hypothesize_score(s, d, idx, 2.0)
+        slow = hg.hg_ransac_hypothesize_score(s, d, idx, 2.0, decide_all_f64=True)
+        assert torch.equal(fast["counts"], slow["counts"]) and torch.equal(fast["best_H"], slow["best_H"]), (npts, nh)
+        rej = oracle.sample_check(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy(), 10.0)
+        chk = hg.hg_ransac_hypothesize_score(s, d, idx, 2.0, reject_degenerate=True, min_area_px2=10.0)
+        cc = chk["counts"].cpu().numpy()
+        assert (cc[rej] == 0).all() and np.array_equal(cc[~rej], fast["counts"].cpu().numpy()[~rej]), (npts, nh)
+        assert hg.ransac_stats(chk["workspace"])["n_rejected"] == int(rej.sum())

@@ -11,7 +11,7 @@
 //                 sure inlier, a > 2 Bc a sure outlier; the rare pair in between is decided on the
 //                 spot in fp64 by the definition (reading R9) from the fp64 H kept in shared memory.
 //                 Where the table comes from ("operand paths"):
-//                   - tables of <= 4096 points scored by >= 148 CTAs: the packed table is copied into the
+//                   - tables of <= 4096 points: the packed table is copied into the
 //                     64 KB constant bank; the sweep reads it through the uniform datapath (LDCU.64 ->
 //                     uniform-register FFMA2 operands), which costs no register-file bandwidth -- the
 //                     limiter of a three-operand FFMA2 stream on this part;
@@ -1124,7 +1124,8 @@ static int part_entries_for(int n_pairs, int64_t n_hyp, int ctas_per_sm = 2)
 {
     const int64_t ctas = (n_hyp + kRBlock - 1) / kRBlock;
     if (ctas >= kSplitBelowCtas) return n_pairs;
-    int64_t parts = (ctas_per_sm * kSplitBelowCtas + ctas - 1) / ctas;       // aim at ctas_per_sm CTAs per SM
+    int64_t parts = (ctas_per_sm * kSplitBelowCtas) / ctas;                  // at most ctas_per_sm CTAs per SM: one wave, never a second,
+    if (parts < 1) parts = 1;                                                // nearly empty one (16 384 hypotheses: 9 x 32 CTAs, not 10 x 32)
     const int64_t max_parts = n_pairs / kMinPartEntries > 0 ? n_pairs / kMinPartEntries : 1;
     if (parts > max_parts) parts = max_parts;
     if (parts <= 1) return n_pairs;
@@ -1255,10 +1256,11 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
         ransac_prep_kernel<<<blocks, 256, 0, st>>>(s2, d2, n_pts, n_pairs, inv_t, table, hdr);
         if (launch_status() != HG_OK) return HG_ERR_CUDA;
     }
-    // Operand path: a table that fits the constant bank, scored by rounds that fill the machine without splitting the
-    // table, goes through the uniform datapath; the verification mode never reads the table.
+    // Operand path: a table that fits the constant bank goes through the uniform datapath -- also when the launch is split
+    // over table parts (mid-size calls: 7-10 % faster than the staged shared-memory sweep); the verification mode never
+    // reads the table.
     const int64_t first_round = round_hyp < n_hyp ? round_hyp : n_hyp;
-    const bool use_const = n_pairs <= kConstPairs && !may_split(first_round) && !(flags & HG_RANSAC_DECIDE_ALL_F64);
+    const bool use_const = n_pairs <= kConstPairs && !(flags & HG_RANSAC_DECIDE_ALL_F64);
     const size_t stash = size_t(kQueueCap) * kRBlock * sizeof(unsigned) + kStages * sizeof(uint64_t);
     const size_t smem = (use_const ? 0 : size_t(kStages) * kChunkPairs * 32) + stash;
     auto* score = use_const ? ransac_score_kernel<true> : ransac_score_kernel<false>;
@@ -1283,7 +1285,7 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     for (int64_t h0 = 0; h0 < n_hyp; h0 += round_hyp) {
         const int64_t h1 = (h0 + round_hyp < n_hyp) ? h0 + round_hyp : n_hyp;
         hs.h0 = h0; hs.h1 = h1;
-        hs.part_entries = (hs.acc && !use_const) ? part_entries_for(n_pairs, h1 - h0) : n_pairs;
+        hs.part_entries = hs.acc ? part_entries_for(n_pairs, h1 - h0) : n_pairs;
         const unsigned parts = static_cast<unsigned>((n_pairs + hs.part_entries - 1) / hs.part_entries);
         const dim3 grid(static_cast<unsigned>((h1 - h0 + kRBlock - 1) / kRBlock), parts);
         score<<<grid, kRBlock, smem, st>>>(s2, d2, n_pts, table, n_pairs, hs, inv_t, t, counts, hdr);

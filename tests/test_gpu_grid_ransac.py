@@ -117,11 +117,13 @@ def check_ransac(wl, t, out, ref):
     return diff
 
 
-# operand paths of the score kernel: fewer than 148 x 512 hypotheses -> table split over blockIdx.y, staged in shared
-# memory; more, with <= 4096 points -> constant bank / uniform datapath; more points -> shared-memory stages, no split
+# operand paths of the score kernel: tables of <= 4096 points -> constant bank / uniform datapath (launches of fewer than
+# 148 x 512 hypotheses also split the table over blockIdx.y); more points -> shared-memory stages (split likewise); small
+# calls on small tables -> the one-kernel path
 @pytest.mark.parametrize("n_pts,n_hyp,t", [(4096, 6000, 3.0), (1001, 5000, 3.0), (100, 777, 1.5),
                                            (4, 1, 3.0), (2500, 3000, 0.75), (9000, 1500, 3.0),
-                                           (1001, 80000, 3.0), (4095, 76000, 1.0), (17, 75776, 3.0), (9001, 76000, 3.0)])
+                                           (1001, 80000, 3.0), (4095, 76000, 1.0), (17, 75776, 3.0), (9001, 76000, 3.0),
+                                           (4095, 30000, 3.0), (1001, 30001, 2.0), (8191, 20000, 3.0)])   # split: constant bank / staged
 def test_ransac_counts_match_oracle(n_pts, n_hyp, t):
     wl = W.ransac_workload(n_pts=n_pts, n_hyp=n_hyp, seed=W.SEED_BASE + 4 + n_pts)
     out = hg.hg_ransac_hypothesize_score(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), wl["hyp_idx"].to(DEV), t)
@@ -174,7 +176,9 @@ def test_ransac_full_config4_every_hypothesis():
 
 @pytest.mark.parametrize("n_pts,n_hyp,t,scale", [(4096, 1 << 20, 3.0, 1.0),        # C4 in full, constant-bank path
                                                  (2001, 100000, 0.5, 1.0),          # odd table, tight threshold
-                                                 (1000, 4096, 3.0, 1.0),            # split shared-memory path
+                                                 (1000, 4096, 3.0, 1.0),            # one-kernel path
+                                                 (3001, 30000, 3.0, 1.0),           # constant bank, split over the table
+                                                 (6001, 9000, 3.0, 1.0),            # shared-memory stages, split over the table
                                                  (6001, 80000, 3.0, 1.0),           # staged shared-memory path
                                                  (1500, 90000, 3e6, 1e6)])          # coordinates x 1e6: the band scales
 def test_ransac_fp32_sweep_equals_fp64_decisions(n_pts, n_hyp, t, scale):

@@ -364,3 +364,23 @@ def test_ransac_tiny_call_pairs_exactly_at_the_threshold(n_pts, n_hyp):
     assert hg.ransac_stats(fast["workspace"])["n_pairs_f64"] >= 0.4 * n_pts * n_hyp
     ref = oracle.ransac(s.numpy(), d.numpy(), idx.numpy(), t, band_rel=1e-4)
     assert (np.abs(fast["counts"].cpu().numpy().astype(np.int64) - ref["counts"]) <= ref["band_counts"]).all()
+
+
+def test_ransac_calls_on_two_streams_share_the_constant_bank_safely():
+    """The packed table of a call lives in the one 64 KB constant bank of the device; calls on different streams are
+    ordered against each other by the library (ConstTableGuard).  Two streams issue interleaved calls on different data;
+    every result must equal the one of the same call issued alone."""
+    wls = [W.ransac_workload(n_pts=4096 - 7 * k, n_hyp=90000 + 1000 * k, seed=W.SEED_BASE + 700 + k) for k in range(4)]
+    dev_wl = [{k: v.to(DEV) for k, v in wl.items() if isinstance(v, torch.Tensor)} for wl in wls]
+    alone = [hg.hg_ransac_hypothesize_score(w["src_xy"], w["dst_xy"], w["hyp_idx"], 3.0) for w in dev_wl]
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [None] * 4
+    for rep in range(3):
+        for k in range(4):
+            with torch.cuda.stream(streams[k % 2]):
+                outs[k] = hg.hg_ransac_hypothesize_score(dev_wl[k]["src_xy"], dev_wl[k]["dst_xy"], dev_wl[k]["hyp_idx"], 3.0)
+    torch.cuda.synchronize()
+    for k in range(4):
+        assert torch.equal(outs[k]["counts"], alone[k]["counts"]), k
+        assert outs[k]["best_index"].item() == alone[k]["best_index"].item() and torch.equal(outs[k]["best_H"], alone[k]["best_H"])

@@ -371,6 +371,15 @@ def run_extras(hg, W, dev, src, dst, H, peak, peak_src, cpu=True):
             s_np, d_np, i_np = wls["src_xy"].cpu().numpy(), wls["dst_xy"].cpu().numpy(), wls["hyp_idx"].cpu().numpy()
             row["cpu_baseline"] = timed_oracle(lambda: oracle.ransac(s_np, d_np, i_np, 3.0), 1, "calls/s",
                                                "the whole call (%d hypotheses x %d correspondences), fp64 oracle" % (n_hyp_s, n_pts_s), 0.5)
+        if n_hyp_s <= 1024:           # the same call with on-device Philox sampling (adaptive entry point, one round)
+            try:
+                fa_s = lambda: hg.hg_ransac_adaptive(wls["src_xy"], wls["dst_xy"], 7, n_hyp_s, n_hyp_s, 3.0, 0.0, want_counts=False, workspace=wss)
+                fa_s(); fa_s()
+                ga = graph_of([fa_s] * 10)
+                row["us_per_call_graph_sampled_on_device"] = event_time_ms(ga.replay, 20) / 200 * 1e3
+                del ga
+            except Exception as e:
+                row["sampled_error"] = repr(e)[:200]
         small["%dx%d" % (n_hyp_s, n_pts_s)] = row
     ex["ransac_table6_scale"] = small
     ex.update(run_next_rows(hg, W, dev, peak, peak_src))

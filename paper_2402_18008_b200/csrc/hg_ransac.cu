@@ -807,7 +807,8 @@ __device__ __forceinline__ void tiny_stats(RansacHeader* __restrict__ hdr, unsig
 __global__ void __launch_bounds__(kTinyThreads)
 ransac_tiny_kernel(const float2* __restrict__ src_xy, const float2* __restrict__ dst_xy, int n_pts, int n_pairs, HypSource hs,
                    double inv_t, double t, int* __restrict__ counts, RansacHeader* __restrict__ hdr, TinySlot* __restrict__ slots,
-                   float* __restrict__ best_H, long long* __restrict__ best_index, int* __restrict__ best_count)
+                   float* __restrict__ best_H, long long* __restrict__ best_index, int* __restrict__ best_count,
+                   long long* __restrict__ n_evaluated)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4* tb = reinterpret_cast<float4*>(smem_raw);                   // n_pairs * kTinyEntry float4: the whole table
@@ -831,7 +832,10 @@ ransac_tiny_kernel(const float2* __restrict__ src_xy, const float2* __restrict__
     const long long hidx = hs.h0 + static_cast<long long>(blockIdx.x) * kTinyHyp + lane;
     const bool active = hidx < hs.h1;
     int4 id = make_int4(0, 0, 0, 0);                                    // beyond the last hypothesis: a degenerate sample
-    if (active) id = __ldg(hs.idx + hidx);
+    if (active) {                                                       // caller's indices, or sampled on the device (R19)
+        id = hypothesis_indices(hs, hidx, n_pts);
+        if (hs.idx_out && part == 0 && wid == 0) hs.idx_out[hidx] = id;
+    }
 
     // One pass over the table: every CTA packs all of it into its shared memory (the sampled correspondences are gathered
     // from there, one memory latency earlier than a dependent global gather) and takes the coordinate bounds; it sweeps only
@@ -981,6 +985,10 @@ ransac_tiny_kernel(const float2* __restrict__ src_xy, const float2* __restrict__
     tiny_stats(hdr, n64, n_band);
     ticket = __shfl_sync(0xffffffffu, ticket, wl);
     if (ticket != gridDim.x - 1) return;
+    if (lane == 0) {                                          // a single round: every hypothesis was scored (adaptive entry point)
+        hdr->n_evaluated = static_cast<unsigned long long>(hs.h1);
+        if (n_evaluated) *n_evaluated = hs.h1;
+    }
     // the last group: every group has issued its slot; the best slot of all
     const int n_groups = static_cast<int>(gridDim.x);
     if (n_groups <= 32) {                                     // one slot per lane, key and H in one round trip
@@ -1204,13 +1212,14 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     (void)workspace_bytes;
 
     const int64_t tiny_groups = (n_hyp + kTinyHyp - 1) / kTinyHyp;
-    if (!adaptive && acc_bytes && n_pts <= kFusedMaxPts && tiny_groups <= (n_pts <= kTinyWidePts ? kTinyMaxGroupsWide : kTinyMaxGroups) &&
+    // (the adaptive entry point with a single round -- round_hyp >= max_hyp -- is the same call with on-device sampling)
+    if ((!adaptive || round_hyp >= n_hyp) && acc_bytes && n_pts <= kFusedMaxPts && tiny_groups <= (n_pts <= kTinyWidePts ? kTinyMaxGroupsWide : kTinyMaxGroups) &&
         size_t(tiny_groups) * sizeof(TinySlot) <= acc_bytes) {
         // tiny call: a cluster of CTAs per 32 hypotheses, the table split over the cluster and over the warps of each
         // CTA; the accumulator area holds the candidates
         HypSource hs;
         hs.idx = reinterpret_cast<const int4*>(hyp_idx);
-        hs.idx_out = nullptr;
+        hs.idx_out = reinterpret_cast<int4*>(hyp_idx_out);
         hs.seed = seed;
         hs.flags = flags;
         hs.reject_lim2 = reject_lim2;
@@ -1238,7 +1247,7 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
         cfg.numAttrs = parts > 1 ? 2 : 1;
         TinySlot* cand = reinterpret_cast<TinySlot*>(ws + kHeaderBytes);
         if (cudaLaunchKernelEx(&cfg, ransac_tiny_kernel, s2, d2, n_pts, n_pairs, hs, inv_t, t, counts, hdr, cand, best_H,
-                               reinterpret_cast<long long*>(best_index), best_count) != cudaSuccess) {
+                               reinterpret_cast<long long*>(best_index), best_count, reinterpret_cast<long long*>(n_evaluated)) != cudaSuccess) {
             (void)cudaGetLastError();
             return HG_ERR_CUDA;
         }
@@ -1259,7 +1268,6 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     // Operand path: a table that fits the constant bank goes through the uniform datapath -- also when the launch is split
     // over table parts (mid-size calls: 7-10 % faster than the staged shared-memory sweep); the verification mode never
     // reads the table.
-    const int64_t first_round = round_hyp < n_hyp ? round_hyp : n_hyp;
     const bool use_const = n_pairs <= kConstPairs && !(flags & HG_RANSAC_DECIDE_ALL_F64);
     const size_t stash = size_t(kQueueCap) * kRBlock * sizeof(unsigned) + kStages * sizeof(uint64_t);
     const size_t smem = (use_const ? 0 : size_t(kStages) * kChunkPairs * 32) + stash;

@@ -5,6 +5,8 @@
 // so H follows from the target quadrangle alone (Eq. 44-45; Algorithm 1):
 // 47 FLOPs, and only the 8 offsets are read -- 32 B in + 36 B out = 68 B per homography instead of
 // the general solver's 100 B.  Same streaming skeleton as hg_batched.cu; fp64 registers, fp32 I/O.
+#include <type_traits>
+
 #include "hg_device.cuh"
 #include "hg_host.h"
 
@@ -349,16 +351,18 @@ grid_backward_kernel(const float* __restrict__ offsets, RectSrc rs, int grid_w, 
     const int total = per_row * grid_h;
     const float* g_item = grad_grid + static_cast<int64_t>(2) * grid_w * grid_h * b;
     const int d_row = kRectBlock / per_row, d_col = kRectBlock - d_row * per_row;
-    int row = threadIdx.x / per_row, col = threadIdx.x - row * per_row;
+    const int row0 = threadIdx.x / per_row;
+    float frow = static_cast<float>(row0), fcol = static_cast<float>(PIX * (static_cast<int>(threadIdx.x) - row0 * per_row));   // lattice indices, exact in fp32
+    const float f_drow = static_cast<float>(d_row), f_dcol = static_cast<float>(PIX * d_col), f_width = static_cast<float>(PIX * per_row);
     constexpr int kUnitBytes = 8 * PIX;
     constexpr int kDepth = kGridBwdDepth;
     extern __shared__ __align__(16) unsigned char stage_raw[];
     unsigned char (*stage)[4][kRectBlock][kUnitBytes] = reinterpret_cast<unsigned char (*)[4][kRectBlock][kUnitBytes]>(stage_raw);
-    auto issue = [&](int batch) {
+    auto issue = [&](int batch, int slot) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const int qc = min((batch * 4 + u) * kRectBlock + static_cast<int>(threadIdx.x), total - 1);   // past the end: read again, zeroed below
-            const uint32_t dst = smem_u32(&stage[batch % kDepth][u][threadIdx.x][0]);
+            const uint32_t dst = smem_u32(&stage[slot][u][threadIdx.x][0]);
             const void* src = reinterpret_cast<const unsigned char*>(g_item) + static_cast<size_t>(qc) * kUnitBytes;
             if (PIX == 2) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(src) : "memory");
             else          asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(dst), "l"(src) : "memory");
@@ -366,8 +370,8 @@ grid_backward_kernel(const float* __restrict__ offsets, RectSrc rs, int grid_w, 
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     const int n_batches = (total + 4 * kRectBlock - 1) / (4 * kRectBlock);
-    issue(0);                                    // in flight while warp 0 solves
-    if (n_batches > 1) issue(1);
+    issue(0, 0);                                 // in flight while warp 0 solves
+    if (n_batches > 1) issue(1, 1);
     else asm volatile("cp.async.commit_group;" ::: "memory");
     if (threadIdx.x < 32) {
         const float4* op = reinterpret_cast<const float4*>(offsets + 8 * b);
@@ -399,25 +403,32 @@ grid_backward_kernel(const float* __restrict__ offsets, RectSrc rs, int grid_w, 
     // memory, three batches of four 16-byte units in flight per thread: bytes in flight do not cost registers (with plain
     // loads ptxas kept two of the four in flight at 54 registers and the kernel ran at 0.62 of the copy rate), and since a
     // thread reads back only what it copied itself, no barrier is needed -- cp.async.wait_group orders it.
-    for (int k = 0; k < n_batches; ++k) {
-        if (k + 2 < n_batches) issue(k + 2);
-        else asm volatile("cp.async.commit_group;" ::: "memory");
-        asm volatile("cp.async.wait_group 2;" ::: "memory");
-        const bool full = (k + 1) * 4 * kRectBlock <= total;           // CTA-uniform: only the last batch can be ragged
+    // one batch = four units of this thread from slot `slot`; RAGGED: units past the end of the item count as a zero gradient
+    auto batch = [&](int k, int slot, auto ragged) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             float4 g4;
-            if (PIX == 2) g4 = *reinterpret_cast<const float4*>(&stage[k % kDepth][u][threadIdx.x][0]);
-            else { const float2 t = *reinterpret_cast<const float2*>(&stage[k % kDepth][u][threadIdx.x][0]); g4 = make_float4(t.x, t.y, 0.f, 0.f); }
-            float fj = static_cast<float>(row), fi = static_cast<float>(PIX * col);
-            if (!full && (k * 4 + u) * kRectBlock + static_cast<int>(threadIdx.x) >= total) {
-                g4 = make_float4(0.f, 0.f, 0.f, 0.f); fi = 0.f; fj = 0.f;                 // past the end: zero gradient at lattice point (0, 0)
+            if (PIX == 2) g4 = *reinterpret_cast<const float4*>(&stage[slot][u][threadIdx.x][0]);
+            else { const float2 t = *reinterpret_cast<const float2*>(&stage[slot][u][threadIdx.x][0]); g4 = make_float4(t.x, t.y, 0.f, 0.f); }
+            float fi = fcol, fj = frow;
+            if (decltype(ragged)::value && (k * 4 + u) * kRectBlock + static_cast<int>(threadIdx.x) >= total) {
+                g4 = make_float4(0.f, 0.f, 0.f, 0.f); fi = 0.f; fj = 0.f;                 // lattice point (0, 0): a finite W
             }
             grid_bwd_pixel(l01, l02, l03, l6, l7, l8, fi, fj, make_float2(g4.x, g4.y), acc, c0);
             if (PIX == 2) grid_bwd_pixel(l01, l02, l03, l6, l7, l8, fi + 1.f, fj, make_float2(g4.z, g4.w), acc, c0);
-            col += d_col; row += d_row;
-            if (col >= per_row) { col -= per_row; ++row; }
+            fcol += f_dcol; frow += f_drow;
+            if (fcol >= f_width) { fcol -= f_width; frow += 1.f; }
         }
+    };
+    int slot = 0;
+    for (int k = 0; k < n_batches; ++k) {
+        const int next = slot + 2 >= kDepth ? slot + 2 - kDepth : slot + 2;
+        if (k + 2 < n_batches) issue(k + 2, next);
+        else asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 2;" ::: "memory");
+        if ((k + 1) * 4 * kRectBlock <= total) batch(k, slot, std::false_type());       // CTA-uniform: only the last batch can be ragged
+        else batch(k, slot, std::true_type());
+        slot = slot + 1 == kDepth ? 0 : slot + 1;
     }
     // S_1 = (a i, a j, a), S_2 = (b i, b j, b), S_3 = -(c' i, c' j, c')
     const float s[9] = { acc[0].x, acc[1].x, acc[2].x, acc[0].y, acc[1].y, acc[2].y, -acc[3].x, -acc[3].y, -c0 };

@@ -300,9 +300,12 @@ def test_ransac_adaptive_agrees_with_explicit_indices():
     assert torch.equal(plain["best_H"], out["best_H"])
 
 
-@pytest.mark.parametrize("n_pts,max_hyp,round_hyp", [(4, 10, 1000), (1001, 700, 5000), (37, 1, 1), (2049, 3000, 2999)])
+@pytest.mark.parametrize("n_pts,max_hyp,round_hyp", [(4, 10, 1000), (1001, 700, 5000), (37, 1, 1), (2049, 3000, 2999),
+                                                     (1000, 1024, 1024), (500, 256, 1 << 20), (4096, 9472, 9472), (2000, 20480, 30000),
+                                                     (4096, 9473, 9473)])
 def test_ransac_adaptive_boundary_shapes(n_pts, max_hyp, round_hyp):
-    """round_hyp > max_hyp (one ragged round), odd tables, the smallest table: same rule as the oracle's loop."""
+    """round_hyp > max_hyp (one ragged round), odd tables, the smallest table: same rule as the oracle's loop.  A single
+    round on a small table is the one-kernel path with on-device sampling (the last case is just past its range)."""
     wl = W.ransac_workload(n_pts=n_pts, n_hyp=4, seed=W.SEED_BASE + 200 + n_pts, inlier_frac=0.6)
     out = hg.hg_ransac_adaptive(wl["src_xy"].to(DEV), wl["dst_xy"].to(DEV), 42, max_hyp, round_hyp, 3.0, 0.0, want_idx=True)
     ref = oracle.ransac_adaptive(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), 42, max_hyp, round_hyp, 3.0, 0.0)

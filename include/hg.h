@@ -202,8 +202,8 @@ HG_API int hg_aca_rect_backward_soa(const float* offsets, float x0, float y0, fl
  *   grad_G       : nullable, float[n][3][3]: dL/dG for G = H/h33 (what hg_aca_rect_backward takes; its (3,3) entry is
  *                  the formal partial and is not used)                              (write, 36 B per item)
  * An item whose H sends a lattice point to infinity (W = 0) gets non-finite gradients.
- * Errors: HG_ERR_INVALID_ARG (NULL with n > 0, n < 0, sizes < 1, w == 0 or h == 0), HG_ERR_ALIGNMENT (offsets, grad_grid,
- * grad_offsets not 16-byte aligned, grad_G not 4-byte aligned), HG_ERR_CUDA.                                           */
+ * Errors: HG_ERR_INVALID_ARG (NULL with n > 0, n < 0, sizes < 1 or > 2^24 or grid_w * grid_h >= 2^30, w == 0 or h == 0),
+ * HG_ERR_ALIGNMENT (offsets, grad_grid, grad_offsets not 16-byte aligned, grad_G not 4-byte aligned), HG_ERR_CUDA.        */
 HG_API int hg_offsets_to_grid_backward(const float* offsets, float x0, float y0, float w, float h,
                          int32_t grid_w, int32_t grid_h, const float* grad_grid, float* grad_offsets,
                          float* grad_G, int64_t n, void* cuda_stream);

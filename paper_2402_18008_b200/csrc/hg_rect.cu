@@ -560,7 +560,8 @@ extern "C" int hg_offsets_to_grid_backward(const float* offsets, float x0, float
 {
     using namespace hg;
     if (n < 0 || grid_w < 1 || grid_h < 1) return HG_ERR_INVALID_ARG;
-    if (static_cast<int64_t>(grid_w) * grid_h > 0x3fffffffLL) return HG_ERR_INVALID_ARG;
+    if (grid_w > (1 << 24) || grid_h > (1 << 24) || static_cast<int64_t>(grid_w) * grid_h > 0x3fffffffLL)
+        return HG_ERR_INVALID_ARG;                      // lattice indices are carried in fp32 (exact below 2^24)
     if (!(w != 0.0f) || !(h != 0.0f) || !(w == w) || !(h == h)) return HG_ERR_INVALID_ARG;
     if (n == 0) return HG_OK;
     if (!offsets || !grad_grid || !grad_offsets) return HG_ERR_INVALID_ARG;

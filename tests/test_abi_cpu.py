@@ -120,6 +120,8 @@ def test_grid_backward_argument_validation():
     assert f(FAKE, 0.0, 0.0, 127.0, 0.0, 128, 128, FAKE, FAKE, None, 4, None) == -1
     assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 0, 128, FAKE, FAKE, None, 4, None) == -1
     assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, -3, FAKE, FAKE, None, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, (1 << 24) + 1, 1, FAKE, FAKE, None, 4, None) == -1
+    assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 1 << 16, 1 << 15, FAKE, FAKE, None, 4, None) == -1
     assert f(None, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, FAKE, None, 4, None) == -1
     assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, None, FAKE, None, 4, None) == -1
     assert f(FAKE, 0.0, 0.0, 127.0, 127.0, 128, 128, FAKE, None, None, 4, None) == -1

@@ -200,7 +200,10 @@ def test_f64_storage_matches_oracle(method, n, layout):
     ((0.0, 0.0, 255.0, 255.0), 256, 256, 256, 256, 1, 2, 40.0),          # plane too large to stage: gather form, row bands
     ((0.0, 0.0, 99.0, 79.0), 100, 80, 130, 90, 4, 7, 10.0),              # img_w % 4 != 0: staged by plain loads; 4 channels
     ((0.0, 0.0, 199.0, 199.0), 200, 200, 200, 200, 3, 2, 30.0),          # gather form, 3 channels
-    ((0.0, 0.0, 127.0, 127.0), 128, 128, 128, 128, 3, 1, 60.0)])         # one item: (channel, band) CTAs; large offsets -> frame taps
+    ((0.0, 0.0, 127.0, 127.0), 128, 128, 128, 128, 3, 1, 60.0),          # one item: (channel, band) CTAs; large offsets -> frame taps
+    ((0.0, 0.0, 127.0, 127.0), 128, 128, 128, 128, 1, 700, 32.0),        # large batches: several waves of (item, channel) CTAs
+    ((0.0, 0.0, 63.0, 47.0), 64, 48, 72, 60, 3, 260, 14.0),
+    ((2.0, 1.0, 40.0, 30.0), 35, 27, 48, 36, 2, 301, 8.0)])
 def test_warp_matches_oracle(rect, ow, oh, iw, ih, C, n, max_off):
     off = W.offsets_workload(n, seed=W.SEED_BASE + 70 + ow, max_offset=max_off)
     img = torch.rand((n, C, ih, iw), generator=torch.Generator().manual_seed(ow), dtype=torch.float32)

@@ -384,3 +384,28 @@ def test_ransac_calls_on_two_streams_share_the_constant_bank_safely():
     for k in range(4):
         assert torch.equal(outs[k]["counts"], alone[k]["counts"]), k
         assert outs[k]["best_index"].item() == alone[k]["best_index"].item() and torch.equal(outs[k]["best_H"], alone[k]["best_H"])
+
+
+def test_ransac_tiny_call_protocol_stress():
+    """The one-kernel path synchronises through stamped slots and a ticket, with no fence between them: 3000 calls on one
+    workspace, alternating between three inputs of different shapes (so every call sees the leftovers of a different
+    one), each result checked against the one computed alone."""
+    shapes = [(1000, 1024), (500, 256), (333, 4000)]
+    wls = [W.ransac_workload(n_pts=a, n_hyp=b, seed=40 + a) for a, b in shapes]
+    dev_wl = [{k: v.to(DEV) for k, v in wl.items() if isinstance(v, torch.Tensor)} for wl in wls]
+    alone = [hg.hg_ransac_hypothesize_score(w["src_xy"], w["dst_xy"], w["hyp_idx"], 3.0) for w in dev_wl]
+    want = [(int(o["best_index"].item()), int(o["best_count"].item()), o["best_H"].clone(), int(o["counts"].sum().item())) for o in alone]
+    ws = torch.empty(max(hg.hg_ransac_workspace_bytes(a, b) for a, b in shapes), dtype=torch.uint8, device=DEV)
+    ws.fill_(0xAB)                                                    # garbage in, as the contract allows
+    outs = [dict(o) for o in alone]
+    bad = 0
+    for it in range(3000):
+        k = (it * 7 + it // 5) % 3
+        o = hg.hg_ransac_hypothesize_score(dev_wl[k]["src_xy"], dev_wl[k]["dst_xy"], dev_wl[k]["hyp_idx"], 3.0,
+                                           counts=outs[k]["counts"], workspace=ws,
+                                           best=(outs[k]["best_H"], outs[k]["best_index"], outs[k]["best_count"]))
+        if it % 10 == 9 or it > 2950:                                 # most calls run back to back without a host sync
+            bi, bc = int(o["best_index"].item()), int(o["best_count"].item())
+            ok = (bi, bc) == want[k][:2] and torch.equal(o["best_H"], want[k][2]) and int(o["counts"].sum().item()) == want[k][3]
+            bad += 0 if ok else 1
+    assert bad == 0

@@ -260,3 +260,24 @@ def test_sass_of_the_hot_loops_keeps_its_operand_paths():
     assert "MEMBAR.SC" not in tiny and "STAS" in tiny                        # no fence between the slot stores and the ticket; st.async exchange
     gb = sass("grid_backward_kernelILi2E")
     assert gb.count("LDGSTS") >= 4 and gb.count("FFMA2") >= 8                # asynchronous staging, packed fp32 partials
+
+
+def test_bench_reference_arm_prints_the_contract_line():
+    """`bench.py --impl reference` (the oracle on the host cores; needs no GPU): one JSON line with the keys the driver reads,
+    the same metric / unit / workload as the GPU arm, and nothing of the CUDA library loaded on that path."""
+    import json
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    r = subprocess.run([sys.executable, str(root / "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "1"],
+                       capture_output=True, text=True, timeout=600, cwd=str(root))
+    assert r.returncode == 0, r.stderr[-500:]
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["unit"] == "homographies/s" and line["higher_is_better"] is True
+    assert line["metric"].startswith("homographies/sec (ACA fp32, batch 2^26)") and line["n_gpus"] == 1
+    assert line["steps"] == 1 and line["warmup"] == 1 and line["value"] > 0 and line["ms_per_step"] > 0
+    assert line["config"]["workload"].startswith("C3") and line["vs_baseline"] is None and line["data"] == "synthetic"
+    cb, e2e = line["cpu_baseline"], line["e2e"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] == line["value"] and cb["sample"]
+    assert e2e == {"value": line["value"], "unit": line["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}

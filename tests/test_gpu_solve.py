@@ -204,3 +204,28 @@ def test_full_size_config3_sampled_against_oracle():
     torch.cuda.synchronize()
     Hn = W.h_soa_to_aos(Hs[:, idx].contiguous().cpu()).numpy()
     print("C3 sampled sks", check_parity(Hn, s, d, "sks"))
+
+
+def test_bench_line_carries_the_contract_keys():
+    """bench.py on a reduced batch (2^22 sets, no extras, no oracle leg): one JSON line with the contract's keys -- the roofline
+    object of the step kernel, the end-to-end leg through the host-buffer entry point with its copied bytes, the clock
+    sample, and one launch of the library's kernel per timed step."""
+    import json
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    r = subprocess.run([sys.executable, str(root / "bench.py"), "--steps", "4", "--warmup", "3", "--log2n", "22", "--no-extras", "--no-cpu"],
+                       capture_output=True, text=True, timeout=600, cwd=str(root))
+    assert r.returncode == 0, r.stderr[-800:]
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["unit"] == "homographies/s" and line["higher_is_better"] is True and line["n_gpus"] == 1 and line["steps"] == 4
+    assert line["gpu_launches"] == 4 and line["dtype"] == "f64" and line["scaling"] == "weak" and line["vs_baseline"] is None
+    rf = line["roofline"]
+    assert rf["bound"] == "hbm" and rf["unit"] == "GB/s" and rf["peak"] > 1000 and abs(rf["frac"] - rf["achieved"] / rf["peak"]) < 1e-9
+    assert rf["algorithmic_bytes_per_launch"] == 100 * (1 << 22)
+    assert abs(line["value"] - (1 << 22) / (line["ms_per_step"] * 1e-3)) <= 1e-6 * line["value"]
+    e2e = line["e2e"]
+    assert e2e["h2d_bytes_per_step"] == 64 * (1 << 22) and e2e["d2h_bytes_per_step"] == 36 * (1 << 22) and 0 < e2e["value"] < line["value"]
+    assert e2e["matches_device_result"] is True
+    assert line["clocks"]["sm_mhz"] > 0 and isinstance(line["clocks"]["reasons"], list)

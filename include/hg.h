@@ -294,7 +294,8 @@ HG_API int hg_ransac_hypothesize_score(const float* src_xy, const float* dst_xy,
  *    hypotheses scored and best count c, w = c / n_pts and the run stops iff
  *    done * log1p(-w^4) <= log1p(-confidence) (fp64), i.e. done >= log(1-confidence)/log(1-w^4);
  *    confidence <= 0 scores all max_hyp hypotheses.  No host synchronisation: every round is
- *    enqueued, rounds after the stop return immediately.
+ *    enqueued, rounds after the stop return immediately.  A single round (round_hyp >= max_hyp) on a small table takes
+ *    the one-kernel path of hg_ransac_hypothesize_score with the sampling done inside it.
  *   seed, max_hyp, round_hyp : max_hyp <= 2^31-1, round_hyp >= 1, at most 65536 rounds
  *   confidence     : < 1
  *   counts         : nullable, int32[max_hyp]; entries >= *n_evaluated are not written

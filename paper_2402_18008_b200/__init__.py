@@ -133,7 +133,8 @@ class CallPlan:
     marshalled and checked once -- and re-issues exactly those calls on `plan()`.  For loops that call the library on the
     same buffers every iteration (the paper's Table 6 / Table 7 regime): a 1 us kernel then costs a ctypes call, not the
     8 us of tensor checks and conversions.  The caller keeps the tensors alive and at their addresses; the stream is the
-    one that was current while recording.  (A CUDA graph of the same calls is cheaper still; this needs no capture.)"""
+    one that was current while recording.  One plan is recorded at a time, by one thread.  (A CUDA graph of the same calls is
+    cheaper still; this needs no capture.)"""
 
     def __init__(self):
         self._calls = []

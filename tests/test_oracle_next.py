@@ -129,6 +129,38 @@ def test_grid_backward_translation_and_corner_identities():
         assert np.abs(go1 - want).max() <= 1e-9 * np.abs(g).max()
 
 
+def test_grid_backward_equals_library_autograd_through_the_dlt_system():
+    """A pin that shares nothing with the oracle's arithmetic: the 8 x 8 DLT system of Eq. 2-3 solved by the library
+    (torch.linalg.solve, fp64), the grid projected from that H, and the gradient taken by torch.autograd."""
+    import torch
+    off, g, rect = _grid_case(n=5, gw=7, gh=6, seed=21)
+    x0, y0, w, h = rect
+    gh, gw = g.shape[1], g.shape[2]
+    corners = torch.tensor([[x0, y0], [x0 + w, y0], [x0 + w, y0 + h], [x0, y0 + h]], dtype=torch.float64)
+    o = torch.tensor(off.astype(np.float64), requires_grad=True)
+    dst = corners[None] + o                                            # [n, 4, 2]
+    n = o.shape[0]
+    x, y = corners[:, 0][None].expand(n, 4), corners[:, 1][None].expand(n, 4)
+    u, v = dst[..., 0], dst[..., 1]
+    one, zero = torch.ones_like(x), torch.zeros_like(x)
+    rows_u = torch.stack([x, y, one, zero, zero, zero, -u * x, -u * y], dim=-1)
+    rows_v = torch.stack([zero, zero, zero, x, y, one, -v * x, -v * y], dim=-1)
+    A = torch.cat([rows_u, rows_v], dim=1)                             # [n, 8, 8]
+    rhs = torch.cat([u, v], dim=1)[..., None]
+    hvec = torch.linalg.solve(A, rhs)[..., 0]
+    H = torch.cat([hvec, torch.ones((n, 1), dtype=torch.float64)], dim=1).reshape(n, 3, 3)
+    xs = x0 + torch.arange(gw, dtype=torch.float64) * w / (gw - 1)
+    ys = y0 + torch.arange(gh, dtype=torch.float64) * h / (gh - 1)
+    P = torch.stack([xs[None, :].expand(gh, gw), ys[:, None].expand(gh, gw), torch.ones((gh, gw), dtype=torch.float64)], dim=-1)
+    XYW = torch.einsum("nrc,jic->njir", H, P)
+    grid = XYW[..., :2] / XYW[..., 2:3]
+    _, grid_ref = oracle.offsets_to_grid(off, *rect, gw, gh)
+    assert np.abs(grid.detach().numpy() - grid_ref).max() <= 1e-9      # same forward map, by another solver
+    (grid * torch.tensor(g)).sum().backward()
+    go = oracle.offsets_to_grid_backward(off, *rect, g)
+    assert np.abs(go - o.grad.numpy()).max() <= 1e-8 * np.abs(g).sum(axis=(1, 2, 3)).max()
+
+
 def test_grid_backward_equals_pixel_jacobian_through_the_h_backward():
     """The same gradient by another route: dL/dG summed pixel by pixel from the projection's own partials (quotient rule,
     written out here with numpy on the oracle's H), then pulled back through the offsets -> G backward of Algorithm 1

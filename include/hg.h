@@ -49,7 +49,8 @@ typedef enum {
     HG_ERR_INVALID_ARG = -1, /* NULL pointer with n > 0, negative size, unknown enum value        */
     HG_ERR_ALIGNMENT   = -2, /* a base pointer is not 16-byte aligned                             */
     HG_ERR_CUDA        = -3, /* a CUDA runtime call or kernel launch failed                       */
-    HG_ERR_WORKSPACE   = -4  /* workspace_bytes < hg_ransac_workspace_bytes(...)                  */
+    HG_ERR_WORKSPACE   = -4, /* workspace_bytes < hg_ransac_workspace_bytes(...)                  */
+    HG_ERR_TOO_LARGE   = -5  /* a size is beyond the fixed capacity of a no-allocation entry point  */
 } hg_status_t;
 
 /* Memory layout of the point sets and of H.
@@ -353,6 +354,52 @@ HG_API int hg_ransac_hypothesize_score_host(const float* src_xy_host, const floa
                                      int32_t n_pts, const int32_t* hyp_idx_host, int64_t n_hyp,
                                      float threshold_px, int32_t* counts_host, float* best_H_host,
                                      int64_t* best_index_host, int32_t* best_count_host);
+
+/* --------------------------------------------------------------------------------------------
+ * hg_ransac_hypothesize_score_noalloc -- hg_ransac_hypothesize_score for callers that have no device
+ * memory to hand over as a workspace and no way of getting any.
+ *
+ * Who that is: code that runs where cudaMalloc / cudaFree are off limits or would break a promise --
+ * a plugin or filter called from inside somebody else's frame loop (the host application owns the
+ * memory pool and a cudaMalloc there stalls every stream of the device), a control loop with a
+ * latency budget in which an allocator call is an unbounded wait, a process whose other threads are
+ * capturing streams in the global capture mode (an allocation made meanwhile fails), and embedders
+ * whose memory is accounted up front and who must not see the library grow the footprint later.
+ * Such callers already own their inputs and outputs; the only thing the ordinary entry point asks of
+ * them beyond that is the scratch workspace, and this entry point brings its own.
+ *
+ * Same operation, same results (bit for bit: it runs the one-kernel small-call path of
+ * hg_ransac_hypothesize_score) and the same arguments minus
+ * `workspace` / `workspace_bytes`.  The scratch -- the 128-byte header and one 96-byte result slot per
+ * group of 32 hypotheses -- lives in a fixed array inside the library image:
+ *   - capacity: n_pts <= HG_RANSAC_NOALLOC_MAX_PTS (4096) and n_hyp <= HG_RANSAC_NOALLOC_MAX_HYP
+ *     (9472 = 296 groups); the array is HG_RANSAC_NOALLOC_SCRATCH_BYTES (28 672) of device memory
+ *     that every GPU which loads libhg holds from module load until the process exits, used or not.
+ *     Anything larger is refused with HG_ERR_TOO_LARGE before any work is enqueued -- take the
+ *     ordinary entry point with a workspace of your own for that.
+ *   - the call performs no cudaMalloc, no cudaFree and calls nothing that allocates (no event or stream
+ *     creation either); it enqueues the zeroing kernel and the scoring kernel on `cuda_stream` and returns.
+ *   - first call on each device: the library looks up the device address of the array (once per device,
+ *     with that device current -- make the device of the buffers current before calling, as for every
+ *     entry point) and remembers it.  Make that first call during start-up, outside any stream capture;
+ *     later calls do no such set-up.
+ *   - ONE array per device, shared by every call: each call zeroes the words it depends on (header and
+ *     its slots) on the stream before using them and leaves its own statistics and slots behind, so the
+ *     contents between calls are the last call's.  Two calls that can be on the GPU at the same time
+ *     (different streams with no ordering between them, or two host threads) zero and write the same
+ *     words: that is a race -- wrong best_* outputs, or a final step that waits for a slot the other call
+ *     wiped and never finishes.  Keep all calls of a device on one stream, or order them with events.
+ *     The statistics words (HG_RANSAC_STAT_WORDS) are not readable through this entry point.
+ * Errors: as hg_ransac_hypothesize_score (HG_ERR_INVALID_ARG, HG_ERR_ALIGNMENT, HG_ERR_CUDA), never
+ * HG_ERR_WORKSPACE; HG_ERR_TOO_LARGE as above.  n_hyp == 0 is HG_OK and does nothing.
+ * -------------------------------------------------------------------------------------------- */
+#define HG_RANSAC_NOALLOC_MAX_PTS       4096
+#define HG_RANSAC_NOALLOC_MAX_HYP       9472
+#define HG_RANSAC_NOALLOC_SCRATCH_BYTES 28672
+HG_API int hg_ransac_hypothesize_score_noalloc(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                                        const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
+                                        int32_t* counts, float* best_H, int64_t* best_index,
+                                        int32_t* best_count, void* cuda_stream);
 
 /* Human-readable name of a status code (static storage, never NULL). */
 HG_API const char* hg_status_string(int status);

@@ -23,6 +23,7 @@ __all__ = [
     "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
     "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
     "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex", "RANSAC_REJECT_DEGENERATE", "RANSAC_DECIDE_ALL_F64",
+    "hg_ransac_hypothesize_score_noalloc", "RANSAC_NOALLOC_MAX_PTS", "RANSAC_NOALLOC_MAX_HYP",
     "hg_status_string", "hg_version", "hg_built_for_sm", "EXPORTS",
 ]
 
@@ -33,6 +34,8 @@ NORM_NONE, NORM_H33, NORM_FROBENIUS = 0, 1, 2
 PREC_F64, PREC_F32 = 0, 1
 RANSAC_STAT_WORDS = 6
 RANSAC_REJECT_DEGENERATE, RANSAC_DECIDE_ALL_F64 = 1, 2
+HG_ERR_TOO_LARGE = -5
+RANSAC_NOALLOC_MAX_PTS, RANSAC_NOALLOC_MAX_HYP = 4096, 9472
 
 # every symbol include/hg.h declares
 EXPORTS = [
@@ -40,7 +43,7 @@ EXPORTS = [
     "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward", "hg_aca_rect_backward_soa", "hg_offsets_to_grid_backward", "hg_affine_batched",
     "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64", "hg_ransac_workspace_bytes", "hg_ransac_hypothesize_score",
     "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive", "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex",
-    "hg_status_string", "hg_version", "hg_built_for_sm",
+    "hg_ransac_hypothesize_score_noalloc", "hg_status_string", "hg_version", "hg_built_for_sm",
 ]
 
 
@@ -100,13 +103,15 @@ def lib() -> ctypes.CDLL:
         L.hg_ransac_adaptive_ex.argtypes = [_vp, _vp, _c_i32, ctypes.c_uint64, _c_i64, _c_i64, _c_f32, _c_f32, _vp, _vp, _vp, _vp, _vp,
                                             _vp, _vp, _vp, ctypes.c_size_t, _vp]
         L.hg_ransac_hypothesize_score_host.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp]
+        L.hg_ransac_hypothesize_score_noalloc.argtypes = [_vp, _vp, _c_i32, _vp, _c_i64, _c_f32, _vp, _vp, _vp, _vp, _vp]
         L.hg_status_string.argtypes = [_c_int]
         L.hg_status_string.restype = ctypes.c_char_p
         for name in ("hg_aca_batched", "hg_sks_batched", "hg_aca_batched_host", "hg_sks_batched_host",
                      "hg_offsets_to_grid", "hg_offsets_to_warp", "hg_aca_rect_batched", "hg_aca_rect_backward",
                      "hg_aca_rect_backward_soa", "hg_offsets_to_grid_backward", "hg_affine_batched", "hg_sk_batched", "hg_aca_batched_f64", "hg_sks_batched_f64",
                      "hg_ransac_hypothesize_score", "hg_ransac_hypothesize_score_host", "hg_ransac_adaptive",
-                     "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex", "hg_version", "hg_built_for_sm"):
+                     "hg_ransac_hypothesize_score_ex", "hg_ransac_adaptive_ex", "hg_ransac_hypothesize_score_noalloc",
+                     "hg_version", "hg_built_for_sm"):
             getattr(L, name).restype = _c_int
         _lib = L
     return _lib
@@ -569,6 +574,34 @@ def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, co
 
 
 hg_ransac_hypothesize_score_ex = hg_ransac_hypothesize_score      # one Python function serves both C entry points
+
+
+def hg_ransac_hypothesize_score_noalloc(src_xy, dst_xy, hyp_idx, threshold_px: float, counts=None, best=None, stream=None):
+    """hg_ransac_hypothesize_score without a workspace, for code that must not allocate device memory while it runs
+    (called from inside another application's frame loop or memory pool, under a latency budget, or beside threads
+    that are capturing streams): the scratch is a fixed 28 KB array inside libhg, so the limits are
+    n_pts <= RANSAC_NOALLOC_MAX_PTS (4096) and n_hyp <= RANSAC_NOALLOC_MAX_HYP (9472); larger calls raise HgError
+    with status HG_ERR_TOO_LARGE (-5).  In keeping with that, this wrapper creates no tensor either: every output is
+    the caller's -- counts int32 [n_hyp] or None, best = (best_H [3,3] f32, best_index [1] i64, best_count [1] i32) or
+    None -- and the return value is None.  Results equal those of hg_ransac_hypothesize_score.  All calls of one
+    device share the one array: keep them on one stream (or ordered by events); calls that overlap on the GPU race.
+    The first call on a device looks up the array's address; make it at start-up, outside any stream capture."""
+    n_pts, n_hyp = int(src_xy.shape[0]), int(hyp_idx.shape[0])
+    if tuple(src_xy.shape) != (n_pts, 2) or tuple(dst_xy.shape) != (n_pts, 2):
+        raise ValueError("src_xy, dst_xy are float32 [n_pts, 2]")
+    if tuple(hyp_idx.shape) != (n_hyp, 4):
+        raise ValueError("hyp_idx is int32 [n_hyp, 4]")
+    if counts is not None and counts.numel() < n_hyp:
+        raise ValueError("counts is int32 [n_hyp]")
+    best_H, best_index, best_count = best if best is not None else (None, None, None)
+    dev = _same_device(src_xy, dst_xy, hyp_idx, counts, best_H, best_index, best_count)
+    args = (_ptr(src_xy, torch.float32, "cuda", "src_xy"), _ptr(dst_xy, torch.float32, "cuda", "dst_xy"), n_pts,
+            _ptr(hyp_idx, torch.int32, "cuda", "hyp_idx"), n_hyp, float(threshold_px),
+            _ptr(counts, torch.int32, "cuda", "counts"), _ptr(best_H, torch.float32, "cuda", "best_H"),
+            _ptr(best_index, torch.int64, "cuda", "best_index"), _ptr(best_count, torch.int32, "cuda", "best_count"))
+    with _on(dev):
+        st = _c("hg_ransac_hypothesize_score_noalloc")(*args, _stream(stream))
+    _check(st, "hg_ransac_hypothesize_score_noalloc")
 
 
 def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, threshold_px: float, confidence: float,

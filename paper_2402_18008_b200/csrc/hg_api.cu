@@ -11,6 +11,7 @@ extern "C" const char* hg_status_string(int status)
         case HG_ERR_ALIGNMENT:   return "HG_ERR_ALIGNMENT: a base pointer is not sufficiently aligned";
         case HG_ERR_CUDA:        return "HG_ERR_CUDA: a CUDA runtime call or kernel launch failed";
         case HG_ERR_WORKSPACE:   return "HG_ERR_WORKSPACE: workspace smaller than hg_ransac_workspace_bytes()";
+        case HG_ERR_TOO_LARGE:   return "HG_ERR_TOO_LARGE: size beyond the fixed capacity of a no-allocation entry point";
         default:                 return "unknown hg status";
     }
 }

@@ -1447,3 +1447,112 @@ extern "C" int hg_ransac_hypothesize_score_host(const float* src_xy, const float
     if (dev) cudaFree(dev);
     return rc;
 }
+
+// ---- the entry point that allocates nothing (include/hg.h: hg_ransac_hypothesize_score_noalloc) ----------------------
+// For callers that cannot give the library a workspace because they cannot allocate one (see the header for who they
+// are).  The one-kernel small-call path needs little scratch -- the header and one TinySlot per 32 hypotheses -- so
+// that scratch is a fixed array in the library image.  The launch below repeats the tiny-call branch of ransac_run on
+// purpose: the existing entry points are left exactly as they are.
+namespace hg {
+
+constexpr size_t kNoAllocScratchBytes = (kHeaderBytes + size_t(kTinyMaxGroups) * sizeof(TinySlot) + 255) & ~size_t(255);
+static_assert(kNoAllocScratchBytes == HG_RANSAC_NOALLOC_SCRATCH_BYTES, "hg.h states the size of the array");
+static_assert(HG_RANSAC_NOALLOC_MAX_HYP == kTinyMaxGroups * kTinyHyp, "hg.h states the hypothesis limit");
+static_assert(HG_RANSAC_NOALLOC_MAX_PTS == kFusedMaxPts, "hg.h states the table limit");
+
+// Device memory that exists on every GPU that loads this module, from load to process exit.  In HOST code this name is
+// only a handle for the runtime's symbol calls -- it is not the device address and must never be passed to a kernel.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocScratchBytes];
+
+// The device address of g_noalloc_scratch on the CURRENT device: asked from the runtime once per device (the array has a
+// different address on each), under a lock, and cached.  No allocation: the array is part of the loaded module.
+static int noalloc_scratch_address(unsigned char** out)
+{
+    constexpr int kMaxDevices = 64;
+    static std::mutex m;
+    static unsigned char* addr[kMaxDevices] = {};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { (void)cudaGetLastError(); return HG_ERR_CUDA; }
+    std::lock_guard<std::mutex> lock(m);
+    if (!addr[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || !p) { (void)cudaGetLastError(); return HG_ERR_CUDA; }
+        if (!aligned16(p)) return HG_ERR_ALIGNMENT;           // cannot happen (__align__(256)); a wrong address must not get through
+        addr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = addr[dev];
+    return HG_OK;
+}
+
+}  // namespace hg
+
+extern "C" int hg_ransac_hypothesize_score_noalloc(const float* src_xy, const float* dst_xy, int32_t n_pts,
+                                                   const int32_t* hyp_idx, int64_t n_hyp, float threshold_px,
+                                                   int32_t* counts, float* best_H, int64_t* best_index,
+                                                   int32_t* best_count, void* cuda_stream)
+{
+    using namespace hg;
+    if (n_hyp < 0 || n_pts < 4) return HG_ERR_INVALID_ARG;
+    if (!(threshold_px > 0.0f) || !(threshold_px < 3.0e38f)) return HG_ERR_INVALID_ARG;
+    if (n_hyp == 0) return HG_OK;
+    if (!src_xy || !dst_xy || !hyp_idx) return HG_ERR_INVALID_ARG;
+    if (!aligned16(src_xy) || !aligned16(dst_xy) || !aligned16(hyp_idx)) return HG_ERR_ALIGNMENT;
+    if ((counts && !aligned4(counts)) || (best_H && !aligned4(best_H)) ||
+        (best_index && (reinterpret_cast<uintptr_t>(best_index) & 7u)) || (best_count && !aligned4(best_count)))
+        return HG_ERR_ALIGNMENT;
+    // the fixed array holds the scratch of at most this much; nothing has been enqueued yet
+    if (n_pts > HG_RANSAC_NOALLOC_MAX_PTS || n_hyp > HG_RANSAC_NOALLOC_MAX_HYP) return HG_ERR_TOO_LARGE;
+
+    unsigned char* ws = nullptr;                               // device address of the array on the current device
+    const int rc = noalloc_scratch_address(&ws);
+    if (rc != HG_OK) return rc;
+
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    RansacHeader* hdr = reinterpret_cast<RansacHeader*>(ws);
+    TinySlot* cand = reinterpret_cast<TinySlot*>(ws + kHeaderBytes);
+    const float2* s2 = reinterpret_cast<const float2*>(src_xy);
+    const float2* d2 = reinterpret_cast<const float2*>(dst_xy);
+    const int n_pairs = (n_pts + 1) / 2;
+    const double t = static_cast<double>(threshold_px);
+    const double inv_t = 1.0 / t;
+    const int64_t groups = (n_hyp + kTinyHyp - 1) / kTinyHyp;
+    if (kHeaderBytes + size_t(groups) * sizeof(TinySlot) > kNoAllocScratchBytes) return HG_ERR_TOO_LARGE;
+
+    HypSource hs;
+    hs.idx = reinterpret_cast<const int4*>(hyp_idx);
+    hs.idx_out = nullptr;
+    hs.seed = 0ull;
+    hs.flags = 0u;
+    hs.reject_lim2 = 0.0;
+    hs.check_stop = 0;
+    hs.acc = nullptr;
+    hs.h0 = 0; hs.h1 = n_hyp;
+    const int parts = tiny_parts(n_pairs, groups);
+    hs.part_entries = ((n_pairs + parts - 1) / parts + 7) & ~7;
+    const size_t smem = size_t(n_pairs) * kTinyEntry * sizeof(float4) + size_t(kQueueCap) * kTinyThreads * sizeof(unsigned);
+    if (cudaFuncSetAttribute(ransac_tiny_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return HG_ERR_CUDA;
+    }
+    // the array keeps the previous call's header, ticket and stamped slots: what this call reads starts at zero
+    ransac_zero_kernel<<<1, 256, 0, st>>>(reinterpret_cast<uint4*>(hdr), int((kHeaderBytes + size_t(groups) * sizeof(TinySlot)) / 16));
+    if (launch_status() != HG_OK) return HG_ERR_CUDA;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(groups), static_cast<unsigned>(parts), 1);
+    cfg.blockDim = dim3(kTinyThreads, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attrs[2];
+    attrs[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attrs[0].val.programmaticStreamSerializationAllowed = 1;
+    attrs[1].id = cudaLaunchAttributeClusterDimension;
+    attrs[1].val.clusterDim.x = 1; attrs[1].val.clusterDim.y = static_cast<unsigned>(parts); attrs[1].val.clusterDim.z = 1;
+    cfg.attrs = attrs;
+    cfg.numAttrs = parts > 1 ? 2 : 1;
+    if (cudaLaunchKernelEx(&cfg, ransac_tiny_kernel, s2, d2, n_pts, n_pairs, hs, inv_t, t, counts, hdr, cand, best_H,
+                           reinterpret_cast<long long*>(best_index), best_count, static_cast<long long*>(nullptr)) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return HG_ERR_CUDA;
+    }
+    return launch_status();
+}

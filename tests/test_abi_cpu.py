@@ -34,7 +34,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_status_strings():
     assert hg.hg_status_string(0) == "HG_OK"
-    for code in (-1, -2, -3, -4):
+    for code in (-1, -2, -3, -4, -5):
         assert hg.hg_status_string(code).startswith("HG_ERR_")
     assert "unknown" in hg.hg_status_string(-99)
 
@@ -178,6 +178,28 @@ def test_ransac_argument_validation_and_workspace():
     assert call(idx=FAKE + 4) == -2
     assert call(bi=FAKE + 4) == -2
     assert call(wsb=128) == -4
+
+
+def test_ransac_noalloc_argument_validation_and_limits():
+    """Everything hg_ransac_hypothesize_score_noalloc refuses is refused before it touches the GPU (so it can be checked here)."""
+    f = hg.lib().hg_ransac_hypothesize_score_noalloc
+    ok = [FAKE, FAKE, 100, FAKE, 10, 3.0, FAKE, FAKE, FAKE, FAKE, None]
+    names = ["src", "dst", "n_pts", "idx", "n_hyp", "t", "counts", "bH", "bi", "bc", "st"]
+
+    def call(**kw):
+        a = list(ok)
+        for k, v in kw.items():
+            a[names.index(k)] = v
+        return f(*a)
+
+    assert call(n_hyp=0) == 0
+    assert call(n_pts=3) == -1 and call(n_hyp=-1) == -1 and call(t=0.0) == -1 and call(src=None) == -1 and call(idx=None) == -1
+    assert call(idx=FAKE + 4) == -2 and call(bi=FAKE + 4) == -2
+    assert call(n_pts=hg.RANSAC_NOALLOC_MAX_PTS + 1) == hg.HG_ERR_TOO_LARGE == -5
+    assert call(n_hyp=hg.RANSAC_NOALLOC_MAX_HYP + 1) == -5 and call(n_hyp=1 << 40) == -5
+    text = (ROOT / "include" / "hg.h").read_text()
+    assert "#define HG_RANSAC_NOALLOC_MAX_PTS       %d" % hg.RANSAC_NOALLOC_MAX_PTS in text
+    assert "#define HG_RANSAC_NOALLOC_MAX_HYP       %d" % hg.RANSAC_NOALLOC_MAX_HYP in text
 
 
 def test_ransac_adaptive_argument_validation():

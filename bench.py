@@ -348,7 +348,7 @@ def run_extras(hg, W, dev, src, dst, H, peak, peak_src, cpu=True):
     # The scale of the paper's Table 6 (<= 1000 matches per image pair, a few to a few thousand loops; solver +
     # verification loops 4.5-154 us on a CPU core): us per call, plain launches and inside a CUDA graph.
     small = {}
-    for n_pts_s, n_hyp_s in ((1000, 1024), (500, 256), (2000, 16384)):       # the last one: the generic split path (5 launches)
+    for n_pts_s, n_hyp_s in ((1000, 1024), (500, 256), (2000, 16384)):       # the last one: still the one-kernel path (<= 20 480 hypotheses on <= 2048 points)
         wls = W.ransac_workload(n_pts=n_pts_s, n_hyp=n_hyp_s, seed=W.SEED_BASE + 44, device=dev)
         wss = torch.empty(hg.hg_ransac_workspace_bytes(n_pts_s, n_hyp_s), dtype=torch.uint8, device=dev)
         o0 = hg.hg_ransac_hypothesize_score(wls["src_xy"], wls["dst_xy"], wls["hyp_idx"], 3.0, want_counts=False, workspace=wss)

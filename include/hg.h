@@ -12,11 +12,12 @@
  *  - Every pointer is a DEVICE pointer owned by the caller unless the name ends in `_host`
  *    (those entry points take HOST pointers, pinned or pageable, and do the copies themselves).
  *  - The library allocates no device memory (the `_host` entry points allocate and free their
- *    own staging buffers and streams inside the call) and keeps no state, with one exception: the
- *    RANSAC entry points stage tables of <= 4096 correspondences in the device's 64 KB constant
- *    bank.  Calls that do so are ordered against each other through an internal event (thread-safe;
- *    they may be issued from any streams), but under CUDA stream capture that ordering cannot be
- *    recorded: replays of a captured RANSAC call must not overlap other RANSAC calls on that device.
+ *    own staging buffers and streams inside the call).  Its only state is internal to the RANSAC
+ *    entry points, which stage tables of <= 4096 correspondences in the device's 64 KB constant
+ *    bank: calls that do so are ordered against each other through an internal event, and a call made
+ *    on a capturing stream stages its table in shared memory instead, so every entry point is
+ *    thread-safe and may be issued on any streams, captured or not (the one exception is
+ *    hg_ransac_hypothesize_score_noalloc, whose calls share a fixed scratch array -- see there).
  *  - Device entry points only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as void*;
  *    NULL = the legacy default stream) and never synchronise; `_host` entry points return
  *    after their result is complete in host memory.
@@ -259,7 +260,9 @@ HG_API int hg_sks_batched_f64(const double* src, const double* dst, double* H, i
  * the band is decided in fp64 by the same kernel, so counts equal an fp64 evaluation.
  * Launches: a call of <= 9472 hypotheses (<= 20 480 on <= 2048 points) on <= 4096 points is one kernel behind a
  * one-CTA zeroing kernel (7 us for 1024 x 1000); larger calls are zero + prep + score
- * (+ best for calls of fewer than 148 x 512 hypotheses) + finalize.  Capturable in a CUDA graph; never synchronises.
+ * (+ best for calls of fewer than 148 x 512 hypotheses) + finalize.  Never synchronises.  Capturable in a CUDA graph: a
+ * captured call reads its table from shared-memory stages rather than the constant bank (7-10 % slower on tables of <= 4096
+ * points), which makes the graph self-contained -- its replays may overlap any other call of the library.
  *   src_xy, dst_xy : float[n_pts][2] correspondences                  (read)
  *   hyp_idx        : int32[n_hyp][4], the 4 indices of a row distinct and in [0,n_pts)
  *                    (out-of-range indices are undefined behaviour)   (read, 16 B per hyp.)
@@ -342,7 +345,9 @@ HG_API int hg_ransac_adaptive_ex(const float* src_xy, const float* dst_xy, int32
 
 /* After a RANSAC call has completed on its stream, the first 6 int64 words of the workspace hold
  * statistics of that call (device memory; copy them out to read):
- *   [0] packed best key, [1] number of hypotheses that had at least one pair decided in fp64,
+ *   [0] packed best key, [1] number of (hypothesis, table slice) combinations with at least one pair decided in fp64
+ *   (= the number of such hypotheses when the launch does not split the table; the one-kernel path and the split launches
+ *   count a hypothesis once per slice it was undecided in),
  *   [2] number of (hypothesis, point) pairs decided in fp64, [3] hypotheses scored (adaptive mode),
  *   [4] hypotheses rejected by HG_RANSAC_REJECT_DEGENERATE, [5] pairs that fell inside the table-wide
  *   fp32 band and were re-tested against the per-pair band.                  */

@@ -1116,6 +1116,8 @@ constexpr int kTinyMaxGroups = 296;     // tiny path: at most two CTAs per SM's 
 constexpr int kTinyMaxGroupsWide = 640; // ... and up to 20 480 hypotheses on tables of <= kTinyWidePts points, where it still beats the
 constexpr int kTinyWidePts = 2048;      //     five launches of the generic path (16 384 x 2000: 30.6 vs 36.5 us; 37 888 x 2000: 56 vs 52)
 constexpr size_t kTicketBytes = 128;    // so that the accumulator area of the smallest call still holds one TinySlot
+// dynamic shared memory of the largest one-kernel call: the packed table of kFusedMaxPts points + the per-thread queues
+constexpr size_t kTinyMaxSmem = size_t(kFusedMaxPts / 2) * kTinyEntry * sizeof(float4) + size_t(kQueueCap) * kTinyThreads * sizeof(unsigned);
 static bool may_split(int64_t n_hyp) { return (n_hyp + kRBlock - 1) / kRBlock < kSplitBelowCtas; }
 
 // Tiny path: CTAs (table parts) per group of 32 hypotheses -- a power of two <= 8 (the cluster size), doubled while the
@@ -1156,24 +1158,21 @@ namespace hg {
 
 // The constant-bank copy of the table is the one piece of per-device state in the library.  Calls that use it are
 // ordered against each other: a call makes its stream wait for the event the previous user recorded after its last
-// scoring launch, then overwrites c_table.  Under stream capture no cross-stream ordering can be expressed (and
-// none is recorded): replays of a captured call must not overlap other RANSAC work on the same device.
+// scoring launch, then overwrites c_table.  Under stream capture no such cross-stream ordering can be recorded, so a
+// call on a capturing stream never uses the constant bank (ransac_run takes the staged shared-memory operands
+// instead): a captured call is self-contained and its replays may overlap any other RANSAC work.
 class ConstTableGuard {
 public:
     explicit ConstTableGuard(cudaStream_t st) : st_(st), lock_(mutex())
     {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { status_ = HG_ERR_CUDA; return; }
-        capturing_ = cs != cudaStreamCaptureStatusNone;
         if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) { status_ = HG_ERR_CUDA; return; }
-        if (capturing_) return;
         Slot& s = slots()[dev_];
         if (!s.ev && cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming) != cudaSuccess) { status_ = HG_ERR_CUDA; return; }
         if (s.used && cudaStreamWaitEvent(st, s.ev, 0) != cudaSuccess) status_ = HG_ERR_CUDA;
     }
     ~ConstTableGuard()
     {
-        if (status_ != HG_OK || capturing_) return;
+        if (status_ != HG_OK) return;
         Slot& s = slots()[dev_];
         if (cudaEventRecord(s.ev, st_) == cudaSuccess) s.used = true;
     }
@@ -1187,7 +1186,6 @@ private:
     cudaStream_t st_;
     std::unique_lock<std::mutex> lock_;
     int dev_ = -1, status_ = HG_OK;
-    bool capturing_ = false;
 };
 
 // Shared by the device entry points.  Sampling mode: hyp_idx == nullptr.  round_hyp == n_hyp and
@@ -1229,7 +1227,9 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
         const int parts = tiny_parts(n_pairs, tiny_groups);
         hs.part_entries = ((n_pairs + parts - 1) / parts + 7) & ~7;
         const size_t smem = size_t(n_pairs) * kTinyEntry * sizeof(float4) + size_t(kQueueCap) * kTinyThreads * sizeof(unsigned);
-        if (cudaFuncSetAttribute(ransac_tiny_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
+        // always the largest size the path can ask for: the attribute belongs to the function, not to the launch, so a per-call
+        // value set by one host thread could be lowered by another between this call and the launch below
+        if (cudaFuncSetAttribute(ransac_tiny_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTinyMaxSmem)) != cudaSuccess)
             return HG_ERR_CUDA;
         ransac_zero_kernel<<<1, 256, 0, st>>>(reinterpret_cast<uint4*>(hdr), int((kHeaderBytes + size_t(tiny_groups) * sizeof(TinySlot)) / 16));
         if (launch_status() != HG_OK) return HG_ERR_CUDA;
@@ -1268,7 +1268,11 @@ static int ransac_run(const float* src_xy, const float* dst_xy, int32_t n_pts, c
     // Operand path: a table that fits the constant bank goes through the uniform datapath -- also when the launch is split
     // over table parts (mid-size calls: 7-10 % faster than the staged shared-memory sweep); the verification mode never
     // reads the table.
-    const bool use_const = n_pairs <= kConstPairs && !(flags & HG_RANSAC_DECIDE_ALL_F64);
+    // A call that is being captured into a CUDA graph stages its operands in shared memory: the constant bank is shared by
+    // every stream of the device, and a replay cannot be ordered against the calls that will be running then.
+    cudaStreamCaptureStatus capture = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &capture) != cudaSuccess) { (void)cudaGetLastError(); return HG_ERR_CUDA; }
+    const bool use_const = n_pairs <= kConstPairs && !(flags & HG_RANSAC_DECIDE_ALL_F64) && capture == cudaStreamCaptureStatusNone;
     const size_t stash = size_t(kQueueCap) * kRBlock * sizeof(unsigned) + kStages * sizeof(uint64_t);
     const size_t smem = (use_const ? 0 : size_t(kStages) * kChunkPairs * 32) + stash;
     auto* score = use_const ? ransac_score_kernel<true> : ransac_score_kernel<false>;
@@ -1530,7 +1534,7 @@ extern "C" int hg_ransac_hypothesize_score_noalloc(const float* src_xy, const fl
     const int parts = tiny_parts(n_pairs, groups);
     hs.part_entries = ((n_pairs + parts - 1) / parts + 7) & ~7;
     const size_t smem = size_t(n_pairs) * kTinyEntry * sizeof(float4) + size_t(kQueueCap) * kTinyThreads * sizeof(unsigned);
-    if (cudaFuncSetAttribute(ransac_tiny_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) {
+    if (cudaFuncSetAttribute(ransac_tiny_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTinyMaxSmem)) != cudaSuccess) {
         (void)cudaGetLastError();
         return HG_ERR_CUDA;
     }

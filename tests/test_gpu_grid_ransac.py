@@ -323,6 +323,54 @@ def test_ransac_tiny_calls_every_cluster_size(n_pts, n_hyp):
     assert chk["best_count"].item() == cc.max() and chk["best_index"].item() == int(np.argmax(cc))
 
 
+def test_ransac_generic_calls_in_a_graph_replayed_beside_an_eager_call():
+    """A captured mid-size call must not touch the constant bank (hg.h: a call on a capturing stream stages its table in
+    shared memory): a graph holding a 4096 x 100 000 and a 6001 x 9000 call is replayed three times on a side stream while
+    eager 4096 x 2^18 calls (constant-bank path) run on another stream.  Every result equals the same call issued alone,
+    and the captured calls match the oracle."""
+    t = 3.0
+    shapes = [(4096, 100000), (6001, 9000)]
+    wls = [W.ransac_workload(n_pts=p, n_hyp=h, seed=W.SEED_BASE + 5000 + p) for p, h in shapes]
+    big = W.ransac_workload(n_pts=4096, n_hyp=1 << 18, seed=W.SEED_BASE + 5999)
+    dev_in = [tuple(wl[k].to(DEV) for k in ("src_xy", "dst_xy", "hyp_idx")) for wl in wls]
+    bs, bd, bidx = (big[k].to(DEV) for k in ("src_xy", "dst_xy", "hyp_idx"))
+    alone = [hg.hg_ransac_hypothesize_score(s, d, i, t) for s, d, i in dev_in]                      # eager, nothing else running
+    big_alone = hg.hg_ransac_hypothesize_score(bs, bd, bidx, t)
+    torch.cuda.synchronize()
+    outs = []
+    for (p, h), (s, d, i) in zip(shapes, dev_in):                                                   # outputs the graph writes into
+        outs.append({"counts": torch.zeros(h, dtype=torch.int32, device=DEV), "best_H": torch.zeros(3, 3, device=DEV),
+                     "best_index": torch.zeros(1, dtype=torch.int64, device=DEV), "best_count": torch.zeros(1, dtype=torch.int32, device=DEV),
+                     "workspace": torch.empty(hg.hg_ransac_workspace_bytes(p, h), dtype=torch.uint8, device=DEV)})
+    side, other = torch.cuda.Stream(), torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            for (s, d, i), o in zip(dev_in, outs):
+                hg.hg_ransac_hypothesize_score(s, d, i, t, counts=o["counts"], workspace=o["workspace"],
+                                               best=(o["best_H"], o["best_index"], o["best_count"]))
+    torch.cuda.synchronize()
+    for rep in range(3):
+        for o in outs:
+            o["counts"].fill_(-1)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(other):
+            eager = [hg.hg_ransac_hypothesize_score(bs, bd, bidx, t) for _ in range(3)]               # ~0.5 ms each, constant bank
+        with torch.cuda.stream(side):
+            g.replay()
+        torch.cuda.synchronize()
+        for o, a in zip(outs, alone):
+            assert torch.equal(o["counts"], a["counts"]), rep
+            assert o["best_index"].item() == a["best_index"].item() and o["best_count"].item() == a["best_count"].item()
+            assert torch.equal(o["best_H"], a["best_H"])
+        for e in eager:
+            assert torch.equal(e["counts"], big_alone["counts"]), rep
+            assert e["best_index"].item() == big_alone["best_index"].item() and torch.equal(e["best_H"], big_alone["best_H"])
+    for wl, o in zip(wls, outs):
+        ref = oracle.ransac(wl["src_xy"].numpy(), wl["dst_xy"].numpy(), wl["hyp_idx"].numpy(), t, band_rel=1e-4)
+        check_ransac(wl, t, o, ref)
+
+
 def test_ransac_tiny_call_replayed_in_a_cuda_graph():
     """The zero kernel and its programmatic dependent are captured as two graph nodes; every replay must start from a
     clean header (ticket, packed maximum) and see the inputs of that replay."""

@@ -74,3 +74,27 @@ def test_combine_best_over_gloo(world, n_hyp, tie):
         assert p.exitcode == 0
     assert all(r[1] for r in res), res
     assert len({(r[2], r[3]) for r in res}) == 1           # every rank holds the same answer
+
+
+def test_bench_gpus_n_starts_n_ranks_or_fails_loudly():
+    """bench.py --gpus N (launch logic only, no GPU): without a launcher and N > 1 it re-executes itself under
+    torch.distributed.run with N ranks on 127.0.0.1; it refuses when fewer than N devices exist (a 1-GPU box must not print an
+    n_gpus: 1 line for --gpus 2); a launcher's WORLD_SIZE is respected and must agree with --gpus."""
+    import argparse
+    import sys
+    import bench
+    a = lambda gpus, impl="ours": argparse.Namespace(gpus=gpus, impl=impl)
+    argv = ["--gpus", "2", "--steps", "3", "--warmup", "3"]
+    cmd = bench.self_launch_if_needed(a(2), argv, env={}, device_count=8)
+    assert cmd[:3] == [sys.executable, "-m", "torch.distributed.run"] and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--nproc-per-node") + 1] == "2" and cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert 0 < int(cmd[cmd.index("--master-port") + 1]) < 65536
+    assert cmd[-len(argv) - 1].endswith("bench.py") and cmd[-len(argv):] == argv
+    assert bench.self_launch_if_needed(a(1), ["--gpus", "1"], env={}, device_count=1) is None            # one GPU: this process
+    assert bench.self_launch_if_needed(a(2), argv, env={"WORLD_SIZE": "2"}, device_count=8) is None       # already launched
+    assert bench.self_launch_if_needed(a(4, "reference"), argv, env={}, device_count=0) is None           # the oracle arm: rank 0 only
+    with pytest.raises(SystemExit) as e:
+        bench.self_launch_if_needed(a(2), argv, env={}, device_count=1)
+    assert "only 1 CUDA device" in str(e.value)
+    with pytest.raises(SystemExit):
+        bench.self_launch_if_needed(a(8), argv, env={"WORLD_SIZE": "2"}, device_count=8)

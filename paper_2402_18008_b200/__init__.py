@@ -137,9 +137,11 @@ class CallPlan:
     """Records the C calls the binding makes inside `with hg.CallPlan() as plan:` -- function, pointers, sizes, stream, as
     marshalled and checked once -- and re-issues exactly those calls on `plan()`.  For loops that call the library on the
     same buffers every iteration (the paper's Table 6 / Table 7 regime): a 1 us kernel then costs a ctypes call, not the
-    8 us of tensor checks and conversions.  The caller keeps the tensors alive and at their addresses; the stream is the
-    one that was current while recording.  One plan is recorded at a time, by one thread.  (A CUDA graph of the same calls is
-    cheaper still; this needs no capture.)"""
+    8 us of tensor checks and conversions.  The plan holds a reference to every tensor whose address it recorded (the caller's
+    and the ones the wrappers allocated: outputs, workspaces), so dropping a returned dict cannot hand that memory to another
+    tensor while the plan lives; each call is replayed with the device that was current when it was recorded, on the stream
+    that was current then.  One plan is recorded at a time, by one thread.  (A CUDA graph of the same calls is cheaper still;
+    this needs no capture.)"""
 
     def __init__(self):
         self._calls = []
@@ -161,8 +163,12 @@ class CallPlan:
         return len(self._calls)
 
     def __call__(self):
-        for f, args, name in self._calls:
-            st = f(*args)
+        for f, args, name, dev in self._calls:
+            if dev != torch.cuda.current_device():
+                with torch.cuda.device(dev):
+                    st = f(*args)
+            else:
+                st = f(*args)
             if st != HG_OK:
                 raise HgError(st, name)
 
@@ -175,7 +181,7 @@ def _c(name: str):
     plan = _plan
 
     def recorded(*args):
-        plan._calls.append((f, args, name))
+        plan._calls.append((f, args, name, torch.cuda.current_device()))     # (called inside `with _on(dev)`)
         return f(*args)
     return recorded
 
@@ -192,6 +198,8 @@ def _ptr(t, dtype, device_type: str, name: str):
         raise ValueError("%s must live on %s, got %s (no fallback path exists)" % (name, device_type, t.device))
     if not t.is_contiguous():
         raise ValueError("%s must be contiguous" % name)
+    if _plan is not None:
+        _plan._keep.append(t)             # a recorded call holds this address: the plan keeps the tensor alive
     return _vp(t.data_ptr())
 
 
@@ -562,8 +570,9 @@ def hg_ransac_hypothesize_score(src_xy, dst_xy, hyp_idx, threshold_px: float, co
             _ptr(hyp_idx, torch.int32, "cuda", "hyp_idx"), n_hyp, float(threshold_px))
     tail = (_ptr(counts, torch.int32, "cuda", "counts"), _ptr(best_H, torch.float32, "cuda", "best_H"),
             _ptr(best_index, torch.int64, "cuda", "best_index"), _ptr(best_count, torch.int32, "cuda", "best_count"),
-            _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()), _stream(stream))
+            _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()))
     with _on(dev):
+        tail = tail + (_stream(stream),)          # the current stream OF THE TENSORS' DEVICE
         if opt is None:
             st = _c("hg_ransac_hypothesize_score")(*head, *tail)
         else:
@@ -631,8 +640,9 @@ def hg_ransac_adaptive(src_xy, dst_xy, seed: int, max_hyp: int, round_hyp: int, 
     tail = (_ptr(counts, torch.int32, "cuda", "counts"), _ptr(idx, torch.int32, "cuda", "hyp_idx_out"),
             _ptr(best_H, torch.float32, "cuda", "best_H"), _ptr(best_index, torch.int64, "cuda", "best_index"),
             _ptr(best_count, torch.int32, "cuda", "best_count"), _ptr(n_eval, torch.int64, "cuda", "n_evaluated"),
-            _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()), _stream(stream))
+            _ptr(workspace, torch.uint8, "cuda", "workspace"), int(workspace.numel()))
     with _on(dev):
+        tail = tail + (_stream(stream),)          # the current stream OF THE TENSORS' DEVICE
         if opt is None:
             st = _c("hg_ransac_adaptive")(*head, *tail)
         else:

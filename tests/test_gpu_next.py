@@ -372,6 +372,27 @@ def test_call_plan_replays_the_recorded_calls():
                 pass
 
 
+def test_call_plan_keeps_the_tensors_it_recorded_alive():
+    """A recorded call holds raw addresses -- also of the tensors the wrapper allocated itself (counts, best_*, workspace).  The
+    plan must keep them alive: after the caller drops the returned dict, memory handed out by the allocator must not be what a
+    replay writes into."""
+    import gc
+    wl = W.ransac_workload(n_pts=1000, n_hyp=1024, seed=8)
+    s, d, idx = (wl[k].to(DEV) for k in ("src_xy", "dst_xy", "hyp_idx"))
+    off = W.offsets_workload(1024, seed=3).to(DEV)
+    with hg.CallPlan() as plan:
+        hg.hg_ransac_hypothesize_score(s, d, idx, 3.0)                                    # every output dropped on the spot
+        hg.hg_offsets_to_grid(off, 0.0, 0.0, 127.0, 127.0, 16, 16)                       # H and grid allocated by the wrapper, dropped
+    gc.collect()
+    kept = sum(t.numel() * t.element_size() for t in plan._keep if isinstance(t, torch.Tensor))
+    assert kept >= 1024 * 4 + 1024 * 16 * 16 * 8                                          # counts + grid at least
+    canary = [torch.full((4096,), 12345, dtype=torch.int32, device=DEV) for _ in range(128)]   # what the allocator hands out next
+    torch.cuda.synchronize()
+    plan(); plan()
+    torch.cuda.synchronize()
+    assert all(bool((c == 12345).all()) for c in canary)
+
+
 # ---- 8(f) row 2, second half: backward through the grid --------------------------------------------------------------
 # tolerance (DESIGN.md section 8): the per-pixel partials and the per-thread sums are fp32 -- about 12 roundings per term
 # plus a serial sum of <= 64 terms, |term| <= |g| * max|d grid / d offset| (< 2 for these quadrangles) -- the CTA

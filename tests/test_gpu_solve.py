@@ -183,27 +183,48 @@ def test_host_buffer_pipeline_matches_device_call():
     assert torch.equal(out3, ref)
 
 
-def test_full_size_config3_sampled_against_oracle():
-    """C3 at BASELINE size (2^26 sets, the launch configuration bench.py times): generated on the
-    GPU, solved in one call, and a strided sample of 2^16 outputs compared with the oracle."""
-    n = 1 << 26
+def test_full_size_config3_every_set_against_oracle():
+    """C3 at BASELINE size (2^26 sets, the launch configuration bench.py times): generated on the GPU, solved in ONE call per
+    method, and EVERY one of the 2^26 outputs of both methods compared with the oracle, slab by slab (2^22 sets per slab: every
+    thread, every vector lane and every CTA of the timed launch is looked at).  Rule: util.check_h_parity_lazy = the rule of
+    every other solver test.  The literal all-sample statistics are printed (DESIGN.md section 8 quotes them)."""
+    from util import check_h_parity_lazy
+    n, slab = 1 << 26, 1 << 22
     free, _ = torch.cuda.mem_get_info()
-    if free < 12 * (1 << 30):
-        pytest.skip("needs ~12 GB of free device memory")
+    if free < 16 * (1 << 30):
+        pytest.skip("needs ~16 GB of free device memory")
     src, dst = W.general_sets(n, seed=W.SEED_BASE + 3, device=DEV, soa=True)
-    H = hg.hg_aca_batched(src, dst, norm=hg.NORM_NONE)
+    Ha = hg.hg_aca_batched(src, dst, norm=hg.NORM_NONE)
+    Hs = hg.hg_sks_batched(src, dst, norm=hg.NORM_NONE)
     torch.cuda.synchronize()
-    idx = torch.arange(0, n, n // (1 << 16), device=DEV)
-    idx = torch.cat([idx, torch.tensor([n - 1, n - 2, n - 3, n - 4], device=DEV)])
-    s = W.to_aos(src[:, idx].contiguous()).cpu().numpy()
-    d = W.to_aos(dst[:, idx].contiguous()).cpu().numpy()
-    Hn = W.h_soa_to_aos(H[:, idx].contiguous().cpu()).numpy()
-    stats = check_parity(Hn, s, d, "aca")
-    print("C3 sampled", stats)
-    Hs = hg.hg_sks_batched(src, dst, H=H, norm=hg.NORM_NONE)
-    torch.cuda.synchronize()
-    Hn = W.h_soa_to_aos(Hs[:, idx].contiguous().cpu()).numpy()
-    print("C3 sampled sks", check_parity(Hn, s, d, "sks"))
+    tot = {m: {"n": 0, "over_1e-3px": 0, "max_elem_ratio": 0.0, "max_reproj": 0.0, "max_reproj_over_S_on_those": 0.0} for m in ("aca", "sks")}
+
+    def check(m, a, Hn, s, d):
+        return m, check_h_parity_lazy(Hn, s, d, oracle.solve(ORACLE[m], s, d), oracle.dlt, label="%s slab at %d" % (m, a))
+
+    # the comparisons are numpy on 4M-set slabs (they release the GIL): a few slabs are checked side by side while the next is copied
+    from concurrent.futures import ThreadPoolExecutor
+    pending = []
+    with ThreadPoolExecutor(max_workers=6) as pool:
+        for a in range(0, n, slab):
+            s = W.to_aos(src[:, a:a + slab].contiguous()).cpu().numpy()
+            d = W.to_aos(dst[:, a:a + slab].contiguous()).cpu().numpy()
+            for m, Hm in (("aca", Ha), ("sks", Hs)):
+                pending.append(pool.submit(check, m, a, W.h_soa_to_aos(Hm[:, a:a + slab]).cpu().numpy(), s, d))
+            while len(pending) > 8:
+                m, st = pending.pop(0).result()                  # re-raises an assertion of that slab
+                t = tot[m]
+                t["n"] += st["n"]; t["over_1e-3px"] += st["over_1e-3px"]
+                for k in ("max_elem_ratio", "max_reproj", "max_reproj_over_S_on_those"):
+                    t[k] = max(t[k], st[k])
+        for f in pending:
+            m, st = f.result()
+            t = tot[m]
+            t["n"] += st["n"]; t["over_1e-3px"] += st["over_1e-3px"]
+            for k in ("max_elem_ratio", "max_reproj", "max_reproj_over_S_on_those"):
+                t[k] = max(t[k], st[k])
+    assert tot["aca"]["n"] == n and tot["sks"]["n"] == n
+    print("C3 every set", tot)
 
 
 def test_bench_line_carries_the_contract_keys():

@@ -882,7 +882,7 @@ def main():
     if tfile.exists():
         try:
             tr = json.loads(tfile.read_text())
-            src_note = "profiles/roofline_traffic.json (committed round-2 ncu --set full captures, dram__bytes_read.sum + dram__bytes_write.sum per launch); not measured in this run"
+            src_note = "profiles/roofline_traffic.json (committed ncu --set full captures of rounds 2-3, dram__bytes_read.sum + dram__bytes_write.sum per launch); not measured in this run"
             if n == 1 << LOG2N:
                 line["roofline"]["traffic"] = tr.get("aca_c3_dram_bytes_per_launch")
                 line["roofline"]["traffic_source"] = src_note
